@@ -1,0 +1,141 @@
+/*
+ * mdpd.h -- C-ABI of the B200-native mDPD timestep library (libmdpd_b200.so).
+ *
+ * One full velocity-Verlet timestep of many-body dissipative particle dynamics for fluid and frozen
+ * wall particles on ONE GPU (sm_100a), as stated in arxiv/paper_1903_10134:
+ *   - pair forces F = F^R + F^D + F^C, weight functions, fluctuation-dissipation   PAPER.md L75   (sec. 2.1)
+ *   - mDPD conservative force, Eq. (1), and the many-body density rho_i
+ *   - velocity-Verlet order x -> rho -> f -> v                                      PAPER.md L125-133 (Algorithm 1)
+ *   - body-force driving, dt = 0.01                                                 PAPER.md L186  (sec. 5.1)
+ *   - frozen ("fixed") solid wall particles                                         PAPER.md L162  (sec. 4.2)
+ * and the readings R1..R18 of DESIGN.md section 3 where the paper is silent (random-force 1/sqrt(dt), the pair
+ * hash, bounce-back at a voxel mask, ...).
+ *
+ * Conventions
+ *   - Every function returns int: MDPD_OK (0) or a negative error code.  Nothing throws, nothing exits.
+ *     mdpd_last_error(h) returns a NUL-terminated description owned by the handle.
+ *   - "host or device" pointers: any pointer cudaMemcpy(..., cudaMemcpyDefault) accepts.  The library copies; the
+ *     caller keeps ownership of everything it passes in.
+ *   - All device work is enqueued on the stream given to mdpd_create (0 = legacy default stream).
+ *   - A handle is not thread-safe.  One handle = one simulation on one device.
+ *   - There is no CPU fallback: without a CUDA device mdpd_create fails with MDPD_ECUDA.
+ */
+#ifndef MDPD_H_
+#define MDPD_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MDPD_OK 0
+#define MDPD_EINVAL (-1)    /* bad argument / unsupported parameter value                         */
+#define MDPD_ENOMEM (-2)    /* workspace too small or allocation failed                           */
+#define MDPD_ECUDA (-3)     /* a CUDA runtime call failed (text in mdpd_last_error)               */
+#define MDPD_EOVERFLOW (-4) /* neighbour-list capacity exceeded: raise mdpd_params.max_neigh      */
+#define MDPD_ESTATE (-5)    /* call order (e.g. step before load_particles)                       */
+#define MDPD_ENAN (-6)      /* a non-finite coordinate appeared                                   */
+#define MDPD_EINSOLID (-7)  /* fluid particle(s) start inside a solid voxel                       */
+
+typedef struct mdpd_ctx mdpd_ctx; /* opaque */
+
+/* Plain-old-data; copied by mdpd_set_params.  Units: rc = 1, mass = 1, kT = 1 (DPD units). */
+typedef struct {
+  float box[3];           /* periodic box [0,Lx) x [0,Ly) x [0,Lz); each L >= 3 (rc + skin)                           */
+  float rc, rd;           /* force and density cut-offs, rd <= rc (1.0, 0.75)      */
+  float A, B;             /* Eq. (1): attractive A < 0, many-body repulsive B > 0 (-40, 25)   */
+  float gamma, sigma;     /* dissipative / random amplitudes, sigma^2 = 2 gamma kT (4.5, 3.0)           */
+  float kT;               /* informational: if > 0 the library checks |sigma^2 - 2 gamma kT| <= 1e-3 sigma^2          */
+  float s;                /* exponent of wR = (1 - r/rc)^s; only s = 1 is implemented          PAPER.md L75 (R15)     */
+  float mass, dt;         /* particle mass (1), timestep (0.01)         */
+  float g[3];             /* body acceleration on fluid particles         */
+  float skin;             /* Verlet-list skin (default 0.25); list radius = rc + skin; rebuild when the largest
+                             displacement since the last build exceeds skin/2                   DESIGN.md R3, R4      */
+  uint32_t seed;          /* seed of the pair hash      */
+  uint32_t max_neigh;     /* total list capacity per particle (near + far part); 0 = automatic                       */
+  uint32_t reorder_every; /* Morton reorder every N list rebuilds; only 0/1 (= every rebuild) is implemented (R16)    */
+  uint32_t flags;         /* MDPD_FLAG_* */
+} mdpd_params;
+
+#define MDPD_FLAG_NO_GRAPH 1u /* launch kernels one by one instead of replaying the captured CUDA graph */
+
+/* Create a handle on CUDA device `device`; `cuda_stream` is a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream)
+ * or NULL for the default stream.  The handle must be destroyed with mdpd_destroy. */
+int mdpd_create(mdpd_ctx** out, int device, void* cuda_stream);
+int mdpd_destroy(mdpd_ctx* h);
+
+/* Validate and store parameters.  Before load_particles: any field.  After load_particles only g, dt, seed, A, B,
+ * gamma, sigma, kT may change (box, cut-offs, skin, capacities are frozen: MDPD_ESTATE otherwise). */
+int mdpd_set_params(mdpd_ctx* h, const mdpd_params* p);
+
+/* Device bytes needed for n particles (+ an optional mask of mask_dims = {nx, ny, nz} voxels).  Returns 0 on bad input. */
+size_t mdpd_workspace_bytes(const mdpd_params* p, uint64_t n, int has_mask, const uint32_t mask_dims[3]);
+
+/* Give the library its device memory: `dev_ptr` (256-byte aligned, >= mdpd_workspace_bytes) is OWNED BY THE CALLER
+ * (e.g. a torch uint8 tensor) and must outlive the handle.  If never called, load_particles allocates with cudaMalloc
+ * and mdpd_destroy frees that allocation. */
+int mdpd_set_workspace(mdpd_ctx* h, void* dev_ptr, size_t bytes);
+
+/* Load n particles.  pos, vel: [n][3] float32, host or device.  type: [n] uint8 (0 = fluid, 1 = frozen wall) or NULL
+ * (all fluid).  The tag of a particle is its index in this call and is permanent.  Positions are wrapped into the box;
+ * frozen particles get v = 0.  Builds the cell list / neighbour list and evaluates rho and f at step index 0.
+ * n = 0 is allowed.  Synchronises the stream. */
+int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* vel, const uint8_t* type);
+
+/* Optional voxel mask for the no-slip bounce-back (R7): mask[nz][ny][nx] uint8, 1 = solid, host or device;
+ * dims = {nx, ny, nz}; nx * voxel == Lx etc.  NULL clears the mask.  Call after load_particles (the workspace must have
+ * been sized with the mask).  Returns MDPD_EINSOLID if a fluid particle lies in a solid voxel (count in last_error). */
+int mdpd_load_wall_mask(mdpd_ctx* h, const uint8_t* mask, const uint32_t dims[3], float voxel);
+
+/* Advance nsteps velocity-Verlet steps (Algorithm 1).  Asynchronous on the stream: device-side
+ * faults (list overflow, NaN) are latched and reported by the next synchronising call (get_state, get_counters). */
+int mdpd_step(mdpd_ctx* h, uint32_t nsteps);
+
+/* Copy the state out in TAG order.  pos, vel, force: [n][3] float32; rho: [n] float32; any pointer may be NULL; host or
+ * device.  vel are the full-step velocities; force and rho are those of the last force evaluation.  Forces on frozen
+ * particles are reported only after mdpd_compute_forces (the step path does not compute them: they are never used).
+ * Synchronises the stream and returns a latched device fault if there is one. */
+int mdpd_get_state(mdpd_ctx* h, float* pos, float* vel, float* force, float* rho, uint64_t* step);
+
+/* Checkpoint / resume: set the step index used by the hash (forces are NOT recomputed; call mdpd_compute_forces). */
+int mdpd_set_step_counter(mdpd_ctx* h, uint64_t step);
+
+/* ---- parity / diagnostics exports (the GPU-vs-oracle comparison needs them) ---- */
+
+/* rho and f (on every particle, frozen ones included) from the current x, v at the current step index. */
+int mdpd_compute_forces(mdpd_ctx* h);
+
+/* All tag pairs (a < b) with r < rcut, found through the Verlet list with the kernels' own fp32 predicate
+ * (r^2 < rcut^2); rcut <= rc + skin.  For rcut > rc the result is complete only right after a list build
+ * (load_particles, or any step that rebuilt).  *count receives the number found; up to cap pairs are written
+ * to `pairs` ([cap][2] uint32, HOST memory), sorted lexicographically. */
+int mdpd_get_pairs(mdpd_ctx* h, float rcut, uint64_t* count, uint32_t* pairs, uint64_t cap);
+
+/* Run the DEVICE hash kernel: out[q] = HASH(min(pairs[q]), max(pairs[q]), step, seed of the handle).
+ * pairs: [npairs][2] uint32, out: [npairs] uint32, host or device. */
+int mdpd_rng_fill(mdpd_ctx* h, uint64_t npairs, const uint32_t* pairs, uint32_t step, uint32_t* out);
+
+/* out[0] steps done, [1] list rebuilds, [2] bounce-back events, [3] longest neighbour list (near + far) at the last
+ * build, [4] sum of list lengths at the last build, [5] list-overflow events, [6] NaN events, [7] kernels launched
+ * by this handle so far.  Synchronises the stream. */
+int mdpd_get_counters(mdpd_ctx* h, uint64_t out[8]);
+
+const char* mdpd_last_error(const mdpd_ctx* h);
+
+/* ---- measurement: per-kernel device times of the step path (CUDA events on the handle's stream) ---- */
+#define MDPD_PROF_SLOTS 16
+/* Start bracketing every kernel this handle launches with a pair of CUDA events. */
+int mdpd_profile_begin(mdpd_ctx* h);
+/* Stop, synchronise the stream and return, per kernel slot, the summed device time [ms] and the launch count since
+ * mdpd_profile_begin.  Slots past the last named one stay 0.  (Kernels of the rebuild chain are launched every step
+ * and return at once when the displacement trigger did not fire: their launch count includes those.) */
+int mdpd_profile_end(mdpd_ctx* h, double ms[MDPD_PROF_SLOTS], uint64_t launches[MDPD_PROF_SLOTS]);
+/* Name of a kernel slot ("k_force", "k_density", ...; "" past the last one).  Static storage. */
+const char* mdpd_profile_name(int slot);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MDPD_H_ */
