@@ -1,0 +1,334 @@
+#!/usr/bin/env python
+"""bench.py -- particle-timesteps/s of the full mDPD timestep on B200 (BASELINE.json metric), one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 4a|4b|0|1|2|3] [--impl ours|reference]
+
+A "step" is one full velocity-Verlet mDPD timestep (Algorithm 1): integrate + bounce-back +
+rebuild trigger, [cell binning + Morton sort + Verlet list when the trigger fires], density pass, pair-force pass.
+The timed region is K consecutive steps enqueued by ONE mdpd_step(h, K) call, bracketed by barrier + synchronize and
+CUDA events on the launching stream; list rebuilds that fall into the window are included.
+
+* value      : N_particles * K / t with the state already resident in HBM.
+* e2e        : the same metric through the C-ABI with HOST buffers: mdpd_load_particles(pinned host arrays) ->
+               mdpd_step(K) -> mdpd_get_state(pinned host arrays), host<->device copies inside the timed region.
+* roofline   : dominant kernel's algorithmic bytes per launch / its mean CUDA-event duration.
+* cpu_baseline / --impl reference : the fp64 oracle (oracle/, as it stands, serial C) on a bounded sample.
+* N > 1      : "replicas only": every rank runs an independent replica of the workload, no collective on
+               the data path; value = all ranks' particle-steps / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "particle-timesteps/sec per mDPD step on 1 B200"
+UNIT = "particle-steps/s"
+EQUILIBRATE = 200   # untimed steps after loading the random state (the paper equilibrates before timing)
+
+
+def workload_name(w, n):
+    return {"4a": f"config 4a: periodic mDPD liquid 175^3, density 6, {n} particles",
+            "4b": f"config 4b: periodic mDPD liquid 55^3, density 6, {n} particles",
+            "0": f"config 0: periodic mDPD liquid 10^3, {n} particles",
+            "1": f"config 1: liquid-vapor slab 40x20x20, {n} particles",
+            "2": f"config 2: Poiseuille flow between frozen walls 20^3, {n} particles",
+            "3": f"config 3: voxelised pore network 64^3, {n} particles"}[w]
+
+
+# --------------------------------------------------------------------------------------------- clocks sampling
+class ClockSampler:
+    """Samples SM clock and throttle reasons of one GPU through NVML while the timed region runs."""
+
+    def __init__(self, index, period=0.05):
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._th = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception as e:  # noqa: BLE001
+            self._nv = None
+            self.err = repr(e)
+
+    _BITS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+             0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost",
+             0x100: "display_clock_setting"}
+
+    def _run(self):
+        nv = self._nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self._h))
+                for bit, name in self._BITS.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:  # noqa: BLE001
+                pass
+            self._stop.wait(self.period)
+
+    def __enter__(self):
+        if self._nv is not None:
+            self._th = threading.Thread(target=self._run, daemon=True)
+            self._th.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._th is not None:
+            self._th.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def physical_gpu_index(local):
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local])
+        except Exception:  # noqa: BLE001
+            return local
+    return local
+
+
+# ------------------------------------------------------------------------------------------------ oracle legs
+def oracle_sample_edge(budget_particle_steps):
+    """Edge of the cubic density-6 sub-box whose particle count fits the budget (6 <= edge <= 40)."""
+    edge = int(np.floor((budget_particle_steps / 6.0) ** (1.0 / 3.0)))
+    return int(min(40, max(6, edge)))
+
+
+def run_oracle_sample(workload, nsteps, edge, warm=0):
+    """Times `nsteps` timesteps of the fp64 oracle on a bounded sample of the workload.  Returns (rate, n, seconds)."""
+    import mdpd_workloads as wl
+    from oracle.mdpd_ref import RefSim
+    if workload in ("4a", "4b"):
+        c = wl.make_liquid(float(edge), seed=wl.BASE_SEED + 4)
+        sample = f"periodic mDPD liquid {edge}^3 at density 6 ({len(c['pos'])} particles), same parameters"
+    else:
+        c = wl.make_config(int(workload))
+        sample = f"the full config {workload} ({len(c['pos'])} particles)"
+    s = RefSim(c["params"])
+    s.load_particles(c["pos"].astype(np.float64), c["vel"].astype(np.float64), c["type"])
+    if c.get("mask") is not None:
+        s.load_wall_mask(c["mask"], c["voxel"])
+    if warm:
+        s.step(warm)
+    t0 = time.perf_counter()
+    s.step(nsteps)
+    dt = time.perf_counter() - t0
+    n = len(c["pos"])
+    s.close()
+    return n * nsteps / dt, n, dt, sample
+
+
+def main_reference(args, rank, world):
+    """--impl reference: the oracle as it stands on the host cores (serial C, 1 thread); rank 0 only."""
+    if rank != 0:
+        return 0
+    K, W = args.steps, args.warmup
+    budget = 150.0 * 4.0e5 / max(1, K + W)      # ~150 s of oracle time at ~4e5 particle-steps/s per core
+    edge = oracle_sample_edge(budget)
+    rate, n, dt, sample = run_oracle_sample(args.workload, K, edge, warm=W)
+    line = {"metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus, "steps": K, "warmup": W,
+            "ms_per_step": 1e3 * dt / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "impl": "reference",
+            "config": {"workload": workload_name(args.workload, "sampled"), "sample": sample},
+            "cpu_baseline": {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
+                             "sample": f"{sample}; {K} steps per run, one timestep per step"},
+            "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# --------------------------------------------------------------------------------------------------- our arm
+def algorithmic_bytes(kernel, n, n_list, n_near):
+    """Bytes one launch must move through HBM if every gathered neighbour load hits cache (DESIGN.md section 7,
+    SURVEY.md 8(d)): per particle, density = pos 16 + 4 n_near + rho 4; force = pos 16 + (vel, rho) 16 + 4 n_list +
+    force 16; integrate = pos r/w 32 + vel r/w 32 + force 16 + xbuild 16."""
+    per = {"k_density": 16 + 4 * n_near + 4, "k_force": 16 + 16 + 4 * n_list + 16, "k_integrate": 96,
+           "k_build_list": 16 + 4 * n_list + 4}.get(kernel)
+    return None if per is None else per * n
+
+
+def main_ours(args, rank, world, local):
+    import torch
+    import torch.distributed as dist
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the mDPD path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    import mdpd_workloads as wl
+    import paper_1903_10134_b200 as pk
+    from paper_1903_10134_b200.build import build as build_cuda
+    if rank == 0:
+        build_cuda()
+    if world > 1:
+        dist.barrier()
+
+    K, W = args.steps, max(3, args.warmup)
+    c = wl.make_config(args.workload if args.workload in ("4a", "4b") else int(args.workload))
+    n = len(c["pos"])
+    md = None if c.get("mask") is None else c["mask"].shape[::-1]
+    # pinned host buffers (inputs of the e2e leg, outputs of get_state)
+    h_pos = torch.from_numpy(c["pos"]).pin_memory()
+    h_vel = torch.from_numpy(c["vel"]).pin_memory()
+    h_typ = torch.from_numpy(c["type"]).pin_memory()
+    o_pos = torch.empty((n, 3), dtype=torch.float32).pin_memory()
+    o_vel = torch.empty((n, 3), dtype=torch.float32).pin_memory()
+
+    sim = pk.Simulation(c["params"], device=local)
+
+    def load():
+        sim.load_particles(h_pos, h_vel, h_typ, mask_dims=md)
+        if c.get("mask") is not None:
+            sim.load_wall_mask(c["mask"], c["voxel"])
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    load()
+    sim.step(EQUILIBRATE)
+    sim.step(W)
+    sim.counters()                                 # synchronises; raises on a latched device fault
+    c0 = sim.counters()
+
+    # ---- timed region: K steps, state resident in HBM --------------------------------------------------------
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    with ClockSampler(physical_gpu_index(local)) as clk:
+        e0.record()
+        sim.step(K)
+        e1.record()
+        torch.cuda.synchronize()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    c1 = sim.counters()
+    launches = c1["launches"] - c0["launches"]
+    rebuilds = c1["rebuilds"] - c0["rebuilds"]
+    n_list = c1["sum_nbr"] / n
+    n_near = c1["sum_near"] / n
+
+    # ---- per-kernel CUDA-event times over another K steps (same stream) --------------------------------------
+    sim.profile_begin()
+    sim.step(K)
+    prof = sim.profile_end()
+    tot = sum(v[0] for v in prof.values())
+    hot = [k for k in prof if k != "other"]
+    dom = max(hot, key=lambda k: prof[k][0])
+    kernels = {k: {"ms_total": round(prof[k][0], 4), "launches": prof[k][1],
+                   "share": round(prof[k][0] / tot, 4) if tot else None} for k in prof}
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:  # noqa: BLE001
+        pass
+    peak_gbs, peak_src = (peaks["hbm_gbs"], "MEASURED_PEAKS.json hbm_gbs") if "hbm_gbs" in peaks else \
+        (6650.0, "B200_PROFILING.md fallback")
+    roof = {"bound": "hbm", "kernel": dom, "peak": peak_gbs, "unit": "GB/s", "peak_source": peak_src,
+            "traffic": None}
+    ab = algorithmic_bytes(dom, n, n_list, n_near)
+    dom_ms = prof[dom][0] / max(1, prof[dom][1])
+    if ab is not None and dom_ms > 0:
+        roof.update(achieved=ab / (dom_ms * 1e-3) / 1e9, algorithmic_bytes_per_launch=ab,
+                    ms_per_launch=dom_ms)
+        roof["frac"] = roof["achieved"] / peak_gbs
+    also = {}
+    for k in ("k_density", "k_force", "k_integrate"):
+        b = algorithmic_bytes(k, n, n_list, n_near)
+        t = prof[k][0] / max(1, prof[k][1])
+        if b and t > 0:
+            also[k] = {"achieved_gbs": round(b / (t * 1e-3) / 1e9, 1), "frac": round(b / (t * 1e-3) / 1e9 / peak_gbs, 4),
+                       "ms_per_launch": round(t, 5)}
+    roof["per_kernel"] = also
+
+    # ---- e2e: host buffers -> C-ABI -> host buffers, copies inside the timed region --------------------------
+    barrier()
+    t0 = time.perf_counter()
+    load()                                          # H2D of pos, vel, type (+ mask) from pinned memory
+    sim.step(K)
+    sim.get_state(out={"pos": o_pos, "vel": o_vel}, force=False, rho=False)   # D2H, synchronises
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    barrier()
+    h2d = n * (12 + 12 + 1) + (int(np.prod(md)) if md is not None else 0)
+    d2h = n * 24
+
+    # ---- max over ranks ---------------------------------------------------------------------------------------
+    if world > 1:
+        t = torch.tensor([ms, e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, e2e_s = float(t[0]), float(t[1])
+    value = world * n * K / (ms * 1e-3)
+    e2e_v = world * n * K / e2e_s
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": workload_name(args.workload, n), "particles_per_gpu": n,
+                       "parallelism": "replicas only" if world > 1 else "1 gpu",
+                       "equilibration_steps": EQUILIBRATE, "skin": c["params"]["skin"],
+                       "l2": "inputs larger than L2" if n * 700 > 126e6 * 2 else "inputs fit L2 (small case)",
+                       "rebuilds_in_window": rebuilds, "mean_list_len": round(n_list, 2),
+                       "mean_near_len": round(n_near, 2), "max_list_len": c1["max_nbr"]},
+            "e2e": {"value": e2e_v, "unit": UNIT, "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
+                    "note": f"one job = load_particles(host) + {K} steps + get_state(host); bytes are per job / {K}"},
+            "gpu_launches": launches, "clocks": clk.summary(), "roofline": roof, "kernels": kernels}
+
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        edge = oracle_sample_edge(20.0 * 4.0e5 / 20)          # ~20 s: 20 steps of a ~4e5-particle box
+        rate, ns, dt, sample = run_oracle_sample(args.workload, 20, edge)
+        line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                "sample": f"{sample}; 20 timesteps in {dt:.1f} s (serial C, fp64)"}
+    sim.close()
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="4a", choices=["4a", "4b", "0", "1", "2", "3"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        return main_reference(args, rank, world)
+    if world == 1 and args.gpus > 1:
+        print(f"bench.py: --gpus {args.gpus} needs torchrun (one rank per GPU); running 1 replica", file=sys.stderr)
+    return main_ours(args, rank, world, local)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

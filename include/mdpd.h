@@ -118,8 +118,9 @@ int mdpd_get_pairs(mdpd_ctx* h, float rcut, uint64_t* count, uint32_t* pairs, ui
 int mdpd_rng_fill(mdpd_ctx* h, uint64_t npairs, const uint32_t* pairs, uint32_t step, uint32_t* out);
 
 /* out[0] steps done, [1] list rebuilds, [2] bounce-back events, [3] longest neighbour list (near + far) at the last
- * build, [4] sum of list lengths at the last build, [5] list-overflow events, [6] NaN events, [7] kernels launched
- * by this handle so far.  Synchronises the stream. */
+ * build, [4] sum over particles of the list lengths (near + far) at the last build, [5] the same for the near part
+ * alone, [6] device fault events (list overflows + non-finite coordinates; also latched as an error code),
+ * [7] kernels launched by this handle so far.  Synchronises the stream. */
 int mdpd_get_counters(mdpd_ctx* h, uint64_t out[8]);
 
 const char* mdpd_last_error(const mdpd_ctx* h);

@@ -40,7 +40,7 @@ struct Ctl {
   unsigned err;       // ERR_* bits, latched
   unsigned max_nbr;   // longest list at the last build
   unsigned pair_count_lo;
-  unsigned long long steps, rebuilds, bounces, sum_nbr, overflow, nan_events, pair_count, pad;
+  unsigned long long steps, rebuilds, bounces, sum_nbr, overflow, nan_events, pair_count, sum_near;
 };
 
 struct DevP {  // passed by value to every kernel
@@ -466,11 +466,13 @@ __global__ void __launch_bounds__(TPB) k_build_list(const DevP p) {
   unsigned tot = nn + nf;
   unsigned wmax = __reduce_max_sync(0xffffffffu, tot);
   unsigned wsum = __reduce_add_sync(0xffffffffu, tot);
+  unsigned wnear = __reduce_add_sync(0xffffffffu, nn);
   unsigned wover = __any_sync(0xffffffffu, over);
   if ((threadIdx.x & 31) == 0) {
     Ctl* c = p.ctl;
     atomicMax(&c->max_nbr, wmax);
     atomicAdd(&c->sum_nbr, (unsigned long long)wsum);
+    atomicAdd(&c->sum_near, (unsigned long long)wnear);
     if (wover) {
       atomicOr(&c->err, ERR_OVERFLOW);
       atomicAdd(&c->overflow, 1ull);
@@ -482,6 +484,7 @@ __global__ void k_reset_list_stats(const DevP p) {
   if (!p.ctl->rebuild) return;
   p.ctl->max_nbr = 0;
   p.ctl->sum_nbr = 0;
+  p.ctl->sum_near = 0;
 }
 
 // ----------------------------------------------------------------------------------------------------------------
@@ -1169,8 +1172,8 @@ int mdpd_get_counters(mdpd_ctx* h, uint64_t out[8]) {
   out[2] = c->bounces;
   out[3] = c->max_nbr;
   out[4] = c->sum_nbr;
-  out[5] = c->overflow;
-  out[6] = c->nan_events;
+  out[5] = c->sum_near;
+  out[6] = c->overflow + c->nan_events;
   out[7] = h->launches;
   return rc;
 }
