@@ -211,7 +211,7 @@ def main_ours(args, rank, world, local):
         torch.cuda.synchronize()
 
     load()
-    sim.step(EQUILIBRATE)
+    sim.step(args.equilibrate)
     sim.step(W)
     sim.counters()                                 # synchronises; raises on a latched device fault
     c0 = sim.counters()
@@ -290,7 +290,7 @@ def main_ours(args, rank, world, local):
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": workload_name(args.workload, n), "particles_per_gpu": n,
                        "parallelism": "replicas only" if world > 1 else "1 gpu",
-                       "equilibration_steps": EQUILIBRATE, "skin": c["params"]["skin"],
+                       "equilibration_steps": args.equilibrate, "skin": c["params"]["skin"],
                        "l2": "inputs larger than L2" if n * 700 > 126e6 * 2 else "inputs fit L2 (small case)",
                        "rebuilds_in_window": rebuilds, "mean_list_len": round(n_list, 2),
                        "mean_near_len": round(n_near, 2), "max_list_len": c1["max_nbr"]},
@@ -319,6 +319,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="4a", choices=["4a", "4b", "0", "1", "2", "3"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--equilibrate", type=int, default=EQUILIBRATE, help="untimed steps after loading")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
