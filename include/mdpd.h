@@ -54,7 +54,7 @@ typedef struct {
   float skin;             /* Verlet-list skin (default 0.25); list radius = rc + skin; rebuild when the largest
                              displacement since the last build exceeds skin/2                   DESIGN.md R3, R4      */
   uint32_t seed;          /* seed of the pair hash      */
-  uint32_t max_neigh;     /* total list capacity per particle (near + far part); 0 = automatic                       */
+  uint32_t max_neigh;     /* list capacity per particle, <= 128; 0 = automatic                                       */
   uint32_t reorder_every; /* Morton reorder every N list rebuilds; only 0/1 (= every rebuild) is implemented (R16)    */
   uint32_t flags;         /* MDPD_FLAG_* */
 } mdpd_params;
@@ -117,9 +117,9 @@ int mdpd_get_pairs(mdpd_ctx* h, float rcut, uint64_t* count, uint32_t* pairs, ui
  * pairs: [npairs][2] uint32, out: [npairs] uint32, host or device. */
 int mdpd_rng_fill(mdpd_ctx* h, uint64_t npairs, const uint32_t* pairs, uint32_t step, uint32_t* out);
 
-/* out[0] steps done, [1] list rebuilds, [2] bounce-back events, [3] longest neighbour list (near + far) at the last
- * build, [4] sum over particles of the list lengths (near + far) at the last build, [5] the same for the near part
- * alone, [6] device fault events (list overflows + non-finite coordinates; also latched as an error code),
+/* out[0] steps done, [1] list rebuilds, [2] bounce-back events, [3] longest neighbour list at the last
+ * build, [4] sum over particles of the list lengths at the last build, [5] most particles staged in shared memory
+ * by one tile (tile + halo) at the last build, [6] device fault events (list overflows + non-finite coordinates; also latched as an error code),
  * [7] kernels launched by this handle so far.  Synchronises the stream. */
 int mdpd_get_counters(mdpd_ctx* h, uint64_t out[8]);
 

@@ -104,7 +104,7 @@ def _ptr(a):
     return a.data_ptr()  # torch tensor
 
 
-COUNTER_NAMES = ("steps", "rebuilds", "bounces", "max_nbr", "sum_nbr", "sum_near", "faults", "launches")
+COUNTER_NAMES = ("steps", "rebuilds", "bounces", "max_nbr", "sum_nbr", "max_staged", "faults", "launches")
 
 
 class Simulation:

@@ -5,9 +5,10 @@
 // specification: DESIGN.md sections 3 and 4.  This file shares nothing with oracle/ (the fp64 CPU oracle).
 //
 // Device state: pos float4 = (x, y, z, bits(tag | type << 31)), vel float4 = (vx, vy, vz, rho),
-// both double-buffered for the Morton counting sort; force float4; xbuild float4 (positions at the last list build);
-// Verlet list split in a near part (r < rd + skin at build: all the density pass needs) and a far part, both stored
-// column-major ([k][i]) so that a warp reads consecutive i at fixed k in one coalesced request.
+// both double-buffered for the counting sort into tiles of cells (tiles along the Z-curve, cells x-fastest inside a
+// tile); force float4; xbuild float4 (positions at the last list build); Verlet list of 16-bit indices into the
+// tile's staged shared-memory array, split in a near part (r < rd + skin at build: all the density pass needs) and a
+// far part, both stored column-major ([k][i]) so that a warp reads consecutive i at fixed k in one coalesced request.
 #include "mdpd.h"
 
 #include <cuda_runtime.h>
@@ -24,6 +25,7 @@ namespace {
 
 constexpr unsigned ERR_OVERFLOW = 1u;
 constexpr unsigned ERR_NAN = 2u;
+constexpr unsigned ERR_TILE = 4u;  // a tile + halo does not fit the shared-memory capacity
 constexpr int TPB = 128;           // threads per block of the per-particle kernels
 constexpr int SCAN_TPB = 256;      // scan: 256 threads x 8 items
 constexpr int SCAN_ITEMS = 8;
@@ -39,8 +41,17 @@ struct Ctl {
   unsigned step;      // index k of the time level of the last force evaluation (hash input)
   unsigned err;       // ERR_* bits, latched
   unsigned max_nbr;   // longest list at the last build
-  unsigned pair_count_lo;
-  unsigned long long steps, rebuilds, bounces, sum_nbr, overflow, nan_events, pair_count, sum_near;
+  unsigned max_halo;  // most particles in a tile + halo at the last build
+  unsigned max_own;   // most particles in a tile at the last build
+  unsigned pad0;
+  unsigned long long steps, rebuilds, bounces, sum_nbr, overflow, nan_events, pair_count, pad1;
+};
+
+struct TileInfo {  // one CTA of the list / density / force passes
+  int c0x, c0y, c0z;   // first cell
+  int ex, ey, ez;      // extent in cells (<= 4 each)
+  unsigned rank0;      // sorted rank of the tile's first cell; its cells are ranks rank0 .. rank0 + ncell_own - 1
+  unsigned ncell_own;  // ex * ey * ez
 };
 
 struct DevP {  // passed by value to every kernel
@@ -55,21 +66,22 @@ struct DevP {  // passed by value to every kernel
   unsigned* scan_bsum;   // [nblocks of the scan]
   unsigned* pcell;       // [N] Morton rank of the particle's cell (old order)
   unsigned* order;       // [N] old index of the particle that goes to sorted slot s (unordered inside a cell)
-  unsigned* nbr_near;    // [cap_near][N]
-  unsigned* nbr_far;     // [cap_far][N]
-  unsigned* nnbr;        // [N] near | far << 16
+  uint4* nbr;                // [cap / 8][N] chunks of 8 16-bit staged-slot indices, padded with the sentinel slot
+  unsigned short* self_loc;  // [N] staged slot of the particle itself
+  unsigned* nnbr;            // [N] list length
+  const TileInfo* tiles;     // [ntiles]
   const unsigned char* mask;
   Ctl* ctl;
   // sizes
-  unsigned N, ncell, cap_near, cap_far;
+  unsigned N, ncell, cap, ntiles, tile_cap;
   int ncx, ncy, ncz;
   int mx, my, mz;
   // geometry
   float Lx, Ly, Lz;
   float icx, icy, icz;  // 1 / cell edge
+  float edge_x, edge_y, edge_z;
   float inv_voxel;
-  float rlist2, rnear2, rc2, rd2;
-  float margin;  // particles farther than this from every box face need no minimum-image test
+  float rlist2, rc2, rd2;
   // physics
   float inv_rc, inv_rd, Krho;
   float A, B, gamma, sig_c;  // sig_c = sigma * sqrt(3) * 2^-23 / sqrt(dt)
@@ -80,16 +92,21 @@ struct DevP {  // passed by value to every kernel
 };
 
 __device__ __forceinline__ unsigned f2u(float f) { return __float_as_uint(f); }
+__device__ __forceinline__ unsigned smem_addr(const void* ptr) { return (unsigned)__cvta_generic_to_shared(ptr); }
+__device__ __forceinline__ void sts_u16(unsigned addr, unsigned v) {
+  asm volatile("st.shared.u16 [%0], %1;" ::"r"(addr), "h"((unsigned short)v) : "memory");
+}
+__device__ __forceinline__ unsigned lanemask_lt() {
+  unsigned m;
+  asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+  return m;
+}
 __device__ __forceinline__ float u2f(unsigned u) { return __uint_as_float(u); }
 
-__device__ __forceinline__ float minimg(float d, float L) {
-  const float h = 0.5f * L;
-  if (d > h) d -= L;
-  else if (d < -h) d += L;
-  return d;
-}
-
-__device__ __forceinline__ float wrap1(float x, float L) {  // |x - [0,L)| << L here (one step of drift)  R12
+// Positions are kept UNWRAPPED between list rebuilds (they leave [0, L) by at most skin / 2) so that a particle stays
+// geometrically inside the cell it was sorted into; they are wrapped when the sort runs, for the voxel-mask lookup
+// and on output (R12).
+__device__ __forceinline__ float wrap1(float x, float L) {  // |x - [0,L)| << L here
   if (x >= L) x -= L;
   else if (x < 0.0f) x += L;
   if (x >= L) x = 0.0f;
@@ -166,7 +183,7 @@ __global__ void k_unpack(DevP p, float* __restrict__ pos, float* __restrict__ ve
   const unsigned cur = p.ctl->cur;
   float4 x = p.pos[cur][i], v = p.vel[cur][i], f = p.force[i];
   unsigned tag = f2u(x.w) & 0x7FFFFFFFu;
-  if (pos) { pos[3 * tag] = x.x; pos[3 * tag + 1] = x.y; pos[3 * tag + 2] = x.z; }
+  if (pos) { pos[3 * tag] = wrap1(x.x, p.Lx); pos[3 * tag + 1] = wrap1(x.y, p.Ly); pos[3 * tag + 2] = wrap1(x.z, p.Lz); }
   if (vel) { vel[3 * tag] = v.x; vel[3 * tag + 1] = v.y; vel[3 * tag + 2] = v.z; }
   if (force) { force[3 * tag] = f.x; force[3 * tag + 1] = f.y; force[3 * tag + 2] = f.z; }
   if (rho) rho[tag] = v.w;
@@ -177,6 +194,9 @@ __global__ void k_count_in_solid(DevP p, unsigned* count) {
   if (i >= p.N) return;
   float4 x = p.pos[p.ctl->cur][i];
   if (f2u(x.w) >> 31) return;
+  x.x = wrap1(x.x, p.Lx);
+  x.y = wrap1(x.y, p.Ly);
+  x.z = wrap1(x.z, p.Lz);
   int ix = min((int)(x.x * p.inv_voxel), p.mx - 1), iy = min((int)(x.y * p.inv_voxel), p.my - 1),
       iz = min((int)(x.z * p.inv_voxel), p.mz - 1);
   if (p.mask[((size_t)iz * p.my + iy) * p.mx + ix]) atomicAdd(count, 1u);
@@ -206,13 +226,12 @@ __global__ void __launch_bounds__(TPB) k_integrate(const DevP p, int do_B, int d
         v.x += p.hdt_m * f.x;
         v.y += p.hdt_m * f.y;
         v.z += p.hdt_m * f.z;
-        float nx = wrap1(x.x + p.dt * v.x, p.Lx);
-        float ny = wrap1(x.y + p.dt * v.y, p.Ly);
-        float nz = wrap1(x.z + p.dt * v.z, p.Lz);
+        const float nx = x.x + p.dt * v.x, ny = x.y + p.dt * v.y, nz = x.z + p.dt * v.z;
         bool solid = false;
         if (HAS_MASK) {
-          int ix = min((int)(nx * p.inv_voxel), p.mx - 1), iy = min((int)(ny * p.inv_voxel), p.my - 1),
-              iz = min((int)(nz * p.inv_voxel), p.mz - 1);
+          const float wx = wrap1(nx, p.Lx), wy = wrap1(ny, p.Ly), wz = wrap1(nz, p.Lz);
+          int ix = min((int)(wx * p.inv_voxel), p.mx - 1), iy = min((int)(wy * p.inv_voxel), p.my - 1),
+              iz = min((int)(wz * p.inv_voxel), p.mz - 1);
           if (!(nx == nx && ny == ny && nz == nz)) ix = iy = iz = 0;
           solid = p.mask[((size_t)iz * p.my + iy) * p.mx + ix] != 0;
         }
@@ -227,7 +246,7 @@ __global__ void __launch_bounds__(TPB) k_integrate(const DevP p, int do_B, int d
           x.z = nz;
         }
         const float4 xb = p.xbuild[i];
-        float dx = minimg(x.x - xb.x, p.Lx), dy = minimg(x.y - xb.y, p.Ly), dz = minimg(x.z - xb.z, p.Lz);
+        const float dx = x.x - xb.x, dy = x.y - xb.y, dz = x.z - xb.z;  // unwrapped since the last build
         d2 = dx * dx + dy * dy + dz * dz;
         if (!(d2 < 1e30f)) {
           bad = 1;
@@ -298,6 +317,9 @@ __global__ void __launch_bounds__(TPB) k_cell_count(const DevP p) {
   unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= p.N) return;
   float4 x = p.pos[src][i];
+  x.x = wrap1(x.x, p.Lx);
+  x.y = wrap1(x.y, p.Ly);
+  x.z = wrap1(x.z, p.Lz);
   int cx = cell_coord(x.x, p.icx, p.ncx), cy = cell_coord(x.y, p.icy, p.ncy), cz = cell_coord(x.z, p.icz, p.ncz);
   unsigned c = p.cell_rank[((unsigned)cz * p.ncy + cy) * p.ncx + cx];
   p.pcell[i] = c;
@@ -398,7 +420,10 @@ __global__ void __launch_bounds__(TPB) k_permute(const DevP p) {
   const unsigned i = p.order[s];
   const unsigned c = p.pcell[i];
   const unsigned cs = p.cell_start[c], ce = p.cell_start[c + 1];
-  const float4 x = p.pos[src][i];
+  float4 x = p.pos[src][i];
+  x.x = wrap1(x.x, p.Lx);
+  x.y = wrap1(x.y, p.Ly);
+  x.z = wrap1(x.z, p.Lz);
   const unsigned tag = f2u(x.w) & 0x7FFFFFFFu;
   unsigned rank = 0;
   for (unsigned t = cs; t < ce; ++t) {
@@ -412,67 +437,303 @@ __global__ void __launch_bounds__(TPB) k_permute(const DevP p) {
 }
 
 // ----------------------------------------------------------------------------------------------------------------
-// a3: Verlet list (full list; near part r < rnear = rd + skin first, far part rnear <= r < rc + skin)
+// Tile staging.  A CTA owns one tile of up to 4 x 4 x 4 cells.  The tile and its one-cell halo
+// (<= 6 x 6 x 6 = 216 cells) are copied once into shared memory, cell by cell in halo order (x fastest), in
+// TILE-RELATIVE coordinates with the periodic shift folded in: no minimum-image arithmetic in any inner loop, and
+// pair separations are formed from small numbers (|x| < 8) whatever the box size.  The Verlet list stores 16-bit
+// indices into this staged array, so every neighbour access of the hot loops is a shared-memory load.
 // ----------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(TPB) k_build_list(const DevP p) {
-  if (!p.ctl->rebuild) return;
-  const unsigned cur = p.ctl->cur;
-  unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
-  unsigned nn = 0, nf = 0;
-  bool over = false;
-  if (i < p.N) {
-    const float4 xi = p.pos[cur][i];
-    const int cx = cell_coord(xi.x, p.icx, p.ncx), cy = cell_coord(xi.y, p.icy, p.ncy),
-              cz = cell_coord(xi.z, p.icz, p.ncz);
-    for (int dz = -1; dz <= 1; ++dz) {
-      int oz = cz + dz;
-      float sz = xi.z;
-      if (oz < 0) { oz += p.ncz; sz += p.Lz; }
-      else if (oz >= p.ncz) { oz -= p.ncz; sz -= p.Lz; }
-      for (int dy = -1; dy <= 1; ++dy) {
-        int oy = cy + dy;
-        float sy = xi.y;
-        if (oy < 0) { oy += p.ncy; sy += p.Ly; }
-        else if (oy >= p.ncy) { oy -= p.ncy; sy -= p.Ly; }
-        for (int dx = -1; dx <= 1; ++dx) {
-          int ox = cx + dx;
-          float sx = xi.x;
-          if (ox < 0) { ox += p.ncx; sx += p.Lx; }
-          else if (ox >= p.ncx) { ox -= p.ncx; sx -= p.Lx; }
-          const unsigned c = p.cell_rank[((unsigned)oz * p.ncy + oy) * p.ncx + ox];
-          const unsigned js = p.cell_start[c], je = p.cell_start[c + 1];
-          for (unsigned j = js; j < je; ++j) {
-            const float4 xj = p.pos[cur][j];
-            const float ddx = sx - xj.x, ddy = sy - xj.y, ddz = sz - xj.z;
-            const float r2 = ddx * ddx + ddy * ddy + ddz * ddz;
-            if (r2 < p.rlist2 && j != i) {
-              if (r2 < p.rnear2) {
-                if (nn < p.cap_near) p.nbr_near[(size_t)nn * p.N + i] = j;
-                else over = true;
-                ++nn;
-              } else {
-                if (nf < p.cap_far) p.nbr_far[(size_t)nf * p.N + i] = j;
-                else over = true;
-                ++nf;
-              }
-            }
-          }
-        }
+constexpr int HMAX = 216;                      // halo cells of the largest tile
+constexpr int HTAB = 224;                      // table size (HMAX + 1 rounded up)
+static_assert(HMAX + 1 <= HTAB, "halo table");
+constexpr unsigned QD = 24;                    // depth of the per-lane in-range queue of the force pass
+constexpr unsigned LCAP = 128;                 // per-particle list capacity
+constexpr unsigned LROW = LCAP + 8;            // row pitch of the list build's shared-memory rows (bank spread, 16-byte aligned)
+constexpr int SCH = 4;                         // candidate chunks (of 32) held in registers at a time
+constexpr int BATCH = 16;                      // own particles per row batch of the list build
+
+struct TileSmem {
+  float4* spos;      // [cap] (x_rel, y_rel, z_rel, bits(tag | type << 31))
+  float4* svel;      // [cap] (vx, vy, vz, rho)            (force pass only)
+  unsigned* hbase;   // [HTAB] first staged slot of halo cell h; hbase[nh] = number of staged particles
+  unsigned* hstart;  // [HTAB] global index of the first particle of halo cell h
+  unsigned short* queue;  // [QD][blockDim] (force pass only)
+};
+
+// queue_entries: 16-bit scratch entries behind the tables (force pass: QD per thread; list build: rows per warp)
+__host__ __device__ inline size_t tile_smem_bytes(unsigned cap, bool with_vel, size_t queue_entries) {
+  return (size_t)(cap + 1) * 16 * (with_vel ? 2 : 1) + 2 * HTAB * 4 + queue_entries * 2;  // + sentinel slot
+}
+
+__device__ __forceinline__ TileSmem carve_smem(unsigned char* raw, unsigned cap, bool with_vel) {
+  TileSmem s;
+  s.spos = (float4*)raw;
+  raw += (size_t)(cap + 1) * 16;
+  s.svel = (float4*)raw;
+  if (with_vel) raw += (size_t)(cap + 1) * 16;
+  s.hbase = (unsigned*)raw;
+  raw += HTAB * 4;
+  s.hstart = (unsigned*)raw;
+  raw += HTAB * 4;
+  s.queue = (unsigned short*)raw;
+  return s;
+}
+
+// coordinate of halo position hx in one dimension: wrapped cell index and the two addends of
+//   x_rel = (x + s1) + s2   (both additions exact for own-tile particles)
+__device__ __forceinline__ int halo_cell(int c0, int hx, int nc, float L, float o, float& s1, float& s2) {
+  int c = c0 + hx - 1;
+  if (c < 0) {            // image on the low side: only tiles with c0 == 0 (o == 0)
+    c += nc;
+    s1 = -L;
+    s2 = -o;
+  } else if (c >= nc) {   // image on the high side
+    c -= nc;
+    s1 = L - o;
+    s2 = 0.0f;
+  } else {
+    s1 = -o;
+    s2 = 0.0f;
+  }
+  return c;
+}
+
+__device__ __forceinline__ float tile_origin(int c0, float edge) { return floorf((float)c0 * edge * 64.0f) * (1.0f / 64.0f); }
+
+// Returns the number of staged particles, or 0xFFFFFFFF if the tile does not fit the shared-memory capacity
+// (nothing is staged then).  All threads of the CTA must call it.
+template <bool WITH_VEL>
+__device__ __forceinline__ unsigned stage_tile(const DevP& p, const TileInfo& T, const float4* __restrict__ pos,
+                                               const float4* __restrict__ vel, const TileSmem& sm) {
+  const int hxn = T.ex + 2, hyn = T.ey + 2, hzn = T.ez + 2;
+  const int nh = hxn * hyn * hzn;
+  const float ox = tile_origin(T.c0x, p.edge_x), oy = tile_origin(T.c0y, p.edge_y), oz = tile_origin(T.c0z, p.edge_z);
+  for (int h = threadIdx.x; h < nh; h += blockDim.x) {
+    const int hx = h % hxn, hy = (h / hxn) % hyn, hz = h / (hxn * hyn);
+    float a, b;
+    const int cx = halo_cell(T.c0x, hx, p.ncx, p.Lx, ox, a, b);
+    const int cy = halo_cell(T.c0y, hy, p.ncy, p.Ly, oy, a, b);
+    const int cz = halo_cell(T.c0z, hz, p.ncz, p.Lz, oz, a, b);
+    const unsigned r = p.cell_rank[((unsigned)cz * p.ncy + cy) * p.ncx + cx];
+    const unsigned s = p.cell_start[r];
+    sm.hstart[h] = s;
+    sm.hbase[h] = p.cell_start[r + 1] - s;
+  }
+  __syncthreads();
+  if (threadIdx.x < 32) {  // exclusive scan of the counts by warp 0
+    const int lane = threadIdx.x;
+    unsigned run = 0;
+    for (int b0 = 0; b0 < nh; b0 += 32) {
+      const int h = b0 + lane;
+      const unsigned c = h < nh ? sm.hbase[h] : 0u;
+      unsigned incl = c;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const unsigned t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
       }
+      if (h < nh) sm.hbase[h] = run + incl - c;
+      run += __shfl_sync(0xffffffffu, incl, 31);
     }
-    p.nnbr[i] = min(nn, p.cap_near) | (min(nf, p.cap_far) << 16);
+    if (lane == 0) sm.hbase[nh] = run;
+  }
+  __syncthreads();
+  const unsigned total = sm.hbase[nh];
+  if (total > p.tile_cap) return 0xFFFFFFFFu;
+  // one staged slot per thread and iteration; the halo cell of a slot is found by bisection of hbase (loads of
+  // different iterations are independent: several are in flight per thread)
+#pragma unroll 4
+  for (unsigned sl = threadIdx.x; sl < total; sl += blockDim.x) {
+    int lo = 0, hi = nh;  // hbase[lo] <= sl < hbase[hi]
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (sm.hbase[mid] <= sl) lo = mid;
+      else hi = mid;
+    }
+    const int h = lo;
+    const int hx = h % hxn, hy = (h / hxn) % hyn, hz = h / (hxn * hyn);
+    float ax, bx, ay, by, az, bz;
+    halo_cell(T.c0x, hx, p.ncx, p.Lx, ox, ax, bx);
+    halo_cell(T.c0y, hy, p.ncy, p.Ly, oy, ay, by);
+    halo_cell(T.c0z, hz, p.ncz, p.Lz, oz, az, bz);
+    const unsigned g = sm.hstart[h] + (sl - sm.hbase[h]);
+    float4 x = pos[g];
+    x.x = (x.x + ax) + bx;
+    x.y = (x.y + ay) + by;
+    x.z = (x.z + az) + bz;
+    sm.spos[sl] = x;
+    if (WITH_VEL) sm.svel[sl] = vel[g];
+  }
+  if (threadIdx.x == 0) {  // sentinel slot: list padding points here; it is out of range of everything
+    sm.spos[p.tile_cap] = make_float4(1e9f, 1e9f, 1e9f, 0.f);
+    if (WITH_VEL) sm.svel[p.tile_cap] = make_float4(0.f, 0.f, 0.f, 0.f);
+  }
+  __syncthreads();
+  return total;
+}
+
+// per-tile statistics at every rebuild: largest halo population (shared-memory capacity check) and largest tile
+__global__ void __launch_bounds__(128) k_tile_stats(const DevP p) {
+  if (!p.ctl->rebuild) return;
+  const unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
+  unsigned halo = 0, own = 0;
+  if (t < p.ntiles) {
+    const TileInfo T = p.tiles[t];
+    for (int hz = 0; hz < T.ez + 2; ++hz)
+      for (int hy = 0; hy < T.ey + 2; ++hy)
+        for (int hx = 0; hx < T.ex + 2; ++hx) {
+          float a, b;
+          const int cx = halo_cell(T.c0x, hx, p.ncx, 0.f, 0.f, a, b), cy = halo_cell(T.c0y, hy, p.ncy, 0.f, 0.f, a, b),
+                    cz = halo_cell(T.c0z, hz, p.ncz, 0.f, 0.f, a, b);
+          const unsigned r = p.cell_rank[((unsigned)cz * p.ncy + cy) * p.ncx + cx];
+          halo += p.cell_start[r + 1] - p.cell_start[r];
+        }
+    own = p.cell_start[T.rank0 + T.ncell_own] - p.cell_start[T.rank0];
+  }
+  halo = __reduce_max_sync(0xffffffffu, halo);
+  own = __reduce_max_sync(0xffffffffu, own);
+  if ((threadIdx.x & 31) == 0) {
+    atomicMax(&p.ctl->max_halo, halo);
+    atomicMax(&p.ctl->max_own, own);
+  }
+}
+
+// ----------------------------------------------------------------------------------------------------------------
+// a3: Verlet list (full list: every j != i with r < rc + skin at build time).
+// One warp per own cell.  The candidates of the cell's 27-cell stencil are nine contiguous runs of the staged array
+// (one per (y, z) row of halo cells); they are flattened and held IN REGISTERS, 8 chunks of 32 (one candidate per
+// lane and chunk), while the warp loops over the cell's own particles: one broadcast load of x_i, 32 distances per
+// instruction, one ballot, and the hits are appended to particle i's row in shared memory at ballot-prefix positions
+// (entries in increasing candidate order: deterministic).  Rows are then written out as 16-byte chunks of 8 16-bit
+// staged-slot indices, layout [chunk][i] (coalesced both here and in the density / force passes), padded with the
+// sentinel slot.
+// ----------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_build_list(const DevP p) {
+  if (!p.ctl->rebuild) return;
+  extern __shared__ __align__(16) unsigned char smraw[];
+  const TileSmem sm = carve_smem(smraw, p.tile_cap, false);
+  const unsigned cur = p.ctl->cur;
+  const TileInfo T = p.tiles[blockIdx.x];
+  const unsigned total = stage_tile<false>(p, T, p.pos[cur], nullptr, sm);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
+  if (total == 0xFFFFFFFFu) {  // does not fit: flag it, leave empty lists
+    const unsigned os = p.cell_start[T.rank0], oe = p.cell_start[T.rank0 + T.ncell_own];
+    for (unsigned i = os + threadIdx.x; i < oe; i += blockDim.x) {
+      p.nnbr[i] = 0u;
+      p.self_loc[i] = 0;
+    }
+    if (threadIdx.x == 0) {
+      atomicOr(&p.ctl->err, ERR_TILE);
+      atomicAdd(&p.ctl->overflow, 1ull);
+    }
+    return;
+  }
+  const int hxn = T.ex + 2, hyn = T.ey + 2;
+  // per-warp scratch behind the tables: BATCH rows of LROW entries + BATCH counters
+  unsigned short* const rows = sm.queue + (size_t)warp * (BATCH * LROW + 2 * BATCH);
+  unsigned* const cnt = (unsigned*)(rows + BATCH * LROW);
+  const unsigned sent = p.tile_cap;
+  const unsigned ltmask = lanemask_lt();
+  const unsigned rows_a = smem_addr(rows);
+  unsigned smax = 0, ssum = 0;
+  bool sover = false;
+  for (unsigned oc = warp; oc < T.ncell_own; oc += nwarps) {
+    const int lx = oc % T.ex, ly = (oc / T.ex) % T.ey, lz = oc / (T.ex * T.ey);
+    const int hown = ((lz + 1) * hyn + (ly + 1)) * hxn + lx + 1;
+    const unsigned lb = sm.hbase[hown], nown = sm.hbase[hown + 1] - lb;
+    if (nown == 0) continue;
+    const unsigned gb = sm.hstart[hown];
+    // the nine candidate runs: lane r < 9 holds run r = (dz, dy); inclusive scan of the run lengths
+    unsigned run_b = 0, run_n = 0;
+    if (lane < 9) {
+      const int hrow = ((lz + lane / 3) * hyn + (ly + lane % 3)) * hxn + lx;
+      run_b = sm.hbase[hrow];
+      run_n = sm.hbase[hrow + 3] - run_b;
+    }
+    unsigned incl = run_n;
+#pragma unroll
+    for (int o = 1; o < 16; o <<= 1) {
+      const unsigned t = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += t;
+    }
+    const unsigned ncand = __shfl_sync(0xffffffffu, incl, 8);
+    const unsigned run_o = incl - run_n;  // exclusive offset of the lane's run
+    unsigned rend[9];
+#pragma unroll
+    for (int r = 0; r < 9; ++r) rend[r] = __shfl_sync(0xffffffffu, incl, r);
+    for (unsigned b0 = 0; b0 < nown; b0 += BATCH) {
+      const unsigned nb = min((unsigned)BATCH, nown - b0);
+      // rows start filled with the sentinel: whatever lies behind a list's end is padding
+      {
+        const unsigned s2 = sent | (sent << 16);
+        uint4* r4 = (uint4*)rows;
+        for (int q = lane; q < BATCH * LROW / 8; q += 32) r4[q] = make_uint4(s2, s2, s2, s2);
+        if (lane < BATCH) cnt[lane] = 0u;
+      }
+      __syncwarp();
+      for (unsigned sc = 0; sc < ncand; sc += 32 * SCH) {
+        float cx[SCH], cy[SCH], cz[SCH];
+        unsigned cs[SCH];
+#pragma unroll
+        for (int t = 0; t < SCH; ++t) {  // flat candidate index -> staged slot (past the end: the sentinel, never hit)
+          const unsigned f = sc + t * 32 + lane;
+          unsigned r = 0;
+#pragma unroll
+          for (int q = 0; q < 8; ++q) r += (f >= rend[q]) ? 1u : 0u;
+          const unsigned rb = __shfl_sync(0xffffffffu, run_b, r), ro = __shfl_sync(0xffffffffu, run_o, r);
+          cs[t] = f < ncand ? rb + (f - ro) : sent;
+          const float4 xj = sm.spos[cs[t]];
+          cx[t] = xj.x;
+          cy[t] = xj.y;
+          cz[t] = xj.z;
+        }
+        for (unsigned il = 0; il < nb; ++il) {
+          const unsigned self = lb + b0 + il;
+          const float4 xi = sm.spos[self];  // warp-uniform: broadcast
+          unsigned c = cnt[il];
+          const unsigned row = rows_a + il * (LROW * 2);
+#pragma unroll
+          for (int t = 0; t < SCH; ++t) {
+            const float dx = xi.x - cx[t], dy = xi.y - cy[t], dz = xi.z - cz[t];
+            const float r2 = dx * dx + dy * dy + dz * dz;
+            const bool hit = r2 < p.rlist2 && cs[t] != self;
+            const unsigned b = __ballot_sync(0xffffffffu, hit);
+            const unsigned pos = c + __popc(b & ltmask);
+            if (hit && pos < LCAP) sts_u16(row + pos * 2, cs[t]);
+            c += __popc(b);
+          }
+          if (lane == 0) cnt[il] = c;
+        }
+        __syncwarp();
+      }
+      // write the batch out: lane = particle, one 16-byte chunk per iteration
+      unsigned n = lane < nb ? cnt[lane] : 0u;
+      const unsigned gi = gb + b0 + lane;
+      if (lane < nb && (n > LCAP || n > p.cap)) {  // reported as MDPD_EOVERFLOW; this particle's list is emptied
+        sover = true;
+        n = 0;
+      }
+      const unsigned mx = __reduce_max_sync(0xffffffffu, n);
+      const uint4* const myrow = (const uint4*)(rows + lane * LROW);
+      for (unsigned ch = 0; ch * 8 < mx; ++ch)
+        if (ch * 8 < n) p.nbr[(size_t)ch * p.N + gi] = myrow[ch];
+      if (lane < nb) {
+        p.nnbr[gi] = n;
+        p.self_loc[gi] = (unsigned short)(lb + b0 + lane);
+        smax = max(smax, n);
+        ssum += n;
+      }
+      __syncwarp();
+    }
   }
   // statistics + overflow flag
-  unsigned tot = nn + nf;
-  unsigned wmax = __reduce_max_sync(0xffffffffu, tot);
-  unsigned wsum = __reduce_add_sync(0xffffffffu, tot);
-  unsigned wnear = __reduce_add_sync(0xffffffffu, nn);
-  unsigned wover = __any_sync(0xffffffffu, over);
-  if ((threadIdx.x & 31) == 0) {
+  smax = __reduce_max_sync(0xffffffffu, smax);
+  ssum = __reduce_add_sync(0xffffffffu, ssum);
+  const unsigned wover = __any_sync(0xffffffffu, sover);
+  if (lane == 0) {
     Ctl* c = p.ctl;
-    atomicMax(&c->max_nbr, wmax);
-    atomicAdd(&c->sum_nbr, (unsigned long long)wsum);
-    atomicAdd(&c->sum_near, (unsigned long long)wnear);
+    atomicMax(&c->max_nbr, smax);
+    atomicAdd(&c->sum_nbr, (unsigned long long)ssum);
     if (wover) {
       atomicOr(&c->err, ERR_OVERFLOW);
       atomicAdd(&c->overflow, 1ull);
@@ -484,159 +745,173 @@ __global__ void k_reset_list_stats(const DevP p) {
   if (!p.ctl->rebuild) return;
   p.ctl->max_nbr = 0;
   p.ctl->sum_nbr = 0;
-  p.ctl->sum_near = 0;
+  p.ctl->max_halo = 0;
+  p.ctl->max_own = 0;
+}
+
+__device__ __forceinline__ unsigned list_entry(const uint4& e, const int t) {  // t is a compile-time constant
+  const unsigned w = t < 2 ? e.x : (t < 4 ? e.y : (t < 6 ? e.z : e.w));
+  return (t & 1) ? (w >> 16) : (w & 0xFFFFu);
 }
 
 // ----------------------------------------------------------------------------------------------------------------
 // a5: density pass   rho_i = sum_{j != i, r < rd} 15 / (2 pi rd^3) (1 - r / rd)^2
+// CTA = tile; thread = own particle; neighbours are shared-memory loads through the 16-bit near list.
 // ----------------------------------------------------------------------------------------------------------------
-template <bool PERIODIC>
-__device__ __forceinline__ float density_loop(const DevP& p, const float4* __restrict__ pos, const float4 xi,
-                                              unsigned i, unsigned nn) {
-  float rho = 0.0f;
-  const unsigned* __restrict__ lst = p.nbr_near + i;
-#pragma unroll 4
-  for (unsigned k = 0; k < nn; ++k) {
-    const unsigned j = lst[(size_t)k * p.N];
-    const float4 xj = __ldg(&pos[j]);
-    float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
-    if (PERIODIC) {
-      dx = minimg(dx, p.Lx);
-      dy = minimg(dy, p.Ly);
-      dz = minimg(dz, p.Lz);
-    }
-    const float r2 = dx * dx + dy * dy + dz * dz;
-    if (r2 < p.rd2) {
-      const float r = r2 * rsqrtf(fmaxf(r2, 1e-30f));
-      const float w = 1.0f - r * p.inv_rd;
-      rho += w * w;
-    }
-  }
-  return rho * p.Krho;
-}
-
-__device__ __forceinline__ bool is_interior(const DevP& p, const float4 x) {
-  return x.x >= p.margin && x.x <= p.Lx - p.margin && x.y >= p.margin && x.y <= p.Ly - p.margin && x.z >= p.margin &&
-         x.z <= p.Lz - p.margin;
-}
-
-__global__ void __launch_bounds__(TPB) k_density(const DevP p) {
+__global__ void __launch_bounds__(512) k_density(const DevP p) {
+  extern __shared__ __align__(16) unsigned char smraw[];
+  const TileSmem sm = carve_smem(smraw, p.tile_cap, false);
   const unsigned cur = p.ctl->cur;
-  unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= p.N) return;
-  const float4* __restrict__ pos = p.pos[cur];
-  const float4 xi = pos[i];
-  const unsigned nn = p.nnbr[i] & 0xFFFFu;
-  float rho;
-  if (is_interior(p, xi)) rho = density_loop<false>(p, pos, xi, i, nn);
-  else rho = density_loop<true>(p, pos, xi, i, nn);
-  p.vel[cur][i].w = rho;
+  const TileInfo T = p.tiles[blockIdx.x];
+  if (stage_tile<false>(p, T, p.pos[cur], nullptr, sm) == 0xFFFFFFFFu) return;  // flagged by k_build_list
+  const unsigned os = p.cell_start[T.rank0], oe = p.cell_start[T.rank0 + T.ncell_own];
+  float4* __restrict__ vel = p.vel[cur];
+  for (unsigned i = os + threadIdx.x; i < oe; i += blockDim.x) {
+    const float4 xi = sm.spos[p.self_loc[i]];
+    const unsigned nn = p.nnbr[i];
+    const uint4* __restrict__ lst = p.nbr + i;
+    float rho = 0.0f;
+    uint4 nxt = nn ? lst[0] : make_uint4(0, 0, 0, 0);
+    for (unsigned k0 = 0; k0 < nn; k0 += 8) {
+      const uint4 e = nxt;
+      if (k0 + 8 < nn) nxt = lst[(size_t)((k0 >> 3) + 1) * p.N];  // next chunk in flight while this one is evaluated
+#pragma unroll
+      for (int t = 0; t < 8; ++t) {
+        const float4 xj = sm.spos[list_entry(e, t)];  // padding entries hit the far-away sentinel
+        const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
+        const float r2 = dx * dx + dy * dy + dz * dz;
+        if (r2 < p.rd2) {
+          const float r = r2 * rsqrtf(fmaxf(r2, 1e-30f));
+          const float w = 1.0f - r * p.inv_rd;
+          rho += w * w;
+        }
+      }
+    }
+    vel[i].w = rho * p.Krho;
+  }
 }
 
 // ----------------------------------------------------------------------------------------------------------------
 // a6: pair-force pass (Eq. (1); L186 body force)
 //   F_ij = [A wC + B (rho_i + rho_j) wd - gamma wC^2 (e.v_ij) + sigma wC xi_ij / sqrt(dt)] e_ij ,  s = 1
 // Full list: every pair is evaluated from both ends; the symmetric hash makes F_ij = -F_ji bitwise.
+// The near part (built with r < rd + skin, ~90 % of it inside rc) is evaluated in place; the far part (~10 % inside
+// rc) is first filtered into a per-lane queue in shared memory so that the expensive branch runs with full lanes.
 // ----------------------------------------------------------------------------------------------------------------
 struct ForceAcc {
   float x, y, z;
 };
 
-template <bool PERIODIC, bool FAR>
-__device__ __forceinline__ void force_loop(const DevP& p, const float4* __restrict__ pos,
-                                           const float4* __restrict__ vel, const float4 xi, const float4 vi,
-                                           const unsigned tagi, const unsigned walli, const HashKeys& K, unsigned i,
-                                           unsigned cnt, ForceAcc& acc) {
-  const unsigned* __restrict__ lst = (FAR ? p.nbr_far : p.nbr_near) + i;
-#pragma unroll 2
-  for (unsigned k = 0; k < cnt; ++k) {
-    const unsigned j = lst[(size_t)k * p.N];
-    const float4 xj = __ldg(&pos[j]);
-    float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
-    if (PERIODIC) {
-      dx = minimg(dx, p.Lx);
-      dy = minimg(dy, p.Ly);
-      dz = minimg(dz, p.Lz);
-    }
-    const float r2 = dx * dx + dy * dy + dz * dz;
-    const unsigned wj = f2u(xj.w);
-    if (r2 < p.rc2 && r2 > 1e-12f && !(walli & (wj >> 31))) {
-      const float4 vj = __ldg(&vel[j]);
-      const float rinv = rsqrtf(r2);
-      const float r = r2 * rinv;
-      const float w = 1.0f - r * p.inv_rc;
-      float F = p.A * w;
-      if (!FAR) {  // pairs of the far part have r >= rd for the whole life of the list
-        const float wd = fmaxf(0.0f, 1.0f - r * p.inv_rd);
-        F += p.B * (vi.w + vj.w) * wd;
-      }
-      const float ev = (dx * (vi.x - vj.x) + dy * (vi.y - vj.y) + dz * (vi.z - vj.z)) * rinv;
-      F -= p.gamma * w * w * ev;
-      const unsigned h = pair_hash(tagi, wj & 0x7FFFFFFFu, K);
-      const float xi_s = (float)((int)(h >> 8) - (1 << 23));  // exact
-      F += p.sig_c * w * xi_s;
-      const float Fr = F * rinv;
-      acc.x += Fr * dx;
-      acc.y += Fr * dy;
-      acc.z += Fr * dz;
-    }
-  }
+__device__ __forceinline__ void pair_force(const DevP& p, const float4 xi, const float4 vi, const unsigned tagi,
+                                           const float4 xj, const float4 vj, const float dx, const float dy,
+                                           const float dz, const float r2, const HashKeys& K, ForceAcc& acc) {
+  const float rinv = rsqrtf(r2);
+  const float r = r2 * rinv;
+  const float w = 1.0f - r * p.inv_rc;
+  float F = p.A * w;
+  const float wd = fmaxf(0.0f, 1.0f - r * p.inv_rd);
+  F += p.B * (vi.w + vj.w) * wd;
+  const float ev = (dx * (vi.x - vj.x) + dy * (vi.y - vj.y) + dz * (vi.z - vj.z)) * rinv;
+  F -= p.gamma * w * w * ev;
+  const unsigned h = pair_hash(tagi, f2u(xj.w) & 0x7FFFFFFFu, K);
+  const float xi_s = (float)((int)(h >> 8) - (1 << 23));  // exact
+  F += p.sig_c * w * xi_s;
+  const float Fr = F * rinv;
+  acc.x += Fr * dx;
+  acc.y += Fr * dy;
+  acc.z += Fr * dz;
 }
 
 template <bool ALL>  // ALL: also evaluate the (never used) forces on frozen particles, for parity checks
-__global__ void __launch_bounds__(TPB) k_force(const DevP p) {
+__global__ void __launch_bounds__(512) k_force(const DevP p) {
+  extern __shared__ __align__(16) unsigned char smraw[];
+  const TileSmem sm = carve_smem(smraw, p.tile_cap, true);
   const unsigned cur = p.ctl->cur;
-  unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= p.N) return;
-  const float4* __restrict__ pos = p.pos[cur];
-  const float4* __restrict__ vel = p.vel[cur];
-  const float4 xi = pos[i];
-  const unsigned wi = f2u(xi.w);
-  const unsigned walli = wi >> 31;
-  if (!ALL && walli) return;
-  const float4 vi = vel[i];
+  const TileInfo T = p.tiles[blockIdx.x];
+  if (stage_tile<true>(p, T, p.pos[cur], p.vel[cur], sm) == 0xFFFFFFFFu) return;
+  const unsigned os = p.cell_start[T.rank0], oe = p.cell_start[T.rank0 + T.ncell_own];
   const HashKeys K = make_keys(p.ctl->step, p.seed);
-  const unsigned cnt = p.nnbr[i];
-  ForceAcc acc = {0.f, 0.f, 0.f};
-  if (is_interior(p, xi)) {
-    force_loop<false, false>(p, pos, vel, xi, vi, wi & 0x7FFFFFFFu, walli, K, i, cnt & 0xFFFFu, acc);
-    force_loop<false, true>(p, pos, vel, xi, vi, wi & 0x7FFFFFFFu, walli, K, i, cnt >> 16, acc);
-  } else {
-    force_loop<true, false>(p, pos, vel, xi, vi, wi & 0x7FFFFFFFu, walli, K, i, cnt & 0xFFFFu, acc);
-    force_loop<true, true>(p, pos, vel, xi, vi, wi & 0x7FFFFFFFu, walli, K, i, cnt >> 16, acc);
+  unsigned short* __restrict__ q = sm.queue + threadIdx.x;
+  const unsigned qs = blockDim.x;
+  for (unsigned i = os + threadIdx.x; i < oe; i += blockDim.x) {
+    const unsigned li = p.self_loc[i];
+    const float4 xi = sm.spos[li];
+    const unsigned wi = f2u(xi.w);
+    const unsigned walli = wi >> 31;
+    if (!ALL && walli) continue;
+    const unsigned tagi = wi & 0x7FFFFFFFu;
+    const float4 vi = sm.svel[li];
+    const unsigned nl = p.nnbr[i];
+    const unsigned wmask = ALL ? walli : 0u;  // the step path never evaluates frozen particles
+    ForceAcc acc = {0.f, 0.f, 0.f};
+    const uint4* __restrict__ lst = p.nbr + i;
+    uint4 nxt = nl ? lst[0] : make_uint4(0, 0, 0, 0);
+    unsigned m = 0;
+    for (unsigned k0 = 0; k0 < nl; k0 += 8) {
+      const uint4 e = nxt;
+      if (k0 + 8 < nl) nxt = lst[(size_t)((k0 >> 3) + 1) * p.N];  // next chunk in flight
+#pragma unroll
+      for (int t = 0; t < 8; ++t) {  // filter: in-range entries go to the lane's queue
+        const unsigned j = list_entry(e, t);
+        const float4 xj = sm.spos[j];  // padding entries hit the far-away sentinel
+        const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
+        const float r2 = dx * dx + dy * dy + dz * dz;
+        if (r2 < p.rc2 && r2 > 1e-12f && !(wmask & (f2u(xj.w) >> 31))) {
+          q[m * qs] = (unsigned short)j;
+          ++m;
+        }
+      }
+      // drain, decided for the whole warp: the expensive branch runs with (nearly) full lanes
+      if (__any_sync(__activemask(), m > QD - 8) || k0 + 8 >= nl) {
+#pragma unroll 2
+        for (unsigned t = 0; t < m; ++t) {
+          const unsigned j = q[t * qs];
+          const float4 xj = sm.spos[j];
+          const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
+          const float r2 = dx * dx + dy * dy + dz * dz;
+          pair_force(p, xi, vi, tagi, xj, sm.svel[j], dx, dy, dz, r2, K, acc);
+        }
+        m = 0;
+      }
+    }
+    if (!walli) {
+      acc.x += p.fgx;
+      acc.y += p.fgy;
+      acc.z += p.fgz;
+    }
+    p.force[i] = make_float4(acc.x, acc.y, acc.z, 0.0f);
   }
-  if (!walli) {
-    acc.x += p.fgx;
-    acc.y += p.fgy;
-    acc.z += p.fgz;
-  }
-  p.force[i] = make_float4(acc.x, acc.y, acc.z, 0.0f);
 }
 
 // ----------------------------------------------------------------------------------------------------------------
 // parity exports
 // ----------------------------------------------------------------------------------------------------------------
-__global__ void k_pairs(const DevP p, float rcut2, uint2* out, unsigned long long cap, unsigned long long* count) {
+__global__ void __launch_bounds__(512) k_pairs(const DevP p, float rcut2, uint2* out, unsigned long long cap,
+                                               unsigned long long* count) {
+  extern __shared__ __align__(16) unsigned char smraw[];
+  const TileSmem sm = carve_smem(smraw, p.tile_cap, false);
   const unsigned cur = p.ctl->cur;
-  unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= p.N) return;
-  const float4* __restrict__ pos = p.pos[cur];
-  const float4 xi = pos[i];
-  const unsigned tagi = f2u(xi.w) & 0x7FFFFFFFu;
-  const unsigned cnt = p.nnbr[i];
-  for (int part = 0; part < 2; ++part) {
-    const unsigned n = part ? (cnt >> 16) : (cnt & 0xFFFFu);
-    const unsigned* lst = (part ? p.nbr_far : p.nbr_near) + i;
-    for (unsigned k = 0; k < n; ++k) {
-      const unsigned j = lst[(size_t)k * p.N];
-      const float4 xj = pos[j];
-      const unsigned tagj = f2u(xj.w) & 0x7FFFFFFFu;
-      if (tagi >= tagj) continue;
-      float dx = minimg(xi.x - xj.x, p.Lx), dy = minimg(xi.y - xj.y, p.Ly), dz = minimg(xi.z - xj.z, p.Lz);
-      const float r2 = dx * dx + dy * dy + dz * dz;
-      if (r2 < rcut2) {
-        unsigned long long s = atomicAdd(count, 1ull);
-        if (s < cap) out[s] = make_uint2(tagi, tagj);
+  const TileInfo T = p.tiles[blockIdx.x];
+  if (stage_tile<false>(p, T, p.pos[cur], nullptr, sm) == 0xFFFFFFFFu) return;
+  const unsigned os = p.cell_start[T.rank0], oe = p.cell_start[T.rank0 + T.ncell_own];
+  for (unsigned i = os + threadIdx.x; i < oe; i += blockDim.x) {
+    const float4 xi = sm.spos[p.self_loc[i]];
+    const unsigned tagi = f2u(xi.w) & 0x7FFFFFFFu;
+    const unsigned n = p.nnbr[i];
+    {
+      const uint4* lst = p.nbr + i;
+      for (unsigned k = 0; k < n; ++k) {
+        const uint4 e = lst[(size_t)(k >> 3) * p.N];
+        const unsigned w = (k & 4) ? ((k & 2) ? e.w : e.z) : ((k & 2) ? e.y : e.x);
+        const float4 xj = sm.spos[(k & 1) ? (w >> 16) : (w & 0xFFFFu)];
+        const unsigned tagj = f2u(xj.w) & 0x7FFFFFFFu;
+        if (tagi >= tagj) continue;
+        const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
+        const float r2 = dx * dx + dy * dy + dz * dz;
+        if (r2 < rcut2) {
+          unsigned long long s = atomicAdd(count, 1ull);
+          if (s < cap) out[s] = make_uint2(tagi, tagj);
+        }
       }
     }
   }
@@ -656,10 +931,10 @@ __global__ void k_rng_fill(unsigned long long n, const uint2* __restrict__ pairs
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {
-  size_t pos[2], vel[2], force, xbuild, cell_rank, cell_count, cell_start, scan_bsum, pcell, order, nbr_near, nbr_far,
-      nnbr, mask, ctl, stage, total;
-  unsigned ncx, ncy, ncz, ncell, cap_near, cap_far, scan_blocks;
-  float rlist, rnear;
+  size_t pos[2], vel[2], force, xbuild, cell_rank, cell_count, cell_start, scan_bsum, pcell, order, nbr,
+      nnbr, self_loc, tiles, mask, ctl, stage, total;
+  unsigned ncx, ncy, ncz, ncell, cap, scan_blocks;
+  float rlist;
 };
 
 bool make_layout(const mdpd_params& p, uint64_t n, int has_mask, const uint32_t* md, Layout& L, std::string* why) {
@@ -674,7 +949,6 @@ bool make_layout(const mdpd_params& p, uint64_t n, int has_mask, const uint32_t*
   if (p.reorder_every > 1) return fail("only reorder_every = 0/1 is implemented (DESIGN.md R16)");
   if (n >= (1ull << 31)) return fail("n must be < 2^31");
   L.rlist = p.rc + p.skin;
-  L.rnear = std::min(p.rd + p.skin, L.rlist);
   int nc[3];
   for (int d = 0; d < 3; ++d) {
     if (!(p.box[d] > 0)) return fail("box must be > 0");
@@ -688,18 +962,10 @@ bool make_layout(const mdpd_params& p, uint64_t n, int has_mask, const uint32_t*
   const double PI = 3.14159265358979323846;
   const double vol = (double)p.box[0] * p.box[1] * p.box[2];
   const double dens = std::max(8.0, 1.3 * (double)n / vol);
-  const double m_near = 4.0 / 3.0 * PI * std::pow((double)L.rnear, 3) * dens;
-  const double m_far = 4.0 / 3.0 * PI * (std::pow((double)L.rlist, 3) - std::pow((double)L.rnear, 3)) * dens;
-  auto cap_of = [](double m) { return (unsigned)(std::ceil((m + 6.0 * std::sqrt(m) + 8.0) / 8.0) * 8.0); };
-  if (p.max_neigh == 0) {
-    L.cap_near = cap_of(m_near);
-    L.cap_far = m_far > 0 ? cap_of(m_far) : 8;
-  } else {
-    double fr = m_near / (m_near + m_far);
-    L.cap_near = (unsigned)(std::ceil(p.max_neigh * fr / 8.0) * 8.0);
-    L.cap_far = (unsigned)(std::ceil(p.max_neigh * (1.0 - fr) / 8.0) * 8.0) + 8;
-  }
-  if (L.cap_near > 65535 || L.cap_far > 65535) return fail("max_neigh too large (each part must be < 65536)");
+  const double m_list = 4.0 / 3.0 * PI * std::pow((double)L.rlist, 3) * dens;
+  if (p.max_neigh == 0) L.cap = std::min<unsigned>(LCAP, (unsigned)(std::ceil((m_list + 6.0 * std::sqrt(m_list) + 8.0) / 8.0) * 8.0));
+  else L.cap = (p.max_neigh + 7u) / 8u * 8u;
+  if (L.cap > LCAP) return fail("max_neigh must be <= 128 (the list build assembles a particle's list in shared memory)");
   L.scan_blocks = (L.ncell + SCAN_TILE - 1) / SCAN_TILE;
   const size_t N = (size_t)std::max<uint64_t>(n, 1);
   size_t off = 0;
@@ -719,9 +985,10 @@ bool make_layout(const mdpd_params& p, uint64_t n, int has_mask, const uint32_t*
   L.scan_bsum = take((size_t)L.scan_blocks * 4 + 4);
   L.pcell = take(N * 4);
   L.order = take(N * 4);
-  L.nbr_near = take(N * 4 * L.cap_near);
-  L.nbr_far = take(N * 4 * L.cap_far);
+  L.nbr = take(N * 2 * L.cap);
   L.nnbr = take(N * 4);
+  L.self_loc = take(N * 2);
+  L.tiles = take((size_t)L.ncell * sizeof(TileInfo));  // worst case: one cell per tile
   L.stage = take(N * 40 + 64);  // load/unload staging: pos, vel, force [n][3] + rho [n] (+ type at load)
   size_t mbytes = 0;
   if (has_mask) {
@@ -751,6 +1018,11 @@ struct mdpd_ctx {
   bool has_mask = false;
   uint64_t launches = 0;
   uint64_t host_step = 0;
+  int tile_dim[3] = {4, 4, 4};
+  unsigned block = 256;          // threads per CTA of the density / force passes
+  unsigned block_build = 256;    // threads per CTA of the list build
+  size_t smem_pos = 0, smem_posvel = 0, smem_build = 0;
+  size_t smem_limit = 0;         // cudaDevAttrMaxSharedMemoryPerBlockOptin
   std::string err;
   Ctl* h_ctl = nullptr;  // pinned
   // per-kernel CUDA-event timing (mdpd_profile_begin / _end)
@@ -830,23 +1102,24 @@ void fill_devp(mdpd_ctx* h) {
   d.scan_bsum = (unsigned*)(w + L.scan_bsum);
   d.pcell = (unsigned*)(w + L.pcell);
   d.order = (unsigned*)(w + L.order);
-  d.nbr_near = (unsigned*)(w + L.nbr_near);
-  d.nbr_far = (unsigned*)(w + L.nbr_far);
+  d.nbr = (uint4*)(w + L.nbr);
   d.nnbr = (unsigned*)(w + L.nnbr);
+  d.self_loc = (unsigned short*)(w + L.self_loc);
+  d.tiles = (const TileInfo*)(w + L.tiles);
   d.mask = (const unsigned char*)(w + L.mask);
   d.ctl = (Ctl*)(w + L.ctl);
   d.N = (unsigned)h->n;
   d.ncell = L.ncell;
-  d.cap_near = L.cap_near;
-  d.cap_far = L.cap_far;
+  d.cap = L.cap;
   d.ncx = L.ncx; d.ncy = L.ncy; d.ncz = L.ncz;
   d.Lx = p.box[0]; d.Ly = p.box[1]; d.Lz = p.box[2];
   d.icx = (float)((double)L.ncx / (double)p.box[0]);
   d.icy = (float)((double)L.ncy / (double)p.box[1]);
   d.icz = (float)((double)L.ncz / (double)p.box[2]);
   d.rlist2 = L.rlist * L.rlist;
-  d.rnear2 = L.rnear * L.rnear;
-  d.margin = L.rlist + p.skin + 1e-3f;
+  d.edge_x = (float)((double)p.box[0] / (double)L.ncx);
+  d.edge_y = (float)((double)p.box[1] / (double)L.ncy);
+  d.edge_z = (float)((double)p.box[2] / (double)L.ncz);
 }
 
 void fill_physics(mdpd_ctx* h) {
@@ -866,26 +1139,43 @@ void fill_physics(mdpd_ctx* h) {
   d.seed = p.seed;
 }
 
-// Morton (Z-curve) rank of every cell: walk the codes of the bounding power-of-two cube in increasing order.
-void build_morton_ranks(const Layout& L, std::vector<unsigned>& rank) {
+// Sort order of the cells: tiles of tdim[0] x tdim[1] x tdim[2] cells enumerated along the Z-curve (Morton order of
+// the tile coordinates: neighbouring tiles are close in memory and in L2), cells x-fastest inside a tile (the cells
+// of a tile row, and the whole tile, are contiguous runs of particles).
+void build_tile_ranks(const Layout& L, const int tdim[3], std::vector<unsigned>& rank, std::vector<TileInfo>& tiles) {
   rank.assign(L.ncell, 0u);
-  unsigned mx = std::max(L.ncx, std::max(L.ncy, L.ncz));
+  tiles.clear();
+  const unsigned ntx = (L.ncx + tdim[0] - 1) / tdim[0], nty = (L.ncy + tdim[1] - 1) / tdim[1],
+                 ntz = (L.ncz + tdim[2] - 1) / tdim[2];
+  unsigned mx = std::max(ntx, std::max(nty, ntz));
   int bits = 0;
   while ((1u << bits) < mx) ++bits;
   auto compact = [](unsigned long long v) {  // every third bit
     unsigned r = 0;
-    for (int b = 0; b < 10; ++b) r |= (unsigned)((v >> (3 * b)) & 1ull) << b;
+    for (int b = 0; b < 11; ++b) r |= (unsigned)((v >> (3 * b)) & 1ull) << b;
     return r;
   };
   unsigned next = 0;
   const unsigned long long ncodes = 1ull << (3 * bits);
   for (unsigned long long code = 0; code < ncodes; ++code) {
-    unsigned cx = compact(code), cy = compact(code >> 1), cz = compact(code >> 2);
-    if (cx < L.ncx && cy < L.ncy && cz < L.ncz) rank[((size_t)cz * L.ncy + cy) * L.ncx + cx] = next++;
+    const unsigned tx = compact(code), ty = compact(code >> 1), tz = compact(code >> 2);
+    if (tx >= ntx || ty >= nty || tz >= ntz) continue;
+    TileInfo T;
+    T.c0x = (int)(tx * tdim[0]); T.c0y = (int)(ty * tdim[1]); T.c0z = (int)(tz * tdim[2]);
+    T.ex = std::min<int>(tdim[0], (int)L.ncx - T.c0x);
+    T.ey = std::min<int>(tdim[1], (int)L.ncy - T.c0y);
+    T.ez = std::min<int>(tdim[2], (int)L.ncz - T.c0z);
+    T.rank0 = next;
+    T.ncell_own = (unsigned)(T.ex * T.ey * T.ez);
+    for (int lz = 0; lz < T.ez; ++lz)
+      for (int ly = 0; ly < T.ey; ++ly)
+        for (int lx = 0; lx < T.ex; ++lx)
+          rank[((size_t)(T.c0z + lz) * L.ncy + (T.c0y + ly)) * L.ncx + (T.c0x + lx)] = next++;
+    tiles.push_back(T);
   }
 }
 
-int launch_rebuild_chain(mdpd_ctx* h) {
+int launch_rebuild_chain(mdpd_ctx* h, bool with_list = true) {
   const DevP& d = h->d;
   const unsigned nb = nblk(h->n, TPB);
   cudaStream_t s = h->stream;
@@ -896,16 +1186,16 @@ int launch_rebuild_chain(mdpd_ctx* h) {
   LAUNCH(h, PS_SCAN, (k_scan_add<<<h->L.scan_blocks, SCAN_TPB, 0, s>>>(d)));
   LAUNCH(h, PS_CELL_FILL, (k_cell_fill<<<nb, TPB, 0, s>>>(d)));
   LAUNCH(h, PS_PERMUTE, (k_permute<<<nb, TPB, 0, s>>>(d)));
-  LAUNCH(h, PS_BUILD_LIST, (k_build_list<<<nb, TPB, 0, s>>>(d)));
+  LAUNCH(h, PS_OTHER, (k_tile_stats<<<nblk(d.ntiles, 128), 128, 0, s>>>(d)));
+  if (with_list) LAUNCH(h, PS_BUILD_LIST, (k_build_list<<<d.ntiles, h->block_build, h->smem_build, s>>>(d)));
   return MDPD_OK;
 }
 
 int launch_forces(mdpd_ctx* h, bool all) {
   const DevP& d = h->d;
-  const unsigned nb = nblk(h->n, TPB);
-  LAUNCH(h, PS_DENSITY, (k_density<<<nb, TPB, 0, h->stream>>>(d)));
-  if (all) LAUNCH(h, PS_FORCE, (k_force<true><<<nb, TPB, 0, h->stream>>>(d)));
-  else LAUNCH(h, PS_FORCE, (k_force<false><<<nb, TPB, 0, h->stream>>>(d)));
+  LAUNCH(h, PS_DENSITY, (k_density<<<d.ntiles, h->block, h->smem_pos, h->stream>>>(d)));
+  if (all) LAUNCH(h, PS_FORCE, (k_force<true><<<d.ntiles, h->block, h->smem_posvel, h->stream>>>(d)));
+  else LAUNCH(h, PS_FORCE, (k_force<false><<<d.ntiles, h->block, h->smem_posvel, h->stream>>>(d)));
   return MDPD_OK;
 }
 
@@ -923,10 +1213,15 @@ int sync_and_check(mdpd_ctx* h) {
   CU_TRY(h, cudaGetLastError());
   if (h->h_ctl->err & ERR_NAN)
     return set_err(h, MDPD_ENAN, "non-finite coordinates appeared (%llu events)", h->h_ctl->nan_events);
+  if (h->h_ctl->err & ERR_TILE)
+    return set_err(h, MDPD_EOVERFLOW,
+                   "a tile of %d x %d x %d cells plus its halo holds %u particles, shared-memory capacity is %u "
+                   "(local density too high for this tile size)",
+                   h->tile_dim[0], h->tile_dim[1], h->tile_dim[2], h->h_ctl->max_halo, h->d.tile_cap);
   if (h->h_ctl->err & ERR_OVERFLOW)
     return set_err(h, MDPD_EOVERFLOW,
-                   "neighbour list capacity exceeded (near %u, far %u; longest list needed %u): raise max_neigh",
-                   h->L.cap_near, h->L.cap_far, h->h_ctl->max_nbr);
+                   "neighbour list capacity exceeded (capacity %u, hard limit %u): raise max_neigh or lower skin",
+                   h->L.cap, LCAP);
   return MDPD_OK;
 }
 
@@ -1039,21 +1334,11 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
   h->loaded = false;
   fill_devp(h);
   fill_physics(h);
-  // control block
-  Ctl c0;
-  memset(&c0, 0, sizeof c0);
-  c0.cur = 1;      // the initial sort reads buffer 0 and writes buffer 1
-  c0.rebuild = 1;
-  c0.rebuilds = 1;
-  CU_TRY(h, cudaMemcpyAsync(h->d.ctl, &c0, sizeof c0, cudaMemcpyHostToDevice, h->stream));
-  CU_TRY(h, cudaStreamSynchronize(h->stream));  // c0 is on the stack
   h->host_step = 0;
-  {  // Morton rank table
-    std::vector<unsigned> rank;
-    build_morton_ranks(L, rank);
-    CU_TRY(h, cudaMemcpyAsync(h->d.cell_rank, rank.data(), rank.size() * 4, cudaMemcpyHostToDevice, h->stream));
-    CU_TRY(h, cudaMemsetAsync(h->d.cell_count, 0, (size_t)L.ncell * 4, h->stream));
-    CU_TRY(h, cudaStreamSynchronize(h->stream));
+  {
+    int v = 0;
+    CU_TRY(h, cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device));
+    h->smem_limit = (size_t)v;
   }
   if (n) {
     char* st = h->ws + L.stage;
@@ -1064,7 +1349,78 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
     CU_TRY(h, cudaMemcpyAsync(svel, vel, n * 12, cudaMemcpyDefault, h->stream));
     if (type) CU_TRY(h, cudaMemcpyAsync(stype, type, n, cudaMemcpyDefault, h->stream));
     LAUNCH(h, PS_OTHER, (k_pack<<<nblk(n, TPB), TPB, 0, h->stream>>>(h->d, spos, svel, type ? stype : nullptr, 0u)));
-    launch_rebuild_chain(h);
+  }
+  // Tile shape: the largest candidate that still gives every SM work and whose most populated tile + halo fits in
+  // shared memory (checked on the device after the sort); MDPD_TILE="tx,ty,tz" / MDPD_BLOCK override for experiments.
+  static const int kCand[][3] = {{4, 4, 4}, {4, 4, 2}, {4, 2, 2}, {2, 2, 2}, {2, 2, 1}, {2, 1, 1}, {1, 1, 1}};
+  const int ncand = (int)(sizeof kCand / sizeof kCand[0]);
+  int first = 0;
+  int forced[3] = {0, 0, 0};
+  if (const char* e = getenv("MDPD_TILE")) sscanf(e, "%d,%d,%d", &forced[0], &forced[1], &forced[2]);
+  const bool force_tile = forced[0] >= 1 && forced[0] <= 4 && forced[1] >= 1 && forced[1] <= 4 && forced[2] >= 1 && forced[2] <= 4;
+  if (!force_tile) {
+    auto ntiles_of = [&](const int* t) {
+      return (size_t)((L.ncx + t[0] - 1) / t[0]) * ((L.ncy + t[1] - 1) / t[1]) * ((L.ncz + t[2] - 1) / t[2]);
+    };
+    while (first < 3 && ntiles_of(kCand[first]) < 148) ++first;  // small boxes: down to 2 x 2 x 2
+  }
+  for (int ci = first; ci < ncand; ++ci) {
+    const int* cand = force_tile ? forced : kCand[ci];
+    int tdim[3] = {std::min<int>(cand[0], (int)L.ncx), std::min<int>(cand[1], (int)L.ncy), std::min<int>(cand[2], (int)L.ncz)};
+    std::vector<unsigned> rank;
+    std::vector<TileInfo> tiles;
+    build_tile_ranks(L, tdim, rank, tiles);
+    memcpy(h->tile_dim, tdim, sizeof tdim);
+    h->d.ntiles = (unsigned)tiles.size();
+    const int vol = tdim[0] * tdim[1] * tdim[2];
+    h->block = vol >= 32 ? 512u : 128u;
+    if (const char* e = getenv("MDPD_BLOCK")) {
+      int b = atoi(e);
+      if (b >= 32 && b <= 512 && b % 32 == 0) h->block = (unsigned)b;
+    }
+    h->block_build = vol >= 32 ? 256u : 128u;
+    if (const char* e = getenv("MDPD_BLOCK_BUILD")) {
+      int b = atoi(e);
+      if (b >= 32 && b <= 512 && b % 32 == 0) h->block_build = (unsigned)b;
+    }
+    const size_t fixed = tile_smem_bytes(0, true, (size_t)QD * h->block);
+    const unsigned cap_limit = (unsigned)std::min<size_t>((h->smem_limit - fixed) / 32, 65535);
+    h->d.tile_cap = cap_limit;
+    Ctl c0;
+    memset(&c0, 0, sizeof c0);
+    c0.cur = 1;  // the initial sort reads buffer 0 and writes buffer 1
+    c0.rebuild = 1;
+    c0.rebuilds = 1;
+    CU_TRY(h, cudaMemcpyAsync(h->d.ctl, &c0, sizeof c0, cudaMemcpyHostToDevice, h->stream));
+    CU_TRY(h, cudaMemcpyAsync(h->d.cell_rank, rank.data(), rank.size() * 4, cudaMemcpyHostToDevice, h->stream));
+    CU_TRY(h, cudaMemcpyAsync((void*)h->d.tiles, tiles.data(), tiles.size() * sizeof(TileInfo), cudaMemcpyHostToDevice,
+                              h->stream));
+    CU_TRY(h, cudaMemsetAsync(h->d.cell_count, 0, (size_t)L.ncell * 4, h->stream));
+    if (n) launch_rebuild_chain(h, false);  // sort + tile statistics, no list yet
+    CU_TRY(h, cudaMemcpyAsync(h->h_ctl, h->d.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, h->stream));
+    CU_TRY(h, cudaStreamSynchronize(h->stream));  // c0, rank, tiles are locals
+    const unsigned max_halo = h->h_ctl->max_halo;
+    if (max_halo > cap_limit) {
+      if (force_tile || ci + 1 == ncand)
+        return set_err(h, MDPD_EOVERFLOW, "a tile of %d x %d x %d cells plus halo holds %u particles; shared memory fits %u",
+                       tdim[0], tdim[1], tdim[2], max_halo, cap_limit);
+      continue;  // try the next smaller tile shape
+    }
+    // head-room for density fluctuations between rebuilds of a long run
+    h->d.tile_cap = std::min<unsigned>(cap_limit, ((unsigned)(max_halo * 1.15) + 64 + 63) / 64 * 64);
+    break;
+  }
+  h->smem_pos = tile_smem_bytes(h->d.tile_cap, false, 0);
+  h->smem_posvel = tile_smem_bytes(h->d.tile_cap, true, (size_t)QD * h->block);
+  h->smem_build = tile_smem_bytes(h->d.tile_cap, false, (size_t)(BATCH * LROW + 2 * BATCH) * (h->block_build / 32));
+  if (h->smem_build > h->smem_limit) return set_err(h, MDPD_ENOMEM, "list build needs %zu bytes of shared memory", h->smem_build);
+  CU_TRY(h, cudaFuncSetAttribute(k_build_list, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_build));
+  CU_TRY(h, cudaFuncSetAttribute(k_density, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
+  CU_TRY(h, cudaFuncSetAttribute(k_pairs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
+  CU_TRY(h, cudaFuncSetAttribute(k_force<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
+  CU_TRY(h, cudaFuncSetAttribute(k_force<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
+  if (n) {
+    LAUNCH(h, PS_BUILD_LIST, (k_build_list<<<h->d.ntiles, h->block_build, h->smem_build, h->stream>>>(h->d)));
     launch_forces(h, true);
   }
   h->loaded = true;
@@ -1172,7 +1528,7 @@ int mdpd_get_counters(mdpd_ctx* h, uint64_t out[8]) {
   out[2] = c->bounces;
   out[3] = c->max_nbr;
   out[4] = c->sum_nbr;
-  out[5] = c->sum_near;
+  out[5] = c->max_halo;
   out[6] = c->overflow + c->nan_events;
   out[7] = h->launches;
   return rc;
@@ -1197,7 +1553,7 @@ int mdpd_get_pairs(mdpd_ctx* h, float rcut, uint64_t* count, uint32_t* pairs, ui
     }
   }
   cudaMemsetAsync(dcnt, 0, 8, h->stream);
-  LAUNCH(h, PS_OTHER, (k_pairs<<<nblk(h->n, TPB), TPB, 0, h->stream>>>(h->d, rcut * rcut, dout, cap, dcnt)));
+  LAUNCH(h, PS_OTHER, (k_pairs<<<h->d.ntiles, h->block, h->smem_pos, h->stream>>>(h->d, rcut * rcut, dout, cap, dcnt)));
   unsigned long long c = 0;
   cudaMemcpyAsync(&c, dcnt, 8, cudaMemcpyDeviceToHost, h->stream);
   cudaError_t e = cudaStreamSynchronize(h->stream);
