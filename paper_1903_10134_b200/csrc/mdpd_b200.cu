@@ -43,7 +43,7 @@ struct Ctl {
   unsigned max_nbr;   // longest list at the last build
   unsigned max_halo;  // most particles in a tile + halo at the last build
   unsigned max_own;   // most particles in a tile at the last build
-  unsigned pad0;
+  unsigned has_wall;  // some particle is frozen (set by k_pack)
   unsigned long long steps, rebuilds, bounces, sum_nbr, overflow, nan_events, pair_count, pad1;
 };
 
@@ -69,6 +69,8 @@ struct DevP {  // passed by value to every kernel
   uint4* nbr;                // [cap / 8][N] chunks of 8 16-bit staged-slot indices, padded with the sentinel slot
   unsigned short* self_loc;  // [N] staged slot of the particle itself
   unsigned* nnbr;            // [N] list length
+  uint4* act;                // [cap / 8][N] this step's in-range (r < rc) subset of the list, written by the density pass
+  unsigned short* nact;      // [N] its length
   const TileInfo* tiles;     // [ntiles]
   const unsigned char* mask;
   Ctl* ctl;
@@ -95,6 +97,11 @@ __device__ __forceinline__ unsigned f2u(float f) { return __float_as_uint(f); }
 __device__ __forceinline__ unsigned smem_addr(const void* ptr) { return (unsigned)__cvta_generic_to_shared(ptr); }
 __device__ __forceinline__ void sts_u16(unsigned addr, unsigned v) {
   asm volatile("st.shared.u16 [%0], %1;" ::"r"(addr), "h"((unsigned short)v) : "memory");
+}
+__device__ __forceinline__ float rsqrt_fast(float x) {  // one MUFU.RSQ (2 ulp); callers keep x out of the denormals
+  float y;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
 }
 __device__ __forceinline__ unsigned lanemask_lt() {
   unsigned m;
@@ -165,6 +172,7 @@ __global__ void k_pack(DevP p, const float* __restrict__ pos, const float* __res
   if (x < 0.0f) x = 0.0f;
   if (y < 0.0f) y = 0.0f;
   if (z < 0.0f) z = 0.0f;
+  if (t) atomicOr(&p.ctl->has_wall, 1u);
   p.pos[buf][i] = make_float4(x, y, z, u2f(i | (t << 31)));
   float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
   if (!t) {
@@ -174,6 +182,19 @@ __global__ void k_pack(DevP p, const float* __restrict__ pos, const float* __res
   }
   p.vel[buf][i] = v;
   p.force[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+}
+
+// (re)start the control block for a fresh sort of buffer 0 into buffer 1; keeps has_wall
+__global__ void k_ctl_init(DevP p) {
+  Ctl* c = p.ctl;
+  const unsigned hw = c->has_wall;
+  Ctl z;
+  memset(&z, 0, sizeof z);
+  z.cur = 1;
+  z.rebuild = 1;
+  z.rebuilds = 1;
+  z.has_wall = hw;
+  *c = z;
 }
 
 __global__ void k_unpack(DevP p, float* __restrict__ pos, float* __restrict__ vel, float* __restrict__ force,
@@ -446,7 +467,6 @@ __global__ void __launch_bounds__(TPB) k_permute(const DevP p) {
 constexpr int HMAX = 216;                      // halo cells of the largest tile
 constexpr int HTAB = 224;                      // table size (HMAX + 1 rounded up)
 static_assert(HMAX + 1 <= HTAB, "halo table");
-constexpr unsigned QD = 24;                    // depth of the per-lane in-range queue of the force pass
 constexpr unsigned LCAP = 128;                 // per-particle list capacity
 constexpr unsigned LROW = LCAP + 8;            // row pitch of the list build's shared-memory rows (bank spread, 16-byte aligned)
 constexpr int SCH = 4;                         // candidate chunks (of 32) held in registers at a time
@@ -457,10 +477,10 @@ struct TileSmem {
   float4* svel;      // [cap] (vx, vy, vz, rho)            (force pass only)
   unsigned* hbase;   // [HTAB] first staged slot of halo cell h; hbase[nh] = number of staged particles
   unsigned* hstart;  // [HTAB] global index of the first particle of halo cell h
-  unsigned short* queue;  // [QD][blockDim] (force pass only)
+  unsigned short* queue;  // scratch behind the tables (list build: per-warp rows)
 };
 
-// queue_entries: 16-bit scratch entries behind the tables (force pass: QD per thread; list build: rows per warp)
+// queue_entries: 16-bit scratch entries behind the tables (list build: rows per warp)
 __host__ __device__ inline size_t tile_smem_bytes(unsigned cap, bool with_vel, size_t queue_entries) {
   return (size_t)(cap + 1) * 16 * (with_vel ? 2 : 1) + 2 * HTAB * 4 + queue_entries * 2;  // + sentinel slot
 }
@@ -756,8 +776,12 @@ __device__ __forceinline__ unsigned list_entry(const uint4& e, const int t) {  /
 
 // ----------------------------------------------------------------------------------------------------------------
 // a5: density pass   rho_i = sum_{j != i, r < rd} 15 / (2 pi rd^3) (1 - r / rd)^2
-// CTA = tile; thread = own particle; neighbours are shared-memory loads through the 16-bit near list.
+// CTA = tile; thread = own particle; neighbours are shared-memory loads through the 16-bit list.  The same sweep
+// also emits, for the force pass that follows, the compact list of the entries that are inside rc at THIS step
+// (positions do not change between the two passes): the force pass then touches in-range pairs only.  The compact
+// list is assembled 8 entries at a time in four registers (a 128-bit shift register) and stored as 16-byte chunks.
 // ----------------------------------------------------------------------------------------------------------------
+template <bool HAS_WALL>
 __global__ void __launch_bounds__(512) k_density(const DevP p) {
   extern __shared__ __align__(16) unsigned char smraw[];
   const TileSmem sm = carve_smem(smraw, p.tile_cap, false);
@@ -766,27 +790,53 @@ __global__ void __launch_bounds__(512) k_density(const DevP p) {
   if (stage_tile<false>(p, T, p.pos[cur], nullptr, sm) == 0xFFFFFFFFu) return;  // flagged by k_build_list
   const unsigned os = p.cell_start[T.rank0], oe = p.cell_start[T.rank0 + T.ncell_own];
   float4* __restrict__ vel = p.vel[cur];
+  const unsigned sent = p.tile_cap;
   for (unsigned i = os + threadIdx.x; i < oe; i += blockDim.x) {
     const float4 xi = sm.spos[p.self_loc[i]];
+    const unsigned walli = f2u(xi.w) >> 31;
     const unsigned nn = p.nnbr[i];
     const uint4* __restrict__ lst = p.nbr + i;
+    uint4* __restrict__ ao = p.act + i;  // next chunk to write
     float rho = 0.0f;
+    unsigned a0 = 0, a1 = 0, a2 = 0, a3 = 0, na = 0;
     uint4 nxt = nn ? lst[0] : make_uint4(0, 0, 0, 0);
     for (unsigned k0 = 0; k0 < nn; k0 += 8) {
       const uint4 e = nxt;
       if (k0 + 8 < nn) nxt = lst[(size_t)((k0 >> 3) + 1) * p.N];  // next chunk in flight while this one is evaluated
 #pragma unroll
       for (int t = 0; t < 8; ++t) {
-        const float4 xj = sm.spos[list_entry(e, t)];  // padding entries hit the far-away sentinel
+        const unsigned j = list_entry(e, t);
+        const float4 xj = sm.spos[j];  // padding entries hit the far-away sentinel
         const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
         const float r2 = dx * dx + dy * dy + dz * dz;
-        if (r2 < p.rd2) {
-          const float r = r2 * rsqrtf(fmaxf(r2, 1e-30f));
-          const float w = 1.0f - r * p.inv_rd;
-          rho += w * w;
+        const float rr = fmaxf(r2, 1e-30f);
+        const float w = fmaxf(0.0f, 1.0f - (rr * rsqrt_fast(rr)) * p.inv_rd);  // branch-free: 0 beyond rd
+        rho += w * w;
+        bool in = r2 < p.rc2 && r2 > 1e-12f;  // interacts at this step (R10)
+        if (HAS_WALL) in = in && !(walli & (f2u(xj.w) >> 31));  // frozen-frozen pairs do not (R8)
+        if (in) {
+          a0 = __funnelshift_r(a0, a1, 16);
+          a1 = __funnelshift_r(a1, a2, 16);
+          a2 = __funnelshift_r(a2, a3, 16);
+          a3 = __funnelshift_r(a3, j, 16);
+          ++na;
+          if ((na & 7u) == 0u) {
+            *ao = make_uint4(a0, a1, a2, a3);
+            ao += p.N;
+          }
         }
       }
     }
+    if (na & 7u) {  // last, partial chunk: pad with the sentinel
+      for (unsigned q = na & 7u; q < 8u; ++q) {
+        a0 = __funnelshift_r(a0, a1, 16);
+        a1 = __funnelshift_r(a1, a2, 16);
+        a2 = __funnelshift_r(a2, a3, 16);
+        a3 = __funnelshift_r(a3, sent, 16);
+      }
+      *ao = make_uint4(a0, a1, a2, a3);
+    }
+    p.nact[i] = (unsigned short)na;
     vel[i].w = rho * p.Krho;
   }
 }
@@ -795,8 +845,7 @@ __global__ void __launch_bounds__(512) k_density(const DevP p) {
 // a6: pair-force pass (Eq. (1); L186 body force)
 //   F_ij = [A wC + B (rho_i + rho_j) wd - gamma wC^2 (e.v_ij) + sigma wC xi_ij / sqrt(dt)] e_ij ,  s = 1
 // Full list: every pair is evaluated from both ends; the symmetric hash makes F_ij = -F_ji bitwise.
-// The near part (built with r < rd + skin, ~90 % of it inside rc) is evaluated in place; the far part (~10 % inside
-// rc) is first filtered into a per-lane queue in shared memory so that the expensive branch runs with full lanes.
+// Walks the compact in-range list the density pass wrote for this step: every evaluated pair interacts.
 // ----------------------------------------------------------------------------------------------------------------
 struct ForceAcc {
   float x, y, z;
@@ -805,7 +854,7 @@ struct ForceAcc {
 __device__ __forceinline__ void pair_force(const DevP& p, const float4 xi, const float4 vi, const unsigned tagi,
                                            const float4 xj, const float4 vj, const float dx, const float dy,
                                            const float dz, const float r2, const HashKeys& K, ForceAcc& acc) {
-  const float rinv = rsqrtf(r2);
+  const float rinv = rsqrt_fast(r2);  // r2 > 1e-12 here
   const float r = r2 * rinv;
   const float w = 1.0f - r * p.inv_rc;
   float F = p.A * w;
@@ -831,8 +880,6 @@ __global__ void __launch_bounds__(512) k_force(const DevP p) {
   if (stage_tile<true>(p, T, p.pos[cur], p.vel[cur], sm) == 0xFFFFFFFFu) return;
   const unsigned os = p.cell_start[T.rank0], oe = p.cell_start[T.rank0 + T.ncell_own];
   const HashKeys K = make_keys(p.ctl->step, p.seed);
-  unsigned short* __restrict__ q = sm.queue + threadIdx.x;
-  const unsigned qs = blockDim.x;
   for (unsigned i = os + threadIdx.x; i < oe; i += blockDim.x) {
     const unsigned li = p.self_loc[i];
     const float4 xi = sm.spos[li];
@@ -841,37 +888,22 @@ __global__ void __launch_bounds__(512) k_force(const DevP p) {
     if (!ALL && walli) continue;
     const unsigned tagi = wi & 0x7FFFFFFFu;
     const float4 vi = sm.svel[li];
-    const unsigned nl = p.nnbr[i];
-    const unsigned wmask = ALL ? walli : 0u;  // the step path never evaluates frozen particles
+    const unsigned na = p.nact[i];
     ForceAcc acc = {0.f, 0.f, 0.f};
-    const uint4* __restrict__ lst = p.nbr + i;
-    uint4 nxt = nl ? lst[0] : make_uint4(0, 0, 0, 0);
-    unsigned m = 0;
-    for (unsigned k0 = 0; k0 < nl; k0 += 8) {
+    const uint4* __restrict__ lst = p.act + i;
+    uint4 nxt = na ? lst[0] : make_uint4(0, 0, 0, 0);
+    for (unsigned k0 = 0; k0 < na; k0 += 8) {
       const uint4 e = nxt;
-      if (k0 + 8 < nl) nxt = lst[(size_t)((k0 >> 3) + 1) * p.N];  // next chunk in flight
+      if (k0 + 8 < na) nxt = lst[(size_t)((k0 >> 3) + 1) * p.N];  // next chunk in flight
 #pragma unroll
-      for (int t = 0; t < 8; ++t) {  // filter: in-range entries go to the lane's queue
-        const unsigned j = list_entry(e, t);
-        const float4 xj = sm.spos[j];  // padding entries hit the far-away sentinel
-        const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
-        const float r2 = dx * dx + dy * dy + dz * dz;
-        if (r2 < p.rc2 && r2 > 1e-12f && !(wmask & (f2u(xj.w) >> 31))) {
-          q[m * qs] = (unsigned short)j;
-          ++m;
-        }
-      }
-      // drain, decided for the whole warp: the expensive branch runs with (nearly) full lanes
-      if (__any_sync(__activemask(), m > QD - 8) || k0 + 8 >= nl) {
-#pragma unroll 2
-        for (unsigned t = 0; t < m; ++t) {
-          const unsigned j = q[t * qs];
+      for (int t = 0; t < 8; ++t) {
+        if (k0 + t < na) {
+          const unsigned j = list_entry(e, t);
           const float4 xj = sm.spos[j];
           const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
           const float r2 = dx * dx + dy * dy + dz * dz;
           pair_force(p, xi, vi, tagi, xj, sm.svel[j], dx, dy, dz, r2, K, acc);
         }
-        m = 0;
       }
     }
     if (!walli) {
@@ -932,7 +964,7 @@ inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {
   size_t pos[2], vel[2], force, xbuild, cell_rank, cell_count, cell_start, scan_bsum, pcell, order, nbr,
-      nnbr, self_loc, tiles, mask, ctl, stage, total;
+      act, nact, nnbr, self_loc, tiles, mask, ctl, stage, total;
   unsigned ncx, ncy, ncz, ncell, cap, scan_blocks;
   float rlist;
 };
@@ -986,6 +1018,8 @@ bool make_layout(const mdpd_params& p, uint64_t n, int has_mask, const uint32_t*
   L.pcell = take(N * 4);
   L.order = take(N * 4);
   L.nbr = take(N * 2 * L.cap);
+  L.act = take(N * 2 * L.cap);
+  L.nact = take(N * 2);
   L.nnbr = take(N * 4);
   L.self_loc = take(N * 2);
   L.tiles = take((size_t)L.ncell * sizeof(TileInfo));  // worst case: one cell per tile
@@ -1016,6 +1050,7 @@ struct mdpd_ctx {
   bool ws_owned = false;
   size_t mask_cap = 0;  // bytes reserved for the mask in the workspace
   bool has_mask = false;
+  bool has_wall = false;  // some particle is frozen (type 1)
   uint64_t launches = 0;
   uint64_t host_step = 0;
   int tile_dim[3] = {4, 4, 4};
@@ -1103,6 +1138,8 @@ void fill_devp(mdpd_ctx* h) {
   d.pcell = (unsigned*)(w + L.pcell);
   d.order = (unsigned*)(w + L.order);
   d.nbr = (uint4*)(w + L.nbr);
+  d.act = (uint4*)(w + L.act);
+  d.nact = (unsigned short*)(w + L.nact);
   d.nnbr = (unsigned*)(w + L.nnbr);
   d.self_loc = (unsigned short*)(w + L.self_loc);
   d.tiles = (const TileInfo*)(w + L.tiles);
@@ -1193,7 +1230,8 @@ int launch_rebuild_chain(mdpd_ctx* h, bool with_list = true) {
 
 int launch_forces(mdpd_ctx* h, bool all) {
   const DevP& d = h->d;
-  LAUNCH(h, PS_DENSITY, (k_density<<<d.ntiles, h->block, h->smem_pos, h->stream>>>(d)));
+  if (h->has_wall) LAUNCH(h, PS_DENSITY, (k_density<true><<<d.ntiles, h->block, h->smem_pos, h->stream>>>(d)));
+  else LAUNCH(h, PS_DENSITY, (k_density<false><<<d.ntiles, h->block, h->smem_pos, h->stream>>>(d)));
   if (all) LAUNCH(h, PS_FORCE, (k_force<true><<<d.ntiles, h->block, h->smem_posvel, h->stream>>>(d)));
   else LAUNCH(h, PS_FORCE, (k_force<false><<<d.ntiles, h->block, h->smem_posvel, h->stream>>>(d)));
   return MDPD_OK;
@@ -1340,6 +1378,7 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
     CU_TRY(h, cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device));
     h->smem_limit = (size_t)v;
   }
+  CU_TRY(h, cudaMemsetAsync(h->d.ctl, 0, sizeof(Ctl), h->stream));
   if (n) {
     char* st = h->ws + L.stage;
     float* spos = (float*)st;
@@ -1352,7 +1391,7 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
   }
   // Tile shape: the largest candidate that still gives every SM work and whose most populated tile + halo fits in
   // shared memory (checked on the device after the sort); MDPD_TILE="tx,ty,tz" / MDPD_BLOCK override for experiments.
-  static const int kCand[][3] = {{4, 4, 4}, {4, 4, 2}, {4, 2, 2}, {2, 2, 2}, {2, 2, 1}, {2, 1, 1}, {1, 1, 1}};
+  static const int kCand[][3] = {{4, 4, 2}, {4, 2, 2}, {2, 2, 2}, {2, 2, 1}, {2, 1, 1}, {1, 1, 1}};
   const int ncand = (int)(sizeof kCand / sizeof kCand[0]);
   int first = 0;
   int forced[3] = {0, 0, 0};
@@ -1362,7 +1401,7 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
     auto ntiles_of = [&](const int* t) {
       return (size_t)((L.ncx + t[0] - 1) / t[0]) * ((L.ncy + t[1] - 1) / t[1]) * ((L.ncz + t[2] - 1) / t[2]);
     };
-    while (first < 3 && ntiles_of(kCand[first]) < 148) ++first;  // small boxes: down to 2 x 2 x 2
+    while (first < 2 && ntiles_of(kCand[first]) < 148) ++first;  // small boxes: down to 2 x 2 x 2
   }
   for (int ci = first; ci < ncand; ++ci) {
     const int* cand = force_tile ? forced : kCand[ci];
@@ -1373,32 +1412,20 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
     memcpy(h->tile_dim, tdim, sizeof tdim);
     h->d.ntiles = (unsigned)tiles.size();
     const int vol = tdim[0] * tdim[1] * tdim[2];
-    h->block = vol >= 32 ? 512u : 128u;
-    if (const char* e = getenv("MDPD_BLOCK")) {
-      int b = atoi(e);
-      if (b >= 32 && b <= 512 && b % 32 == 0) h->block = (unsigned)b;
-    }
+    h->block = 512u;  // upper bound while the capacity is probed; set from the tile population below
     h->block_build = vol >= 32 ? 256u : 128u;
-    if (const char* e = getenv("MDPD_BLOCK_BUILD")) {
-      int b = atoi(e);
-      if (b >= 32 && b <= 512 && b % 32 == 0) h->block_build = (unsigned)b;
-    }
-    const size_t fixed = tile_smem_bytes(0, true, (size_t)QD * h->block);
+    const size_t fixed = tile_smem_bytes(0, true, 0);
     const unsigned cap_limit = (unsigned)std::min<size_t>((h->smem_limit - fixed) / 32, 65535);
     h->d.tile_cap = cap_limit;
-    Ctl c0;
-    memset(&c0, 0, sizeof c0);
-    c0.cur = 1;  // the initial sort reads buffer 0 and writes buffer 1
-    c0.rebuild = 1;
-    c0.rebuilds = 1;
-    CU_TRY(h, cudaMemcpyAsync(h->d.ctl, &c0, sizeof c0, cudaMemcpyHostToDevice, h->stream));
+    LAUNCH(h, PS_OTHER, (k_ctl_init<<<1, 1, 0, h->stream>>>(h->d)));  // the initial sort reads buffer 0 and writes buffer 1
     CU_TRY(h, cudaMemcpyAsync(h->d.cell_rank, rank.data(), rank.size() * 4, cudaMemcpyHostToDevice, h->stream));
     CU_TRY(h, cudaMemcpyAsync((void*)h->d.tiles, tiles.data(), tiles.size() * sizeof(TileInfo), cudaMemcpyHostToDevice,
                               h->stream));
     CU_TRY(h, cudaMemsetAsync(h->d.cell_count, 0, (size_t)L.ncell * 4, h->stream));
     if (n) launch_rebuild_chain(h, false);  // sort + tile statistics, no list yet
     CU_TRY(h, cudaMemcpyAsync(h->h_ctl, h->d.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, h->stream));
-    CU_TRY(h, cudaStreamSynchronize(h->stream));  // c0, rank, tiles are locals
+    CU_TRY(h, cudaStreamSynchronize(h->stream));  // rank, tiles are locals
+    h->has_wall = h->h_ctl->has_wall != 0;
     const unsigned max_halo = h->h_ctl->max_halo;
     if (max_halo > cap_limit) {
       if (force_tile || ci + 1 == ncand)
@@ -1406,16 +1433,27 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
                        tdim[0], tdim[1], tdim[2], max_halo, cap_limit);
       continue;  // try the next smaller tile shape
     }
+    // density / force passes: one thread per own particle of the fullest tile (a tile with more loops)
+    h->block = std::min(512u, std::max(64u, (h->h_ctl->max_own + 31u) / 32u * 32u));
+    if (const char* e = getenv("MDPD_BLOCK")) {
+      int b = atoi(e);
+      if (b >= 32 && b <= 512 && b % 32 == 0) h->block = (unsigned)b;
+    }
+    if (const char* e = getenv("MDPD_BLOCK_BUILD")) {
+      int b = atoi(e);
+      if (b >= 32 && b <= 256 && b % 32 == 0) h->block_build = (unsigned)b;
+    }
     // head-room for density fluctuations between rebuilds of a long run
     h->d.tile_cap = std::min<unsigned>(cap_limit, ((unsigned)(max_halo * 1.15) + 64 + 63) / 64 * 64);
     break;
   }
   h->smem_pos = tile_smem_bytes(h->d.tile_cap, false, 0);
-  h->smem_posvel = tile_smem_bytes(h->d.tile_cap, true, (size_t)QD * h->block);
+  h->smem_posvel = tile_smem_bytes(h->d.tile_cap, true, 0);
   h->smem_build = tile_smem_bytes(h->d.tile_cap, false, (size_t)(BATCH * LROW + 2 * BATCH) * (h->block_build / 32));
   if (h->smem_build > h->smem_limit) return set_err(h, MDPD_ENOMEM, "list build needs %zu bytes of shared memory", h->smem_build);
   CU_TRY(h, cudaFuncSetAttribute(k_build_list, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_build));
-  CU_TRY(h, cudaFuncSetAttribute(k_density, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
+  CU_TRY(h, cudaFuncSetAttribute(k_density<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
+  CU_TRY(h, cudaFuncSetAttribute(k_density<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
   CU_TRY(h, cudaFuncSetAttribute(k_pairs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
   CU_TRY(h, cudaFuncSetAttribute(k_force<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
   CU_TRY(h, cudaFuncSetAttribute(k_force<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
