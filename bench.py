@@ -161,13 +161,36 @@ def main_reference(args, rank, world):
 
 
 # --------------------------------------------------------------------------------------------------- our arm
-def algorithmic_bytes(kernel, n, n_list, n_near):
-    """Bytes one launch must move through HBM if every gathered neighbour load hits cache (DESIGN.md section 7,
-    SURVEY.md 8(d)): per particle, density = pos 16 + 4 n_near + rho 4; force = pos 16 + (vel, rho) 16 + 4 n_list +
-    force 16; integrate = pos r/w 32 + vel r/w 32 + force 16 + xbuild 16."""
-    per = {"k_density": 16 + 4 * n_near + 4, "k_force": 16 + 16 + 4 * n_list + 16, "k_integrate": 96,
-           "k_build_list": 16 + 4 * n_list + 4}.get(kernel)
+def algorithmic_bytes(kernel, n, n_list, n_act):
+    """Bytes one launch must move through HBM: per particle, density = pos 16 + list 2 n_list +
+    rho 4 + compact list 2 n_act; force = pos 16 + (vel, rho) 16 + compact list 2 n_act + force 16; integrate = pos r/w
+    32 + vel r/w 32 + force 16 + xbuild 16; list build = pos 16 + list 2 n_list + length and own slot 6."""
+    per = {"k_density": 16 + 2 * n_list + 4 + 2 * n_act, "k_force": 16 + 16 + 2 * n_act + 16, "k_integrate": 96,
+           "k_build_list": 16 + 2 * n_list + 6}.get(kernel)
     return None if per is None else per * n
+
+
+def algorithmic_ops(kernel, n, n_list, n_act):
+    """Thread-level arithmetic/logic operations the formulas need (FMA = 1, no address or loop
+    arithmetic): 13 per listed entry in the density pass (r^2, compare, weight), 48 per in-range pair in the force pass."""
+    per = {"k_density": 13 * n_list, "k_force": 48 * n_act}.get(kernel)
+    return None if per is None else per * n
+
+
+def max_over_ranks(values, world, device):
+    """Replicas only: the one cross-rank operation of the bench is the MAX of the timings."""
+    if world <= 1:
+        return [float(v) for v in values]
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(v) for v in values], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.cpu()]
+
+
+def whole_job_rate(n_per_rank, steps, world, seconds):
+    """particle-steps/s of the whole job: every rank advanced its own replica of n particles by `steps` steps."""
+    return world * n_per_rank * steps / seconds
 
 
 def main_ours(args, rank, world, local):
@@ -230,17 +253,22 @@ def main_ours(args, rank, world, local):
     launches = c1["launches"] - c0["launches"]
     rebuilds = c1["rebuilds"] - c0["rebuilds"]
     n_list = c1["sum_nbr"] / n
-    n_near = n_list                              # one list serves both passes
+    n_act = (c1["sum_act"] - c0["sum_act"]) / max(1, c1["density_passes"] - c0["density_passes"]) / n
+    ts = c1["tile_shape"]
+    tile_shape = [ts & 255, (ts >> 8) & 255, (ts >> 16) & 255]
 
     # ---- per-kernel CUDA-event times over another K steps (same stream) --------------------------------------
     sim.profile_begin()
     sim.step(K)
     prof = sim.profile_end()
+    c2 = sim.counters()
+    reb_prof = c2["rebuilds"] - c1["rebuilds"]
     tot = sum(v[0] for v in prof.values())
     hot = [k for k in prof if k != "other"]
     dom = max(hot, key=lambda k: prof[k][0])
     kernels = {k: {"ms_total": round(prof[k][0], 4), "launches": prof[k][1],
                    "share": round(prof[k][0] / tot, 4) if tot else None} for k in prof}
+    kernels["k_build_list"]["real_rebuilds"] = reb_prof
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
@@ -248,22 +276,44 @@ def main_ours(args, rank, world, local):
         pass
     peak_gbs, peak_src = (peaks["hbm_gbs"], "MEASURED_PEAKS.json hbm_gbs") if "hbm_gbs" in peaks else \
         (6650.0, "B200_PROFILING.md fallback")
-    roof = {"bound": "hbm", "kernel": dom, "peak": peak_gbs, "unit": "GB/s", "peak_source": peak_src,
-            "traffic": None}
-    ab = algorithmic_bytes(dom, n, n_list, n_near)
-    dom_ms = prof[dom][0] / max(1, prof[dom][1])
-    if ab is not None and dom_ms > 0:
-        roof.update(achieved=ab / (dom_ms * 1e-3) / 1e9, algorithmic_bytes_per_launch=ab,
-                    ms_per_launch=dom_ms)
-        roof["frac"] = roof["achieved"] / peak_gbs
-    also = {}
-    for k in ("k_density", "k_force", "k_integrate"):
-        b = algorithmic_bytes(k, n, n_list, n_near)
-        t = prof[k][0] / max(1, prof[k][1])
-        if b and t > 0:
-            also[k] = {"achieved_gbs": round(b / (t * 1e-3) / 1e9, 1), "frac": round(b / (t * 1e-3) / 1e9 / peak_gbs, 4),
-                       "ms_per_launch": round(t, 5)}
-    roof["per_kernel"] = also
+    clocks = clk.summary()
+    sm_mhz = clocks.get("sm_mhz") or clocks.get("sm_max_mhz") or 1965.0
+    alu_peak = 148 * 128 * sm_mhz * 1e6 / 1e9       # Gop/s: 148 SMs x 4 sub-partitions x 32 lanes x f_clk
+
+    def launch_ms(k):   # mean duration of the launches that did work (rebuild-chain kernels: real rebuilds only)
+        cnt = reb_prof if k == "k_build_list" else prof[k][1]
+        return prof[k][0] / max(1, cnt)
+
+    per_kernel = {}
+    for k in ("k_force", "k_density", "k_build_list", "k_integrate"):
+        t = launch_ms(k)
+        if t <= 0:
+            continue
+        ent = {"ms_per_launch": round(t, 5)}
+        b = algorithmic_bytes(k, n, n_list, n_act)
+        if b:
+            ent["hbm_gbs"] = round(b / (t * 1e-3) / 1e9, 1)
+            ent["hbm_frac"] = round(ent["hbm_gbs"] / peak_gbs, 4)
+        o = algorithmic_ops(k, n, n_list, n_act)
+        if o:
+            ent["alu_gops"] = round(o / (t * 1e-3) / 1e9, 1)
+            ent["alu_frac"] = round(ent["alu_gops"] / alu_peak, 4)
+        per_kernel[k] = ent
+    # the bound of a kernel is the larger of its two algorithmic times
+    d = per_kernel.get(dom, {})
+    if d.get("alu_frac", 0) >= d.get("hbm_frac", 0) and "alu_gops" in d:
+        roof = {"bound": "alu", "kernel": dom, "achieved": d["alu_gops"], "peak": round(alu_peak, 1), "unit": "Gop/s",
+                "frac": d["alu_frac"],
+                "peak_source": f"148 SMs x 128 lanes x {sm_mhz:.0f} MHz sampled in this run (DESIGN.md section 7)",
+                "algorithmic_ops_per_launch": algorithmic_ops(dom, n, n_list, n_act)}
+    else:
+        roof = {"bound": "hbm", "kernel": dom, "achieved": d.get("hbm_gbs"), "peak": peak_gbs, "unit": "GB/s",
+                "frac": d.get("hbm_frac"), "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": algorithmic_bytes(dom, n, n_list, n_act)}
+    roof["ms_per_launch"] = d.get("ms_per_launch")
+    roof["traffic"] = None
+    roof["hbm_peak_gbs"] = peak_gbs
+    roof["per_kernel"] = per_kernel
 
     # ---- e2e: host buffers -> C-ABI -> host buffers, copies inside the timed region --------------------------
     barrier()
@@ -278,12 +328,9 @@ def main_ours(args, rank, world, local):
     d2h = n * 24
 
     # ---- max over ranks ---------------------------------------------------------------------------------------
-    if world > 1:
-        t = torch.tensor([ms, e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, e2e_s = float(t[0]), float(t[1])
-    value = world * n * K / (ms * 1e-3)
-    e2e_v = world * n * K / e2e_s
+    ms, e2e_s = max_over_ranks([ms, e2e_s], world, "cuda")
+    value = whole_job_rate(n, K, world, ms * 1e-3)
+    e2e_v = whole_job_rate(n, K, world, e2e_s)
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -293,10 +340,11 @@ def main_ours(args, rank, world, local):
                        "equilibration_steps": args.equilibrate, "skin": c["params"]["skin"],
                        "l2": "inputs larger than L2" if n * 700 > 126e6 * 2 else "inputs fit L2 (small case)",
                        "rebuilds_in_window": rebuilds, "mean_list_len": round(n_list, 2),
-                       "max_list_len": c1["max_nbr"]},
+                       "mean_in_range": round(n_act, 2), "max_list_len": c1["max_nbr"],
+                       "tile_cells": tile_shape, "tiles": c1["ntiles"]},
             "e2e": {"value": e2e_v, "unit": UNIT, "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
                     "note": f"one job = load_particles(host) + {K} steps + get_state(host); bytes are per job / {K}"},
-            "gpu_launches": launches, "clocks": clk.summary(), "roofline": roof, "kernels": kernels}
+            "gpu_launches": launches, "clocks": clocks, "roofline": roof, "kernels": kernels}
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         edge = oracle_sample_edge(20.0 * 4.0e5 / 20)          # ~20 s: 20 steps of a ~4e5-particle box

@@ -99,8 +99,14 @@ int mdpd_step(mdpd_ctx* h, uint32_t nsteps);
  * Synchronises the stream and returns a latched device fault if there is one. */
 int mdpd_get_state(mdpd_ctx* h, float* pos, float* vel, float* force, float* rho, uint64_t* step);
 
-/* Checkpoint / resume: set the step index used by the hash (forces are NOT recomputed; call mdpd_compute_forces). */
+/* Checkpoint / resume.  A state is (pos, vel, force, step) as mdpd_get_state returns them: the force of time level k
+ * was evaluated with the half-step velocities (Algorithm 1 order, R6), so it is part of the state and cannot
+ * be recomputed from the full-step velocities.  Resume = mdpd_load_particles(pos, vel, type) +
+ * mdpd_set_step_counter(step) + mdpd_set_forces(force).
+ * mdpd_set_step_counter sets the step index used by the hash (forces are NOT recomputed).
+ * mdpd_set_forces overwrites the stored forces; force: [n][3] float32 in TAG order, host or device. */
 int mdpd_set_step_counter(mdpd_ctx* h, uint64_t step);
+int mdpd_set_forces(mdpd_ctx* h, const float* force);
 
 /* ---- parity / diagnostics exports (the GPU-vs-oracle comparison needs them) ---- */
 
@@ -117,11 +123,15 @@ int mdpd_get_pairs(mdpd_ctx* h, float rcut, uint64_t* count, uint32_t* pairs, ui
  * pairs: [npairs][2] uint32, out: [npairs] uint32, host or device. */
 int mdpd_rng_fill(mdpd_ctx* h, uint64_t npairs, const uint32_t* pairs, uint32_t step, uint32_t* out);
 
-/* out[0] steps done, [1] list rebuilds, [2] bounce-back events, [3] longest neighbour list at the last
- * build, [4] sum over particles of the list lengths at the last build, [5] most particles staged in shared memory
- * by one tile (tile + halo) at the last build, [6] device fault events (list overflows + non-finite coordinates; also latched as an error code),
- * [7] kernels launched by this handle so far.  Synchronises the stream. */
-int mdpd_get_counters(mdpd_ctx* h, uint64_t out[8]);
+#define MDPD_NCOUNTERS 16
+/* out[0] steps done, [1] list rebuilds, [2] bounce-back events, [3] longest neighbour list at the last build,
+ * [4] sum over particles of the list lengths at the last build, [5] most particles staged in shared memory by one
+ * tile (tile + halo) at the last build, [6] device fault events (list / tile overflows + non-finite coordinates; also
+ * latched as an error code), [7] kernels launched by this handle so far, [8] sum over all density passes so far of
+ * the in-range (r < rc) neighbour counts = pair evaluations of the force passes, [9] number of density passes so far,
+ * [10] tile shape tx | ty << 8 | tz << 16 (cells), [11] number of tiles; [12..15] reserved (0).
+ * Synchronises the stream. */
+int mdpd_get_counters(mdpd_ctx* h, uint64_t out[MDPD_NCOUNTERS]);
 
 const char* mdpd_last_error(const mdpd_ctx* h);
 

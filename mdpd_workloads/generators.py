@@ -56,16 +56,27 @@ def make_liquid(box, density=6.0, seed=BASE_SEED, n=None, **pover):
                 type=np.zeros(n, np.uint8), mask=None, voxel=0.0)
 
 
-def make_slab(box=(40.0, 20.0, 20.0), half_width=10.0, density=6.0, seed=BASE_SEED + 1, **pover):
-    """Config 1: liquid slab |x - Lx/2| < half_width in vacuum (the |x|<10 slab shifted by Lx/2)."""
+def make_slab(box=(40.0, 20.0, 20.0), half_width=10.0, density=6.0, seed=BASE_SEED + 1, lattice=False, **pover):
+    """Config 1: liquid slab |x - Lx/2| < half_width in vacuum (the |x|<10 slab shifted by Lx/2).
+    lattice=False (the config's recipe): uniform-random positions.  lattice=True: a jittered lattice at the same
+    number density -- a gentle start without the pressure shock of overlapping random points, for tests that compare
+    a stationary profile after a short equilibration."""
     rng = np.random.default_rng(seed)
-    n = int(round(density * 2 * half_width * box[1] * box[2]))
-    u = rng.random((n, 3), dtype=np.float32)
-    pos = np.empty((n, 3), np.float32)
-    pos[:, 0] = np.float32(box[0] / 2 - half_width) + u[:, 0] * np.float32(2 * half_width)
-    pos[:, 1] = u[:, 1] * np.float32(box[1])
-    pos[:, 2] = u[:, 2] * np.float32(box[2])
-    pos = _clip_into_box(pos, box)
+    if lattice:
+        lo = (box[0] / 2 - half_width, 0.0, 0.0)
+        hi = (box[0] / 2 + half_width, box[1], box[2])
+        sp = density ** (-1.0 / 3.0)
+        counts = [max(1, int(round((hi[d] - lo[d]) / sp))) for d in range(3)]
+        pos = _clip_into_box(_jittered_lattice(rng, lo, hi, counts).astype(np.float32), box)
+        n = len(pos)
+    else:
+        n = int(round(density * 2 * half_width * box[1] * box[2]))
+        u = rng.random((n, 3), dtype=np.float32)
+        pos = np.empty((n, 3), np.float32)
+        pos[:, 0] = np.float32(box[0] / 2 - half_width) + u[:, 0] * np.float32(2 * half_width)
+        pos[:, 1] = u[:, 1] * np.float32(box[1])
+        pos[:, 2] = u[:, 2] * np.float32(box[2])
+        pos = _clip_into_box(pos, box)
     vel = maxwell_velocities(rng, n)
     return dict(name="slab", params=default_params(box, **pover), pos=pos, vel=vel,
                 type=np.zeros(n, np.uint8), mask=None, voxel=0.0)
@@ -133,7 +144,7 @@ def _periodic_gaussian_field(rng, nvox, corr):
     kk = np.fft.rfftfreq(nvox)
     k2 = k[:, None, None] ** 2 + k[None, :, None] ** 2 + kk[None, None, :] ** 2
     filt = np.exp(-2.0 * (np.pi ** 2) * (corr ** 2) * k2)
-    return np.fft.irfftn(np.fft.rfftn(w) * filt, s=w.shape)
+    return np.fft.irfftn(np.fft.rfftn(w) * filt, s=w.shape, axes=(0, 1, 2))
 
 
 def _periodic_dilate(ind, radius):
@@ -142,7 +153,7 @@ def _periodic_dilate(ind, radius):
     ax = np.minimum(np.arange(n), n - np.arange(n)).astype(np.float64)
     ball = (ax[:, None, None] ** 2 + ax[None, :, None] ** 2 + ax[None, None, :] ** 2) <= radius ** 2
     conv = np.fft.irfftn(np.fft.rfftn(ind.astype(np.float64)) * np.fft.rfftn(ball.astype(np.float64)),
-                         s=ind.shape)
+                         s=ind.shape, axes=(0, 1, 2))
     return conv > 0.5
 
 

@@ -24,6 +24,7 @@ _ERRNAME = {-1: "MDPD_EINVAL", -2: "MDPD_ENOMEM", -3: "MDPD_ECUDA", -4: "MDPD_EO
 # every symbol include/mdpd.h declares
 SYMBOLS = ("mdpd_create", "mdpd_destroy", "mdpd_set_params", "mdpd_workspace_bytes", "mdpd_set_workspace",
            "mdpd_load_particles", "mdpd_load_wall_mask", "mdpd_step", "mdpd_get_state", "mdpd_set_step_counter",
+           "mdpd_set_forces",
            "mdpd_compute_forces", "mdpd_get_pairs", "mdpd_rng_fill", "mdpd_get_counters", "mdpd_last_error",
            "mdpd_profile_begin", "mdpd_profile_end", "mdpd_profile_name")
 MDPD_PROF_SLOTS = 16
@@ -79,6 +80,7 @@ def lib():
         L.mdpd_step.argtypes = [vp, u32]
         L.mdpd_get_state.argtypes = [vp, vp, vp, vp, vp, vp]
         L.mdpd_set_step_counter.argtypes = [vp, u64]
+        L.mdpd_set_forces.argtypes = [vp, vp]
         L.mdpd_compute_forces.argtypes = [vp]
         L.mdpd_get_pairs.argtypes = [vp, f32, vp, vp, u64]
         L.mdpd_rng_fill.argtypes = [vp, u64, vp, u32, vp]
@@ -104,7 +106,8 @@ def _ptr(a):
     return a.data_ptr()  # torch tensor
 
 
-COUNTER_NAMES = ("steps", "rebuilds", "bounces", "max_nbr", "sum_nbr", "max_staged", "faults", "launches")
+COUNTER_NAMES = ("steps", "rebuilds", "bounces", "max_nbr", "sum_nbr", "max_staged", "faults", "launches",
+                 "sum_act", "density_passes", "tile_shape", "ntiles")
 
 
 class Simulation:
@@ -204,6 +207,11 @@ class Simulation:
     def set_step_counter(self, k):
         self._ck(self._L.mdpd_set_step_counter(self._h, int(k)), "mdpd_set_step_counter")
 
+    def set_forces(self, force):
+        if isinstance(force, np.ndarray):
+            force = np.ascontiguousarray(force, np.float32).reshape(-1, 3)
+        self._ck(self._L.mdpd_set_forces(self._h, _ptr(force)), "mdpd_set_forces")
+
     def get_state(self, pos=True, vel=True, force=True, rho=True, out=None):
         """Returns numpy arrays in TAG order (host).  ``out``: optional dict of preallocated host/device buffers."""
         n = self.n
@@ -243,7 +251,7 @@ class Simulation:
         return out
 
     def counters(self):
-        out = np.zeros(8, np.uint64)
+        out = np.zeros(16, np.uint64)
         self._ck(self._L.mdpd_get_counters(self._h, out.ctypes.data), "mdpd_get_counters")
         return {k: int(v) for k, v in zip(COUNTER_NAMES, out)}
 

@@ -44,7 +44,7 @@ struct Ctl {
   unsigned max_halo;  // most particles in a tile + halo at the last build
   unsigned max_own;   // most particles in a tile at the last build
   unsigned has_wall;  // some particle is frozen (set by k_pack)
-  unsigned long long steps, rebuilds, bounces, sum_nbr, overflow, nan_events, pair_count, pad1;
+  unsigned long long steps, rebuilds, bounces, sum_nbr, overflow, nan_events, sum_act, dens_passes;
 };
 
 struct TileInfo {  // one CTA of the list / density / force passes
@@ -208,6 +208,13 @@ __global__ void k_unpack(DevP p, float* __restrict__ pos, float* __restrict__ ve
   if (vel) { vel[3 * tag] = v.x; vel[3 * tag + 1] = v.y; vel[3 * tag + 2] = v.z; }
   if (force) { force[3 * tag] = f.x; force[3 * tag + 1] = f.y; force[3 * tag + 2] = f.z; }
   if (rho) rho[tag] = v.w;
+}
+
+__global__ void k_set_forces(DevP p, const float* __restrict__ force) {  // tag order -> sorted order
+  unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= p.N) return;
+  const unsigned tag = f2u(p.pos[p.ctl->cur][i].w) & 0x7FFFFFFFu;
+  p.force[i] = make_float4(force[3 * tag], force[3 * tag + 1], force[3 * tag + 2], 0.0f);
 }
 
 __global__ void k_count_in_solid(DevP p, unsigned* count) {
@@ -791,6 +798,7 @@ __global__ void __launch_bounds__(512) k_density(const DevP p) {
   const unsigned os = p.cell_start[T.rank0], oe = p.cell_start[T.rank0 + T.ncell_own];
   float4* __restrict__ vel = p.vel[cur];
   const unsigned sent = p.tile_cap;
+  unsigned na_sum = 0;
   for (unsigned i = os + threadIdx.x; i < oe; i += blockDim.x) {
     const float4 xi = sm.spos[p.self_loc[i]];
     const unsigned walli = f2u(xi.w) >> 31;
@@ -837,7 +845,20 @@ __global__ void __launch_bounds__(512) k_density(const DevP p) {
       *ao = make_uint4(a0, a1, a2, a3);
     }
     p.nact[i] = (unsigned short)na;
+    na_sum += na;
     vel[i].w = rho * p.Krho;
+  }
+  // statistics: in-range pairs evaluated per step (the force pass's algorithmic work)
+  __syncthreads();  // the staged image is dead: reuse its first word
+  unsigned* acc = (unsigned*)smraw;
+  if (threadIdx.x == 0) *acc = 0u;
+  __syncthreads();
+  na_sum = __reduce_add_sync(0xffffffffu, na_sum);
+  if ((threadIdx.x & 31) == 0 && na_sum) atomicAdd(acc, na_sum);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    atomicAdd(&p.ctl->sum_act, (unsigned long long)*acc);
+    if (blockIdx.x == 0) atomicAdd(&p.ctl->dens_passes, 1ull);
   }
 }
 
@@ -1533,6 +1554,18 @@ int mdpd_set_step_counter(mdpd_ctx* h, uint64_t step) {
   return MDPD_OK;
 }
 
+int mdpd_set_forces(mdpd_ctx* h, const float* force) {
+  if (!h) return MDPD_EINVAL;
+  if (!h->loaded) return set_err(h, MDPD_ESTATE, "load_particles first");
+  if (h->n == 0) return MDPD_OK;
+  if (!force) return set_err(h, MDPD_EINVAL, "force is NULL");
+  CU_TRY(h, cudaSetDevice(h->device));
+  float* sf = (float*)(h->ws + h->L.stage);
+  CU_TRY(h, cudaMemcpyAsync(sf, force, h->n * 12, cudaMemcpyDefault, h->stream));
+  LAUNCH(h, PS_OTHER, (k_set_forces<<<nblk(h->n, TPB), TPB, 0, h->stream>>>(h->d, sf)));
+  return sync_and_check(h);
+}
+
 int mdpd_get_state(mdpd_ctx* h, float* pos, float* vel, float* force, float* rho, uint64_t* step) {
   if (!h) return MDPD_EINVAL;
   if (!h->loaded) return set_err(h, MDPD_ESTATE, "load_particles first");
@@ -1555,12 +1588,13 @@ int mdpd_get_state(mdpd_ctx* h, float* pos, float* vel, float* force, float* rho
   return rc;
 }
 
-int mdpd_get_counters(mdpd_ctx* h, uint64_t out[8]) {
+int mdpd_get_counters(mdpd_ctx* h, uint64_t out[MDPD_NCOUNTERS]) {
   if (!h || !out) return MDPD_EINVAL;
   if (!h->loaded) return set_err(h, MDPD_ESTATE, "load_particles first");
   CU_TRY(h, cudaSetDevice(h->device));
   int rc = sync_and_check(h);
   const Ctl* c = h->h_ctl;
+  for (int k = 0; k < MDPD_NCOUNTERS; ++k) out[k] = 0;
   out[0] = h->host_step;
   out[1] = c->rebuilds;
   out[2] = c->bounces;
@@ -1569,6 +1603,10 @@ int mdpd_get_counters(mdpd_ctx* h, uint64_t out[8]) {
   out[5] = c->max_halo;
   out[6] = c->overflow + c->nan_events;
   out[7] = h->launches;
+  out[8] = c->sum_act;
+  out[9] = c->dens_passes;
+  out[10] = (uint64_t)h->tile_dim[0] | ((uint64_t)h->tile_dim[1] << 8) | ((uint64_t)h->tile_dim[2] << 16);
+  out[11] = h->d.ntiles;
   return rc;
 }
 

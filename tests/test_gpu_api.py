@@ -1,0 +1,215 @@
+"""C-ABI behaviour on the GPU: call order, error codes, edge cases (empty / tiny / degenerate inputs), ownership,
+checkpoint-resume, determinism.  Every call goes through include/mdpd.h via the ctypes binding."""
+import ctypes as C
+
+import numpy as np
+import pytest
+
+import mdpd_workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("the -m gpu suite needs a CUDA device (no CPU fallback exists)")
+    from paper_1903_10134_b200 import build
+    build()
+    import paper_1903_10134_b200 as pk
+    return pk
+
+
+def ref_state(c, step=0):
+    from oracle.mdpd_ref import RefSim
+    s = RefSim(c["params"])
+    s.load_particles(c["pos"].astype(np.float64), c["vel"].astype(np.float64), c["type"])
+    if step:
+        s.set_step(step)
+        s.compute_forces()
+    return s.get_state()
+
+
+def test_call_order_and_bad_arguments(gpu):
+    L = gpu.lib()
+    h = C.c_void_p()
+    assert L.mdpd_create(C.byref(h), 0, None) == 0
+    assert L.mdpd_step(h, 1) == -5                                   # MDPD_ESTATE: nothing loaded
+    assert L.mdpd_get_state(h, None, None, None, None, None) == -5
+    assert L.mdpd_load_particles(h, 1, None, None, None) == -5       # set_params first
+    assert b"set_params" in L.mdpd_last_error(h)
+    p = gpu.make_params(wl.default_params((10.0, 10.0, 10.0), s=0.5))
+    assert L.mdpd_set_params(h, C.byref(p)) == -1                    # MDPD_EINVAL: s != 1 (R15)
+    p = gpu.make_params(wl.default_params((10.0, 10.0, 10.0), sigma=2.0))
+    assert L.mdpd_set_params(h, C.byref(p)) == -1                    # sigma^2 != 2 gamma kT
+    p = gpu.make_params(wl.default_params((10.0, 10.0, 10.0)))
+    assert L.mdpd_set_params(h, C.byref(p)) == 0
+    assert L.mdpd_load_particles(h, 4, None, None, None) == -1       # NULL arrays with n > 0
+    assert L.mdpd_create(C.byref(C.c_void_p()), 99, None) == -3      # no such device
+    assert L.mdpd_destroy(h) == 0
+    assert L.mdpd_destroy(None) == -1
+
+
+@pytest.mark.parametrize("n", [0, 1, 2])
+def test_tiny_systems(gpu, n):
+    """N = 0, 1, 2 (the degenerate cases): zero / single particle feel nothing but the body force; two particles
+    reproduce the oracle; stepping works."""
+    p = wl.default_params((5.0, 5.0, 5.0), g=(0.0, 0.0, 0.5))
+    pos = np.array([[1.0, 1.0, 1.0], [1.3, 1.4, 1.1]], np.float32)[:n]
+    vel = np.array([[0.5, 0.0, 0.0], [-0.5, 0.2, 0.0]], np.float32)[:n]
+    s = gpu.Simulation(p)
+    s.load_particles(pos, vel)
+    st = s.get_state()
+    assert st["pos"].shape == (n, 3) and st["rho"].shape == (n,)
+    if n == 1:
+        assert st["rho"][0] == 0.0 and np.allclose(st["force"][0], [0, 0, 0.5])
+    if n == 2:
+        r = ref_state(dict(params=p, pos=pos, vel=vel, type=np.zeros(2, np.uint8)))
+        assert np.allclose(st["rho"], r["rho"], rtol=2e-6) and np.allclose(st["force"], r["force"], rtol=1e-5, atol=1e-4)
+    s.step(5)
+    st = s.get_state()
+    assert st["step"] == 5 and np.isfinite(st["pos"]).all()
+    if n == 1:   # free flight under gravity, velocity Verlet is exact for constant force
+        t = 0.05
+        assert np.allclose(st["pos"][0], [1.0 + 0.5 * t, 1.0, 1.0 + 0.25 * t * t], atol=2e-6)
+        assert np.allclose(st["vel"][0], [0.5, 0.0, 0.5 * t], atol=1e-6)
+    s.close()
+
+
+def test_all_particles_in_one_cell_and_periodic_faces(gpu):
+    """Degenerate occupancy: everything in one cell next to a box corner, so neighbours are found across three
+    periodic faces; minimum box (3 cells per dimension)."""
+    rng = np.random.default_rng(3)
+    n = 60
+    pos = ((rng.random((n, 3)) - 0.5) * 1.2) % 3.75
+    pos = pos.astype(np.float32)
+    c = dict(params=wl.default_params((3.75, 3.75, 3.75), max_neigh=128), pos=pos,
+             vel=rng.standard_normal((n, 3)).astype(np.float32), type=np.zeros(n, np.uint8))
+    s = gpu.Simulation(c["params"])
+    s.load_particles(c["pos"], c["vel"])
+    g, r = s.get_state(), ref_state(c)
+    assert np.abs(g["rho"] - r["rho"]).max() <= 1e-4 * np.sqrt((r["rho"] ** 2).mean())
+    assert np.sqrt(((g["force"] - r["force"]) ** 2).sum(1)).max() <= 1e-4 * np.sqrt((r["force"] ** 2).sum(1).mean())
+    s.close()
+
+
+def test_list_capacity_overflow_is_reported(gpu):
+    c = wl.make_liquid(5.0, seed=9, max_neigh=16)     # ~49 neighbours needed
+    s = gpu.Simulation(c["params"])
+    with pytest.raises(gpu.MdpdError) as e:
+        s.load_particles(c["pos"], c["vel"])
+    assert e.value.code == -4                          # MDPD_EOVERFLOW
+    s.close()
+    with pytest.raises(gpu.MdpdError) as e:            # capacity above the hard limit
+        gpu.Simulation(wl.default_params((5.0, 5.0, 5.0), max_neigh=256))
+    assert e.value.code == -1
+
+
+def test_fluid_inside_solid_is_reported(gpu):
+    c = wl.make_poiseuille(L=12.0, wall=2.0, Lxy=6.0, seed=4)
+    c["pos"][0] = (1.0, 1.0, 0.5)                      # a fluid particle inside the lower wall
+    s = gpu.Simulation(c["params"])
+    s.load_particles(c["pos"], c["vel"], c["type"], mask_dims=c["mask"].shape[::-1])
+    with pytest.raises(gpu.MdpdError) as e:
+        s.load_wall_mask(c["mask"], c["voxel"])
+    assert e.value.code == -7                          # MDPD_EINSOLID
+    s.close()
+
+
+def test_nan_input_is_reported(gpu):
+    c = wl.make_liquid(5.0, seed=10)
+    c["vel"][5, 0] = np.nan
+    s = gpu.Simulation(c["params"])
+    s.load_particles(c["pos"], c["vel"])
+    s.step(1)
+    with pytest.raises(gpu.MdpdError) as e:
+        s.get_state()
+    assert e.value.code == -6                          # MDPD_ENAN
+    s.close()
+
+
+def test_determinism_and_checkpoint_resume(gpu):
+    """Two runs from the same input are bitwise identical; a checkpoint (pos, vel, force, step) resumes the
+    trajectory (the force of a time level was evaluated with the half-step velocities, R6, so it is part of the
+    state: mdpd.h 'Checkpoint / resume')."""
+    c = wl.make_liquid(8.0, seed=12)
+    a = gpu.Simulation(c["params"])
+    a.load_particles(c["pos"], c["vel"])
+    a.step(7)
+    mid = a.get_state()
+    a.step(9)
+    fa = a.get_state()
+    b = gpu.Simulation(c["params"])
+    b.load_particles(c["pos"], c["vel"])
+    b.step(16)
+    fb = b.get_state()
+    for k in ("pos", "vel", "force", "rho"):
+        assert np.array_equal(fa[k], fb[k]), k
+    # resume from the step-7 state
+    r = gpu.Simulation(c["params"])
+    r.load_particles(mid["pos"], mid["vel"])
+    r.set_step_counter(7)
+    r.set_forces(mid["force"])
+    r.step(9)
+    fr = r.get_state()
+    assert fr["step"] == 16
+    # the resumed run re-sorts from the saved positions, so its list order can differ: same trajectory to rounding
+    assert np.abs(fr["vel"] - fa["vel"]).max() < 5e-4
+    d = np.abs(fr["pos"] - fa["pos"])
+    assert np.minimum(d, 8.0 - d).max() < 5e-5
+    for s in (a, b, r):
+        s.close()
+
+
+def test_device_pointers_and_caller_owned_outputs(gpu):
+    """load_particles / get_state accept device pointers (torch CUDA tensors): 'host or device' in mdpd.h."""
+    import torch
+    c = wl.make_liquid(6.0, seed=13)
+    s = gpu.Simulation(c["params"])
+    dpos = torch.from_numpy(c["pos"]).cuda()
+    dvel = torch.from_numpy(c["vel"]).cuda()
+    s.load_particles(dpos, dvel, None)
+    out = {"pos": torch.empty_like(dpos), "rho": torch.empty(len(c["pos"]), device="cuda")}
+    st = s.get_state(vel=False, force=False, out=out)
+    h = gpu.Simulation(c["params"])
+    h.load_particles(c["pos"], c["vel"])
+    sh = h.get_state()
+    assert np.array_equal(st["pos"].cpu().numpy(), sh["pos"]) and np.array_equal(st["rho"].cpu().numpy(), sh["rho"])
+    s.close()
+    h.close()
+
+
+def test_parameters_can_change_between_steps(gpu):
+    """g, dt, seed, A, B, gamma, sigma may change after load (mdpd.h); box / cut-offs / skin may not."""
+    c = wl.make_liquid(6.0, seed=14)
+    s = gpu.Simulation(c["params"])
+    s.load_particles(c["pos"], c["vel"])
+    s.set_params(g=(0.0, 0.3, 0.0), seed=99)
+    s.compute_forces()
+    c2 = dict(c, params=dict(c["params"], g=(0.0, 0.3, 0.0), seed=99))
+    r = ref_state(c2)
+    g = s.get_state()
+    assert np.sqrt(((g["force"] - r["force"]) ** 2).sum(1)).max() <= 1e-4 * np.sqrt((r["force"] ** 2).sum(1).mean())
+    with pytest.raises(gpu.MdpdError) as e:
+        s.set_params(skin=0.4)
+    assert e.value.code == -5
+    s.close()
+
+
+def test_counters_and_profile(gpu):
+    c = wl.make_liquid(8.0, seed=15)
+    s = gpu.Simulation(c["params"])
+    s.load_particles(c["pos"], c["vel"])
+    c0 = s.counters()
+    s.profile_begin()
+    s.step(10)
+    prof = s.profile_end()
+    c1 = s.counters()
+    assert c1["steps"] == 10 and c1["launches"] - c0["launches"] >= 30
+    assert prof["k_force"][1] == 10 and prof["k_density"][1] == 10 and prof["k_force"][0] > 0
+    n = len(c["pos"])
+    assert 40 < c1["sum_nbr"] / n < 60                                   # ~49 listed neighbours at skin 0.25
+    assert 20 < (c1["sum_act"] - c0["sum_act"]) / (10 * n) < 30          # ~25 inside rc
+    assert c1["density_passes"] - c0["density_passes"] == 10
+    s.close()
