@@ -342,16 +342,16 @@ __global__ void __launch_bounds__(TPB) k_integrate(const DevP p, int do_B, int d
 __global__ void __launch_bounds__(TPB) k_cell_count(const DevP p) {
   if (!p.ctl->rebuild) return;
   const unsigned src = p.ctl->cur ^ 1u;
-  unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= p.N) return;
-  float4 x = p.pos[src][i];
-  x.x = wrap1(x.x, p.Lx);
-  x.y = wrap1(x.y, p.Ly);
-  x.z = wrap1(x.z, p.Lz);
-  int cx = cell_coord(x.x, p.icx, p.ncx), cy = cell_coord(x.y, p.icy, p.ncy), cz = cell_coord(x.z, p.icz, p.ncz);
-  unsigned c = p.cell_rank[((unsigned)cz * p.ncy + cy) * p.ncx + cx];
-  p.pcell[i] = c;
-  atomicAdd(&p.cell_count[c], 1u);
+  for (unsigned i = blockIdx.x * blockDim.x + threadIdx.x; i < p.N; i += gridDim.x * blockDim.x) {
+    float4 x = p.pos[src][i];
+    x.x = wrap1(x.x, p.Lx);
+    x.y = wrap1(x.y, p.Ly);
+    x.z = wrap1(x.z, p.Lz);
+    int cx = cell_coord(x.x, p.icx, p.ncx), cy = cell_coord(x.y, p.icy, p.ncy), cz = cell_coord(x.z, p.icz, p.ncz);
+    unsigned c = p.cell_rank[((unsigned)cz * p.ncy + cy) * p.ncx + cx];
+    p.pcell[i] = c;
+    atomicAdd(&p.cell_count[c], 1u);
+  }
 }
 
 // exclusive scan of cell_count[0..ncell) into cell_start, three kernels
@@ -431,11 +431,11 @@ __global__ void __launch_bounds__(SCAN_TPB) k_scan_add(const DevP p) {
 
 __global__ void __launch_bounds__(TPB) k_cell_fill(const DevP p) {
   if (!p.ctl->rebuild) return;
-  unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= p.N) return;
-  unsigned c = p.pcell[i];
-  unsigned slot = atomicSub(&p.cell_count[c], 1u) - 1u;  // the histogram counts back down to zero: self-cleaning
-  p.order[p.cell_start[c] + slot] = i;
+  for (unsigned i = blockIdx.x * blockDim.x + threadIdx.x; i < p.N; i += gridDim.x * blockDim.x) {
+    unsigned c = p.pcell[i];
+    unsigned slot = atomicSub(&p.cell_count[c], 1u) - 1u;  // the histogram counts back down to zero: self-cleaning
+    p.order[p.cell_start[c] + slot] = i;
+  }
 }
 
 // Final position inside the cell = rank of the particle's tag among the cell's particles: the sorted order is a pure
@@ -443,8 +443,7 @@ __global__ void __launch_bounds__(TPB) k_cell_fill(const DevP p) {
 __global__ void __launch_bounds__(TPB) k_permute(const DevP p) {
   if (!p.ctl->rebuild) return;
   const unsigned cur = p.ctl->cur, src = cur ^ 1u;
-  unsigned s = blockIdx.x * blockDim.x + threadIdx.x;
-  if (s >= p.N) return;
+  for (unsigned s = blockIdx.x * blockDim.x + threadIdx.x; s < p.N; s += gridDim.x * blockDim.x) {
   const unsigned i = p.order[s];
   const unsigned c = p.pcell[i];
   const unsigned cs = p.cell_start[c], ce = p.cell_start[c + 1];
@@ -462,6 +461,7 @@ __global__ void __launch_bounds__(TPB) k_permute(const DevP p) {
   p.pos[cur][dst] = x;
   p.vel[cur][dst] = p.vel[src][i];
   p.xbuild[dst] = x;
+  }
 }
 
 // ----------------------------------------------------------------------------------------------------------------
@@ -471,6 +471,9 @@ __global__ void __launch_bounds__(TPB) k_permute(const DevP p) {
 // pair separations are formed from small numbers (|x| < 8) whatever the box size.  The Verlet list stores 16-bit
 // indices into this staged array, so every neighbour access of the hot loops is a shared-memory load.
 // ----------------------------------------------------------------------------------------------------------------
+#ifndef MINB
+#define MINB 3
+#endif
 constexpr int HMAX = 216;                      // halo cells of the largest tile
 constexpr int HTAB = 224;                      // table size (HMAX + 1 rounded up)
 static_assert(HMAX + 1 <= HTAB, "halo table");
@@ -789,7 +792,7 @@ __device__ __forceinline__ unsigned list_entry(const uint4& e, const int t) {  /
 // list is assembled 8 entries at a time in four registers (a 128-bit shift register) and stored as 16-byte chunks.
 // ----------------------------------------------------------------------------------------------------------------
 template <bool HAS_WALL>
-__global__ void __launch_bounds__(512) k_density(const DevP p) {
+__global__ void __launch_bounds__(512, MINB) k_density(const DevP p) {
   extern __shared__ __align__(16) unsigned char smraw[];
   const TileSmem sm = carve_smem(smraw, p.tile_cap, false);
   const unsigned cur = p.ctl->cur;
@@ -893,7 +896,7 @@ __device__ __forceinline__ void pair_force(const DevP& p, const float4 xi, const
 }
 
 template <bool ALL>  // ALL: also evaluate the (never used) forces on frozen particles, for parity checks
-__global__ void __launch_bounds__(512) k_force(const DevP p) {
+__global__ void __launch_bounds__(512, MINB) k_force(const DevP p) {
   extern __shared__ __align__(16) unsigned char smraw[];
   const TileSmem sm = carve_smem(smraw, p.tile_cap, true);
   const unsigned cur = p.ctl->cur;
@@ -1235,7 +1238,8 @@ void build_tile_ranks(const Layout& L, const int tdim[3], std::vector<unsigned>&
 
 int launch_rebuild_chain(mdpd_ctx* h, bool with_list = true) {
   const DevP& d = h->d;
-  const unsigned nb = nblk(h->n, TPB);
+  // grid-stride kernels on a grid of a few waves: a step whose trigger did not fire pays ~nothing for them
+  const unsigned nb = std::min(nblk(h->n, TPB), 148u * 16u);
   cudaStream_t s = h->stream;
   LAUNCH(h, PS_OTHER, (k_reset_list_stats<<<1, 1, 0, s>>>(d)));
   LAUNCH(h, PS_CELL_COUNT, (k_cell_count<<<nb, TPB, 0, s>>>(d)));
