@@ -44,7 +44,7 @@ struct Ctl {
   unsigned max_halo;  // most particles in a tile + halo at the last build
   unsigned max_own;   // most particles in a tile at the last build
   unsigned has_wall;  // some particle is frozen (set by k_pack)
-  unsigned long long steps, rebuilds, bounces, sum_nbr, overflow, nan_events, sum_act, dens_passes;
+  unsigned long long steps, rebuilds, bounces, sum_nbr, overflow, nan_events, sum_act, dens_passes, graph_rebuilds, pad2;
 };
 
 struct TileInfo {  // one CTA of the list / density / force passes
@@ -235,7 +235,8 @@ __global__ void k_count_in_solid(DevP p, unsigned* count) {
 // do_B: second half kick of the step just finished; do_A: first half kick + drift of the next step.
 // ----------------------------------------------------------------------------------------------------------------
 template <bool HAS_MASK>
-__global__ void __launch_bounds__(TPB) k_integrate(const DevP p, int do_B, int do_A) {
+__global__ void __launch_bounds__(TPB) k_integrate(const DevP p, int do_B, int do_A, cudaGraphConditionalHandle cond,
+                                                   int use_cond) {
   const unsigned cur = p.ctl->cur;
   const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
   float d2 = 0.0f;
@@ -323,6 +324,10 @@ __global__ void __launch_bounds__(TPB) k_integrate(const DevP p, int do_B, int d
       unsigned md = atomicOr(&c->maxdisp2, 0u);
       unsigned rb = u2f(md) > p.thr2 ? 1u : 0u;
       c->rebuild = rb;
+      if (use_cond) {  // inside the step graph: the IF node that holds the rebuild chain runs only when the trigger fired
+        cudaGraphSetConditional(cond, rb);
+        if (rb) c->graph_rebuilds += 1ull;
+      }
       if (rb) {
         c->cur = cur ^ 1u;
         c->maxdisp2 = 0u;
@@ -602,29 +607,27 @@ __device__ __forceinline__ unsigned stage_tile(const DevP& p, const TileInfo& T,
   return total;
 }
 
-// per-tile statistics at every rebuild: largest halo population (shared-memory capacity check) and largest tile
+// per-tile statistics after the first sort (load time): largest halo population (shared-memory capacity) and largest
+// tile.  One warp per tile, lanes over the halo cells.  During stepping k_build_list keeps the same two maxima.
 __global__ void __launch_bounds__(128) k_tile_stats(const DevP p) {
-  if (!p.ctl->rebuild) return;
-  const unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
-  unsigned halo = 0, own = 0;
-  if (t < p.ntiles) {
-    const TileInfo T = p.tiles[t];
-    for (int hz = 0; hz < T.ez + 2; ++hz)
-      for (int hy = 0; hy < T.ey + 2; ++hy)
-        for (int hx = 0; hx < T.ex + 2; ++hx) {
-          float a, b;
-          const int cx = halo_cell(T.c0x, hx, p.ncx, 0.f, 0.f, a, b), cy = halo_cell(T.c0y, hy, p.ncy, 0.f, 0.f, a, b),
-                    cz = halo_cell(T.c0z, hz, p.ncz, 0.f, 0.f, a, b);
-          const unsigned r = p.cell_rank[((unsigned)cz * p.ncy + cy) * p.ncx + cx];
-          halo += p.cell_start[r + 1] - p.cell_start[r];
-        }
-    own = p.cell_start[T.rank0 + T.ncell_own] - p.cell_start[T.rank0];
+  const unsigned t = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (t >= p.ntiles) return;
+  const TileInfo T = p.tiles[t];
+  const int hxn = T.ex + 2, hyn = T.ey + 2, nh = hxn * hyn * (T.ez + 2);
+  unsigned halo = 0;
+  for (int h = lane; h < nh; h += 32) {
+    const int hx = h % hxn, hy = (h / hxn) % hyn, hz = h / (hxn * hyn);
+    float a, b;
+    const int cx = halo_cell(T.c0x, hx, p.ncx, 0.f, 0.f, a, b), cy = halo_cell(T.c0y, hy, p.ncy, 0.f, 0.f, a, b),
+              cz = halo_cell(T.c0z, hz, p.ncz, 0.f, 0.f, a, b);
+    const unsigned r = p.cell_rank[((unsigned)cz * p.ncy + cy) * p.ncx + cx];
+    halo += p.cell_start[r + 1] - p.cell_start[r];
   }
-  halo = __reduce_max_sync(0xffffffffu, halo);
-  own = __reduce_max_sync(0xffffffffu, own);
-  if ((threadIdx.x & 31) == 0) {
+  halo = __reduce_add_sync(0xffffffffu, halo);
+  if (lane == 0) {
     atomicMax(&p.ctl->max_halo, halo);
-    atomicMax(&p.ctl->max_own, own);
+    atomicMax(&p.ctl->max_own, p.cell_start[T.rank0 + T.ncell_own] - p.cell_start[T.rank0]);
   }
 }
 
@@ -646,6 +649,10 @@ __global__ void __launch_bounds__(256) k_build_list(const DevP p) {
   const TileInfo T = p.tiles[blockIdx.x];
   const unsigned total = stage_tile<false>(p, T, p.pos[cur], nullptr, sm);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
+  if (threadIdx.x == 0) {
+    atomicMax(&p.ctl->max_halo, total == 0xFFFFFFFFu ? sm.hbase[(T.ex + 2) * (T.ey + 2) * (T.ez + 2)] : total);
+    atomicMax(&p.ctl->max_own, p.cell_start[T.rank0 + T.ncell_own] - p.cell_start[T.rank0]);
+  }
   if (total == 0xFFFFFFFFu) {  // does not fit: flag it, leave empty lists
     const unsigned os = p.cell_start[T.rank0], oe = p.cell_start[T.rank0 + T.ncell_own];
     for (unsigned i = os + threadIdx.x; i < oe; i += blockDim.x) {
@@ -1075,8 +1082,17 @@ struct mdpd_ctx {
   size_t mask_cap = 0;  // bytes reserved for the mask in the workspace
   bool has_mask = false;
   bool has_wall = false;  // some particle is frozen (type 1)
-  uint64_t launches = 0;
+  uint64_t launches = 0;         // kernels launched directly (graph replays are added from graph_steps / ctl)
   uint64_t host_step = 0;
+  cudaStream_t ls = nullptr;     // stream the LAUNCH macro targets (the handle's stream, or the capture stream)
+  cudaStream_t cap_stream = nullptr;
+  cudaGraph_t graph = nullptr;   // one timestep: integrate -> IF(trigger){sort + list build} -> density -> force
+  cudaGraphExec_t graph_exec = nullptr;
+  cudaGraphConditionalHandle cond = 0;
+  bool graph_dirty = true;       // kernel arguments (DevP) changed since the capture
+  bool use_graph = true;
+  bool pending_B = false;        // the second half kick of the last step has not been applied yet
+  uint64_t graph_steps = 0;
   int tile_dim[3] = {4, 4, 4};
   unsigned block = 256;          // threads per CTA of the density / force passes
   unsigned block_build = 256;    // threads per CTA of the list build
@@ -1240,7 +1256,7 @@ int launch_rebuild_chain(mdpd_ctx* h, bool with_list = true) {
   const DevP& d = h->d;
   // grid-stride kernels on a grid of a few waves: a step whose trigger did not fire pays ~nothing for them
   const unsigned nb = std::min(nblk(h->n, TPB), 148u * 16u);
-  cudaStream_t s = h->stream;
+  cudaStream_t s = h->ls;
   LAUNCH(h, PS_OTHER, (k_reset_list_stats<<<1, 1, 0, s>>>(d)));
   LAUNCH(h, PS_CELL_COUNT, (k_cell_count<<<nb, TPB, 0, s>>>(d)));
   LAUNCH(h, PS_SCAN, (k_scan_local<<<h->L.scan_blocks, SCAN_TPB, 0, s>>>(d)));
@@ -1248,24 +1264,90 @@ int launch_rebuild_chain(mdpd_ctx* h, bool with_list = true) {
   LAUNCH(h, PS_SCAN, (k_scan_add<<<h->L.scan_blocks, SCAN_TPB, 0, s>>>(d)));
   LAUNCH(h, PS_CELL_FILL, (k_cell_fill<<<nb, TPB, 0, s>>>(d)));
   LAUNCH(h, PS_PERMUTE, (k_permute<<<nb, TPB, 0, s>>>(d)));
-  LAUNCH(h, PS_OTHER, (k_tile_stats<<<nblk(d.ntiles, 128), 128, 0, s>>>(d)));
+  if (!with_list) LAUNCH(h, PS_OTHER, (k_tile_stats<<<nblk((uint64_t)d.ntiles * 32, 128), 128, 0, s>>>(d)));
   if (with_list) LAUNCH(h, PS_BUILD_LIST, (k_build_list<<<d.ntiles, h->block_build, h->smem_build, s>>>(d)));
   return MDPD_OK;
 }
 
 int launch_forces(mdpd_ctx* h, bool all) {
   const DevP& d = h->d;
-  if (h->has_wall) LAUNCH(h, PS_DENSITY, (k_density<true><<<d.ntiles, h->block, h->smem_pos, h->stream>>>(d)));
-  else LAUNCH(h, PS_DENSITY, (k_density<false><<<d.ntiles, h->block, h->smem_pos, h->stream>>>(d)));
-  if (all) LAUNCH(h, PS_FORCE, (k_force<true><<<d.ntiles, h->block, h->smem_posvel, h->stream>>>(d)));
-  else LAUNCH(h, PS_FORCE, (k_force<false><<<d.ntiles, h->block, h->smem_posvel, h->stream>>>(d)));
+  if (h->has_wall) LAUNCH(h, PS_DENSITY, (k_density<true><<<d.ntiles, h->block, h->smem_pos, h->ls>>>(d)));
+  else LAUNCH(h, PS_DENSITY, (k_density<false><<<d.ntiles, h->block, h->smem_pos, h->ls>>>(d)));
+  if (all) LAUNCH(h, PS_FORCE, (k_force<true><<<d.ntiles, h->block, h->smem_posvel, h->ls>>>(d)));
+  else LAUNCH(h, PS_FORCE, (k_force<false><<<d.ntiles, h->block, h->smem_posvel, h->ls>>>(d)));
   return MDPD_OK;
 }
 
-int launch_integrate(mdpd_ctx* h, int do_B, int do_A) {
+int launch_integrate(mdpd_ctx* h, int do_B, int do_A, bool in_graph = false) {
   const unsigned nb = nblk(h->n, TPB);
-  if (h->has_mask) LAUNCH(h, PS_INTEGRATE, (k_integrate<true><<<nb, TPB, 0, h->stream>>>(h->d, do_B, do_A)));
-  else LAUNCH(h, PS_INTEGRATE, (k_integrate<false><<<nb, TPB, 0, h->stream>>>(h->d, do_B, do_A)));
+  const int uc = in_graph ? 1 : 0;
+  if (h->has_mask) LAUNCH(h, PS_INTEGRATE, (k_integrate<true><<<nb, TPB, 0, h->ls>>>(h->d, do_B, do_A, h->cond, uc)));
+  else LAUNCH(h, PS_INTEGRATE, (k_integrate<false><<<nb, TPB, 0, h->ls>>>(h->d, do_B, do_A, h->cond, uc)));
+  return MDPD_OK;
+}
+
+// The second half kick (Algorithm 1 line 7) of the last step is fused with the first half kick of the next one; when
+// the state is read or changed between steps it is applied here.
+int finalize_kick(mdpd_ctx* h) {
+  if (h->pending_B && h->n) launch_integrate(h, 1, 0);
+  h->pending_B = false;
+  return MDPD_OK;
+}
+
+void destroy_graph(mdpd_ctx* h) {
+  if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
+  if (h->graph) cudaGraphDestroy(h->graph);
+  h->graph_exec = nullptr;
+  h->graph = nullptr;
+  h->graph_dirty = true;
+}
+
+// One timestep as a CUDA graph: k_integrate (B + A) -> IF(trigger fired){counting sort, permute, list build} ->
+// k_density -> k_force.  The IF node's condition is set on the device by the last block of k_integrate, so a step whose
+// trigger did not fire launches 3 kernels instead of 11 and the host never learns (or waits for) the decision.
+int build_graph(mdpd_ctx* h) {
+  destroy_graph(h);
+  const uint64_t saved_launches = h->launches;
+  cudaGraph_t g = nullptr;
+  CU_TRY(h, cudaGraphCreate(&g, 0));
+  h->graph = g;
+  CU_TRY(h, cudaGraphConditionalHandleCreate(&h->cond, g, 0, cudaGraphCondAssignDefault));
+  h->ls = h->cap_stream;
+  int rc = MDPD_OK;
+  do {
+    if (cudaStreamBeginCaptureToGraph(h->cap_stream, g, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed) != cudaSuccess) { rc = MDPD_ECUDA; break; }
+    launch_integrate(h, 1, 1, true);
+    cudaStreamCaptureStatus st;
+    const cudaGraphNode_t* deps = nullptr;
+    size_t nd = 0;
+    cudaGraph_t cg = nullptr;
+    if (cudaStreamGetCaptureInfo(h->cap_stream, &st, nullptr, &cg, &deps, &nd) != cudaSuccess) { rc = MDPD_ECUDA; break; }
+    cudaGraphNodeParams cp = {};
+    cp.type = cudaGraphNodeTypeConditional;
+    cp.conditional.handle = h->cond;
+    cp.conditional.type = cudaGraphCondTypeIf;
+    cp.conditional.size = 1;
+    cudaGraphNode_t cn;
+    if (cudaGraphAddNode(&cn, g, deps, nd, &cp) != cudaSuccess) { rc = MDPD_ECUDA; break; }
+    cudaGraph_t body = cp.conditional.phGraph_out[0];
+    if (cudaStreamUpdateCaptureDependencies(h->cap_stream, &cn, 1, cudaStreamSetCaptureDependencies) != cudaSuccess) { rc = MDPD_ECUDA; break; }
+    launch_forces(h, false);
+    cudaGraph_t out = nullptr;
+    if (cudaStreamEndCapture(h->cap_stream, &out) != cudaSuccess) { rc = MDPD_ECUDA; break; }
+    // the body of the IF node: the rebuild chain
+    if (cudaStreamBeginCaptureToGraph(h->cap_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed) != cudaSuccess) { rc = MDPD_ECUDA; break; }
+    launch_rebuild_chain(h);
+    if (cudaStreamEndCapture(h->cap_stream, &out) != cudaSuccess) { rc = MDPD_ECUDA; break; }
+    if (cudaGraphInstantiate(&h->graph_exec, g, 0) != cudaSuccess) { rc = MDPD_ECUDA; break; }
+  } while (0);
+  h->ls = h->stream;
+  h->launches = saved_launches;  // capturing launches nothing
+  if (rc != MDPD_OK) {
+    cudaError_t e = cudaGetLastError();
+    destroy_graph(h);
+    return set_err(h, rc, "building the step graph failed: %s", cudaGetErrorString(e));
+  }
+  h->graph_dirty = false;
   return MDPD_OK;
 }
 
@@ -1308,7 +1390,11 @@ int mdpd_create(mdpd_ctx** out, int device, void* cuda_stream) {
   if (!h) return MDPD_ENOMEM;
   h->device = device;
   h->stream = (cudaStream_t)cuda_stream;
-  if (cudaMallocHost((void**)&h->h_ctl, sizeof(Ctl)) != cudaSuccess) {
+  h->ls = h->stream;
+  if (const char* e = getenv("MDPD_NO_GRAPH")) h->use_graph = !(e[0] && e[0] != '0');
+  if (cudaMallocHost((void**)&h->h_ctl, sizeof(Ctl)) != cudaSuccess ||
+      cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+    if (h->h_ctl) cudaFreeHost(h->h_ctl);
     delete h;
     return MDPD_ECUDA;
   }
@@ -1320,6 +1406,8 @@ int mdpd_destroy(mdpd_ctx* h) {
   if (!h) return MDPD_EINVAL;
   cudaSetDevice(h->device);
   cudaStreamSynchronize(h->stream);
+  destroy_graph(h);
+  if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
   if (h->ws_owned && h->ws) cudaFree(h->ws);
   if (h->h_ctl) cudaFreeHost(h->h_ctl);
   for (auto& r : h->prof_recs) {
@@ -1346,8 +1434,13 @@ int mdpd_set_params(mdpd_ctx* h, const mdpd_params* p) {
     if (memcmp(q.box, p->box, sizeof q.box) || q.rc != p->rc || q.rd != p->rd || q.skin != p->skin ||
         q.max_neigh != p->max_neigh || q.mass != p->mass)
       return set_err(h, MDPD_ESTATE, "box, cut-offs, skin, mass and capacities are frozen after load_particles");
+    if (h->pending_B) {  // the outstanding half kick belongs to the old parameters
+      CU_TRY(h, cudaSetDevice(h->device));
+      finalize_kick(h);
+    }
     h->prm = *p;
     fill_physics(h);
+    h->graph_dirty = true;  // kernel arguments are captured by value
     return MDPD_OK;
   }
   h->prm = *p;
@@ -1395,6 +1488,8 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
   h->n = n;
   h->has_mask = false;
   h->loaded = false;
+  h->pending_B = false;
+  h->graph_dirty = true;
   fill_devp(h);
   fill_physics(h);
   h->host_step = 0;
@@ -1494,6 +1589,7 @@ int mdpd_load_wall_mask(mdpd_ctx* h, const uint8_t* mask, const uint32_t dims[3]
   if (!h) return MDPD_EINVAL;
   if (!h->loaded) return set_err(h, MDPD_ESTATE, "load_particles first");
   CU_TRY(h, cudaSetDevice(h->device));
+  h->graph_dirty = true;
   if (!mask) {
     h->has_mask = false;
     return MDPD_OK;
@@ -1528,12 +1624,23 @@ int mdpd_step(mdpd_ctx* h, uint32_t nsteps) {
   h->host_step += nsteps;
   if (h->n == 0) return MDPD_OK;
   CU_TRY(h, cudaSetDevice(h->device));
-  for (uint32_t it = 0; it < nsteps; ++it) {
-    launch_integrate(h, it > 0, 1);  // [second half kick of the previous step +] half kick, drift, bounce, trigger
-    launch_rebuild_chain(h);         // runs only if the trigger fired (device-side predicate)
-    launch_forces(h, false);         // Algorithm 1 lines 4 and 6 at the new time level, half-step velocities
+  const bool graphs = h->use_graph && !h->prof_on && !(h->prm.flags & MDPD_FLAG_NO_GRAPH);
+  if (graphs && h->graph_dirty && (nsteps > 1 || h->pending_B)) {
+    int rc = build_graph(h);
+    if (rc != MDPD_OK) return rc;
   }
-  launch_integrate(h, 1, 0);  // Algorithm 1 line 7
+  for (uint32_t it = 0; it < nsteps; ++it) {
+    if (graphs && h->pending_B) {  // steady state: one graph replay per step
+      CU_TRY(h, cudaGraphLaunch(h->graph_exec, h->stream));
+      h->graph_steps += 1;
+    } else {
+      // [second half kick of the previous step +] half kick, drift, bounce, trigger
+      launch_integrate(h, h->pending_B ? 1 : 0, 1);
+      launch_rebuild_chain(h);   // every kernel returns at once unless the trigger fired (device-side predicate)
+      launch_forces(h, false);   // Algorithm 1 lines 4 and 6 at the new time level, half-step velocities
+    }
+    h->pending_B = true;         // Algorithm 1 line 7 is fused into the next step (or applied by finalize_kick)
+  }
   CU_TRY(h, cudaGetLastError());
   return MDPD_OK;
 }
@@ -1543,6 +1650,7 @@ int mdpd_compute_forces(mdpd_ctx* h) {
   if (!h->loaded) return set_err(h, MDPD_ESTATE, "load_particles first");
   if (h->n == 0) return MDPD_OK;
   CU_TRY(h, cudaSetDevice(h->device));
+  finalize_kick(h);
   launch_forces(h, true);
   return sync_and_check(h);
 }
@@ -1564,6 +1672,7 @@ int mdpd_set_forces(mdpd_ctx* h, const float* force) {
   if (h->n == 0) return MDPD_OK;
   if (!force) return set_err(h, MDPD_EINVAL, "force is NULL");
   CU_TRY(h, cudaSetDevice(h->device));
+  finalize_kick(h);
   float* sf = (float*)(h->ws + h->L.stage);
   CU_TRY(h, cudaMemcpyAsync(sf, force, h->n * 12, cudaMemcpyDefault, h->stream));
   LAUNCH(h, PS_OTHER, (k_set_forces<<<nblk(h->n, TPB), TPB, 0, h->stream>>>(h->d, sf)));
@@ -1575,6 +1684,7 @@ int mdpd_get_state(mdpd_ctx* h, float* pos, float* vel, float* force, float* rho
   if (!h->loaded) return set_err(h, MDPD_ESTATE, "load_particles first");
   CU_TRY(h, cudaSetDevice(h->device));
   const uint64_t n = h->n;
+  finalize_kick(h);
   if (n) {
     float* spos = (float*)(h->ws + h->L.stage);
     float* svel = spos + 3 * n;
@@ -1606,7 +1716,7 @@ int mdpd_get_counters(mdpd_ctx* h, uint64_t out[MDPD_NCOUNTERS]) {
   out[4] = c->sum_nbr;
   out[5] = c->max_halo;
   out[6] = c->overflow + c->nan_events;
-  out[7] = h->launches;
+  out[7] = h->launches + 3 * h->graph_steps + 8 * c->graph_rebuilds;  // a graph replay launches 3 kernels (+ 8 on a rebuild)
   out[8] = c->sum_act;
   out[9] = c->dens_passes;
   out[10] = (uint64_t)h->tile_dim[0] | ((uint64_t)h->tile_dim[1] << 8) | ((uint64_t)h->tile_dim[2] << 16);
