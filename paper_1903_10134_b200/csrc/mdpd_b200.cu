@@ -1564,7 +1564,16 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
       if (b >= 32 && b <= 256 && b % 32 == 0) h->block_build = (unsigned)b;
     }
     // head-room for density fluctuations between rebuilds of a long run
-    h->d.tile_cap = std::min<unsigned>(cap_limit, ((unsigned)(max_halo * 1.15) + 64 + 63) / 64 * 64);
+    {
+      // at least 15 % over the fullest tile of the initial state; beyond that, all the shared memory that does not
+      // cost a resident CTA of the force pass (the tightest: it stages positions and velocities)
+      const unsigned want = std::min<unsigned>(cap_limit, ((unsigned)(max_halo * 1.15) + 64 + 63) / 64 * 64);
+      const size_t sm_total = h->smem_limit + 1024;  // per-SM shared memory; 1 KB is reserved per resident CTA
+      const size_t per_cta = tile_smem_bytes(want, true, 0) + 1024;
+      const size_t ctas = std::max<size_t>(1, sm_total / per_cta);
+      const size_t room = sm_total / ctas - 1024 - fixed;
+      h->d.tile_cap = std::max<unsigned>(want, std::min<unsigned>(cap_limit, (unsigned)(room / 32 / 64 * 64)));
+    }
     break;
   }
   h->smem_pos = tile_smem_bytes(h->d.tile_cap, false, 0);
