@@ -212,6 +212,8 @@ def main_ours(args, rank, world, local):
 
     K, W = args.steps, max(3, args.warmup)
     c = wl.make_config(args.workload if args.workload in ("4a", "4b") else int(args.workload))
+    if args.skin is not None:
+        c["params"]["skin"] = float(args.skin)
     n = len(c["pos"])
     md = None if c.get("mask") is None else c["mask"].shape[::-1]
     # pinned host buffers (inputs of the e2e leg, outputs of get_state)
@@ -368,6 +370,7 @@ def main():
     ap.add_argument("--workload", default="4a", choices=["4a", "4b", "0", "1", "2", "3"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--equilibrate", type=int, default=EQUILIBRATE, help="untimed steps after loading")
+    ap.add_argument("--skin", type=float, default=None, help="override the Verlet-list skin (default: the config's 0.25)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

@@ -238,10 +238,11 @@ template <bool HAS_MASK>
 __global__ void __launch_bounds__(TPB) k_integrate(const DevP p, int do_B, int do_A, cudaGraphConditionalHandle cond,
                                                    int use_cond) {
   const unsigned cur = p.ctl->cur;
-  const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
-  float d2 = 0.0f;
+  float d2max = 0.0f;
   unsigned bounced = 0, bad = 0;
-  if (i < p.N) {
+  // grid-stride over the particles: a few waves of blocks, so that the same-address atomics of the trigger below are
+  // a few thousand per launch, not one pair per 128 particles
+  for (unsigned i = blockIdx.x * blockDim.x + threadIdx.x; i < p.N; i += gridDim.x * blockDim.x) {
     float4 x = p.pos[cur][i];
     if (!(f2u(x.w) >> 31)) {  // fluid; frozen particles are never integrated (R8)
       float4 v = p.vel[cur][i];
@@ -268,7 +269,7 @@ __global__ void __launch_bounds__(TPB) k_integrate(const DevP p, int do_B, int d
           v.x = -v.x;
           v.y = -v.y;
           v.z = -v.z;
-          bounced = 1;
+          bounced += 1;
         } else {
           x.x = nx;
           x.y = ny;
@@ -276,11 +277,9 @@ __global__ void __launch_bounds__(TPB) k_integrate(const DevP p, int do_B, int d
         }
         const float4 xb = p.xbuild[i];
         const float dx = x.x - xb.x, dy = x.y - xb.y, dz = x.z - xb.z;  // unwrapped since the last build
-        d2 = dx * dx + dy * dy + dz * dz;
-        if (!(d2 < 1e30f)) {
-          bad = 1;
-          d2 = 0.0f;
-        }
+        const float d2 = dx * dx + dy * dy + dz * dz;
+        if (!(d2 < 1e30f)) bad += 1;
+        else d2max = fmaxf(d2max, d2);
         p.pos[cur][i] = x;
       }
       p.vel[cur][i] = v;
@@ -288,7 +287,7 @@ __global__ void __launch_bounds__(TPB) k_integrate(const DevP p, int do_B, int d
   }
   if (!do_A) return;
   // block reduction of the trigger quantities
-  unsigned m = f2u(d2);  // non-negative floats order like their bit patterns
+  unsigned m = f2u(d2max);  // non-negative floats order like their bit patterns
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
   unsigned nb = __reduce_add_sync(0xffffffffu, bounced);
@@ -1279,7 +1278,7 @@ int launch_forces(mdpd_ctx* h, bool all) {
 }
 
 int launch_integrate(mdpd_ctx* h, int do_B, int do_A, bool in_graph = false) {
-  const unsigned nb = nblk(h->n, TPB);
+  const unsigned nb = std::min(nblk(h->n, TPB), 148u * 16u);
   const int uc = in_graph ? 1 : 0;
   if (h->has_mask) LAUNCH(h, PS_INTEGRATE, (k_integrate<true><<<nb, TPB, 0, h->ls>>>(h->d, do_B, do_A, h->cond, uc)));
   else LAUNCH(h, PS_INTEGRATE, (k_integrate<false><<<nb, TPB, 0, h->ls>>>(h->d, do_B, do_A, h->cond, uc)));
