@@ -94,19 +94,10 @@ struct DevP {  // passed by value to every kernel
 };
 
 __device__ __forceinline__ unsigned f2u(float f) { return __float_as_uint(f); }
-__device__ __forceinline__ unsigned smem_addr(const void* ptr) { return (unsigned)__cvta_generic_to_shared(ptr); }
-__device__ __forceinline__ void sts_u16(unsigned addr, unsigned v) {
-  asm volatile("st.shared.u16 [%0], %1;" ::"r"(addr), "h"((unsigned short)v) : "memory");
-}
 __device__ __forceinline__ float rsqrt_fast(float x) {  // one MUFU.RSQ (2 ulp); callers keep x out of the denormals
   float y;
   asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
-}
-__device__ __forceinline__ unsigned lanemask_lt() {
-  unsigned m;
-  asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
-  return m;
 }
 __device__ __forceinline__ float u2f(unsigned u) { return __uint_as_float(u); }
 
@@ -482,9 +473,10 @@ constexpr int HMAX = 216;                      // halo cells of the largest tile
 constexpr int HTAB = 224;                      // table size (HMAX + 1 rounded up)
 static_assert(HMAX + 1 <= HTAB, "halo table");
 constexpr unsigned LCAP = 128;                 // per-particle list capacity
-constexpr unsigned LROW = LCAP + 8;            // row pitch of the list build's shared-memory rows (bank spread, 16-byte aligned)
 constexpr int SCH = 4;                         // candidate chunks (of 32) held in registers at a time
-constexpr int BATCH = 16;                      // own particles per row batch of the list build
+constexpr unsigned MAXCAND = 512;               // candidates (particles of a cell's 27-cell stencil) per window of the list build
+constexpr unsigned MSTRIDE = 17;                // words per particle slot of the hit masks (MAXCAND / 32 + 1: bank spread)
+constexpr unsigned BUILD_SCRATCH16 = (32 * MSTRIDE * 4 + 2 * MAXCAND * 2) / 2;  // per-warp scratch of the list build, in 16-bit units
 
 struct TileSmem {
   float4* spos;      // [cap] (x_rel, y_rel, z_rel, bits(tag | type << 31))
@@ -631,14 +623,18 @@ __global__ void __launch_bounds__(128) k_tile_stats(const DevP p) {
 }
 
 // ----------------------------------------------------------------------------------------------------------------
-// a3: Verlet list (full list: every j != i with r < rc + skin at build time).
-// One warp per own cell.  The candidates of the cell's 27-cell stencil are nine contiguous runs of the staged array
-// (one per (y, z) row of halo cells); they are flattened and held IN REGISTERS, 8 chunks of 32 (one candidate per
-// lane and chunk), while the warp loops over the cell's own particles: one broadcast load of x_i, 32 distances per
-// instruction, one ballot, and the hits are appended to particle i's row in shared memory at ballot-prefix positions
-// (entries in increasing candidate order: deterministic).  Rows are then written out as 16-byte chunks of 8 16-bit
-// staged-slot indices, layout [chunk][i] (coalesced both here and in the density / force passes), padded with the
-// sentinel slot.
+// a3: Verlet list (full list: every j != i with r < rc + skin at build time).  Two phases per pair of own cells.
+//
+// Phase 1, warp per cell ("32 distances per instruction"): the candidates of the cell's 27-cell stencil are nine
+// contiguous runs of the staged array (one per (y, z) row of halo cells); they are flattened and held IN REGISTERS,
+// SCH chunks of 32 at a time (one candidate per lane and chunk), while the warp loops over the cell's own particles:
+// one broadcast load of x_i, one distance per lane, one ballot -- the 32-bit hit mask of (particle, chunk) goes to
+// shared memory.  No per-hit work at all in this phase.
+//
+// Phase 2, thread per particle: the two cells of the pair occupy the two half-warps; every lane walks the set bits
+// of its particle's masks in increasing candidate order (deterministic), looks the staged slot up in the cell's
+// candidate table and pushes it through a 128-bit shift register; every 8 entries one 16-byte chunk is stored
+// straight to the list, layout [chunk][i], the last chunk padded with the sentinel slot.
 // ----------------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_build_list(const DevP p) {
   if (!p.ctl->rebuild) return;
@@ -665,101 +661,155 @@ __global__ void __launch_bounds__(256) k_build_list(const DevP p) {
     return;
   }
   const int hxn = T.ex + 2, hyn = T.ey + 2;
-  // per-warp scratch behind the tables: BATCH rows of LROW entries + BATCH counters
-  unsigned short* const rows = sm.queue + (size_t)warp * (BATCH * LROW + 2 * BATCH);
-  unsigned* const cnt = (unsigned*)(rows + BATCH * LROW);
+  // per-warp scratch behind the tables: hit masks [32 particle slots][MSTRIDE] and two candidate tables [MAXCAND]
+  unsigned* const masks = (unsigned*)(sm.queue + (size_t)warp * BUILD_SCRATCH16);
+  unsigned short* const tables = (unsigned short*)(masks + 32 * MSTRIDE);
   const unsigned sent = p.tile_cap;
-  const unsigned ltmask = lanemask_lt();
-  const unsigned rows_a = smem_addr(rows);
   unsigned smax = 0, ssum = 0;
   bool sover = false;
-  for (unsigned oc = warp; oc < T.ncell_own; oc += nwarps) {
-    const int lx = oc % T.ex, ly = (oc / T.ex) % T.ey, lz = oc / (T.ex * T.ey);
-    const int hown = ((lz + 1) * hyn + (ly + 1)) * hxn + lx + 1;
-    const unsigned lb = sm.hbase[hown], nown = sm.hbase[hown + 1] - lb;
-    if (nown == 0) continue;
-    const unsigned gb = sm.hstart[hown];
-    // the nine candidate runs: lane r < 9 holds run r = (dz, dy); inclusive scan of the run lengths
-    unsigned run_b = 0, run_n = 0;
-    if (lane < 9) {
-      const int hrow = ((lz + lane / 3) * hyn + (ly + lane % 3)) * hxn + lx;
-      run_b = sm.hbase[hrow];
-      run_n = sm.hbase[hrow + 3] - run_b;
-    }
-    unsigned incl = run_n;
+  const int half = lane >> 4, hl = lane & 15;
+  for (unsigned oc0 = 2 * warp; oc0 < T.ncell_own; oc0 += 2 * nwarps) {
+    // the pair's cells: geometry of each (warp-uniform)
+    unsigned c_lb[2], c_n[2], c_gb[2], c_nch[2];
 #pragma unroll
-    for (int o = 1; o < 16; o <<= 1) {
-      const unsigned t = __shfl_up_sync(0xffffffffu, incl, o);
-      if (lane >= o) incl += t;
-    }
-    const unsigned ncand = __shfl_sync(0xffffffffu, incl, 8);
-    const unsigned run_o = incl - run_n;  // exclusive offset of the lane's run
-    unsigned rend[9];
-#pragma unroll
-    for (int r = 0; r < 9; ++r) rend[r] = __shfl_sync(0xffffffffu, incl, r);
-    for (unsigned b0 = 0; b0 < nown; b0 += BATCH) {
-      const unsigned nb = min((unsigned)BATCH, nown - b0);
-      // rows start filled with the sentinel: whatever lies behind a list's end is padding
-      {
-        const unsigned s2 = sent | (sent << 16);
-        uint4* r4 = (uint4*)rows;
-        for (int q = lane; q < BATCH * LROW / 8; q += 32) r4[q] = make_uint4(s2, s2, s2, s2);
-        if (lane < BATCH) cnt[lane] = 0u;
+    for (int hh = 0; hh < 2; ++hh) {
+      const unsigned oc = oc0 + hh;
+      c_lb[hh] = c_n[hh] = c_gb[hh] = c_nch[hh] = 0;
+      if (oc < T.ncell_own) {
+        const int lx = oc % T.ex, ly = (oc / T.ex) % T.ey, lz = oc / (T.ex * T.ey);
+        const int hown = ((lz + 1) * hyn + (ly + 1)) * hxn + lx + 1;
+        c_lb[hh] = sm.hbase[hown];
+        c_n[hh] = sm.hbase[hown + 1] - c_lb[hh];
+        c_gb[hh] = sm.hstart[hown];
       }
-      __syncwarp();
-      for (unsigned sc = 0; sc < ncand; sc += 32 * SCH) {
-        float cx[SCH], cy[SCH], cz[SCH];
-        unsigned cs[SCH];
+    }
+    const unsigned rounds = (max(c_n[0], c_n[1]) + 15u) >> 4;  // 16 particle slots per cell and round
+    for (unsigned rd = 0; rd < rounds; ++rd) {
+      const unsigned b0 = rd * 16u;
+      // phase-2 state of the lane's particle; it persists over the candidate windows
+      const bool act = b0 + hl < (half ? c_n[1] : c_n[0]);
+      const unsigned self = (half ? c_lb[1] : c_lb[0]) + b0 + hl;
+      const unsigned gi = (half ? c_gb[1] : c_gb[0]) + b0 + hl;
+      uint4* out = p.nbr + gi;
+      unsigned a0 = 0, a1 = 0, a2 = 0, a3 = 0, n = 0;
+      bool more = true;
+      for (unsigned win = 0; more; win += MAXCAND) {  // windows of MAXCAND candidates (one window unless very dense)
+        more = false;
+        // ---------------- phase 1: hit masks of this round's particles, cell by cell ----------------
 #pragma unroll
-        for (int t = 0; t < SCH; ++t) {  // flat candidate index -> staged slot (past the end: the sentinel, never hit)
-          const unsigned f = sc + t * 32 + lane;
-          unsigned r = 0;
-#pragma unroll
-          for (int q = 0; q < 8; ++q) r += (f >= rend[q]) ? 1u : 0u;
-          const unsigned rb = __shfl_sync(0xffffffffu, run_b, r), ro = __shfl_sync(0xffffffffu, run_o, r);
-          cs[t] = f < ncand ? rb + (f - ro) : sent;
-          const float4 xj = sm.spos[cs[t]];
-          cx[t] = xj.x;
-          cy[t] = xj.y;
-          cz[t] = xj.z;
-        }
-        for (unsigned il = 0; il < nb; ++il) {
-          const unsigned self = lb + b0 + il;
-          const float4 xi = sm.spos[self];  // warp-uniform: broadcast
-          unsigned c = cnt[il];
-          const unsigned row = rows_a + il * (LROW * 2);
-#pragma unroll
-          for (int t = 0; t < SCH; ++t) {
-            const float dx = xi.x - cx[t], dy = xi.y - cy[t], dz = xi.z - cz[t];
-            const float r2 = dx * dx + dy * dy + dz * dz;
-            const bool hit = r2 < p.rlist2 && cs[t] != self;
-            const unsigned b = __ballot_sync(0xffffffffu, hit);
-            const unsigned pos = c + __popc(b & ltmask);
-            if (hit && pos < LCAP) sts_u16(row + pos * 2, cs[t]);
-            c += __popc(b);
+        for (int hh = 0; hh < 2; ++hh) {
+          c_nch[hh] = 0;
+          if (b0 >= c_n[hh]) continue;  // warp-uniform
+          const unsigned nb = min(16u, c_n[hh] - b0);
+          const unsigned oc = oc0 + hh;
+          const int lx = oc % T.ex, ly = (oc / T.ex) % T.ey, lz = oc / (T.ex * T.ey);
+          // the nine candidate runs: lane r < 9 holds run r = (dz, dy); inclusive scan of the run lengths
+          unsigned run_b = 0, run_n = 0;
+          if (lane < 9) {
+            const int hrow = ((lz + lane / 3) * hyn + (ly + lane % 3)) * hxn + lx;
+            run_b = sm.hbase[hrow];
+            run_n = sm.hbase[hrow + 3] - run_b;
           }
-          if (lane == 0) cnt[il] = c;
+          unsigned incl = run_n;
+#pragma unroll
+          for (int o = 1; o < 16; o <<= 1) {
+            const unsigned t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += t;
+          }
+          const unsigned ncand = __shfl_sync(0xffffffffu, incl, 8);
+          if (win >= ncand) continue;  // this cell has no candidates left
+          const unsigned wend = min(ncand, win + MAXCAND);
+          if (wend < ncand) more = true;
+          c_nch[hh] = (wend - win + 31u) >> 5;
+          const unsigned run_o = incl - run_n;  // exclusive offset of the lane's run
+          unsigned rend[8];
+#pragma unroll
+          for (int r = 0; r < 8; ++r) rend[r] = __shfl_sync(0xffffffffu, incl, r);
+          unsigned short* const tb = tables + hh * MAXCAND;
+          unsigned* const mrow = masks + (hh * 16) * MSTRIDE;
+          for (unsigned sc = win; sc < wend; sc += 32 * SCH) {
+            float cx[SCH], cy[SCH], cz[SCH];
+#pragma unroll
+            for (int t = 0; t < SCH; ++t) {  // flat candidate index -> staged slot (past the end: the sentinel, never hit)
+              const unsigned f = sc + t * 32 + lane;
+              unsigned r = 0;
+#pragma unroll
+              for (int q = 0; q < 8; ++q) r += (f >= rend[q]) ? 1u : 0u;
+              const unsigned rb = __shfl_sync(0xffffffffu, run_b, r), ro = __shfl_sync(0xffffffffu, run_o, r);
+              const unsigned cs = f < wend ? rb + (f - ro) : sent;
+              if (f - win < MAXCAND) tb[f - win] = (unsigned short)cs;
+              const float4 xj = sm.spos[cs];
+              cx[t] = xj.x;
+              cy[t] = xj.y;
+              cz[t] = xj.z;
+            }
+            const unsigned ch0 = (sc - win) >> 5;
+            for (unsigned il = 0; il < nb; ++il) {
+              const float4 xi = sm.spos[c_lb[hh] + b0 + il];  // warp-uniform: broadcast
+              unsigned* const mr = mrow + il * MSTRIDE + ch0;
+#pragma unroll
+              for (int t = 0; t < SCH; ++t) {
+                const float dx = xi.x - cx[t], dy = xi.y - cy[t], dz = xi.z - cz[t];
+                const float r2 = dx * dx + dy * dy + dz * dz;
+                const unsigned b = __ballot_sync(0xffffffffu, r2 < p.rlist2);
+                if (lane == 0) mr[t] = b;
+              }
+            }
+          }
+        }
+        __syncwarp();
+        // ---------------- phase 2: lane = particle; decode the window's masks into the list ----------------
+        {
+          const unsigned nch = act ? (half ? c_nch[1] : c_nch[0]) : 0u;
+          const unsigned* const mr = masks + lane * MSTRIDE;
+          const unsigned short* const tb = tables + half * MAXCAND;
+          // one loop, two kinds of iteration: fetch the next mask word, or consume the lowest set bit of the current one
+          unsigned t = 0, w = 0;
+          unsigned left = nch;  // mask words not fetched yet
+          while (left | w) {
+            if (w == 0u) {
+              w = mr[t];
+              ++t;
+              --left;
+            } else {
+              const unsigned b = __ffs(w) - 1u;
+              w &= w - 1u;
+              const unsigned slot = tb[(t - 1u) * 32u + b];
+              if (slot != self) {
+                a0 = __funnelshift_r(a0, a1, 16);
+                a1 = __funnelshift_r(a1, a2, 16);
+                a2 = __funnelshift_r(a2, a3, 16);
+                a3 = __funnelshift_r(a3, slot, 16);
+                ++n;
+                if ((n & 7u) == 0u && n <= p.cap) {
+                  *out = make_uint4(a0, a1, a2, a3);
+                  out += p.N;
+                }
+              }
+            }
+          }
         }
         __syncwarp();
       }
-      // write the batch out: lane = particle, one 16-byte chunk per iteration
-      unsigned n = lane < nb ? cnt[lane] : 0u;
-      const unsigned gi = gb + b0 + lane;
-      if (lane < nb && (n > LCAP || n > p.cap)) {  // reported as MDPD_EOVERFLOW; this particle's list is emptied
-        sover = true;
-        n = 0;
+      if ((n & 7u) && n <= p.cap) {  // last, partial chunk: pad with the sentinel
+        for (unsigned q = n & 7u; q < 8u; ++q) {
+          a0 = __funnelshift_r(a0, a1, 16);
+          a1 = __funnelshift_r(a1, a2, 16);
+          a2 = __funnelshift_r(a2, a3, 16);
+          a3 = __funnelshift_r(a3, sent, 16);
+        }
+        *out = make_uint4(a0, a1, a2, a3);
       }
-      const unsigned mx = __reduce_max_sync(0xffffffffu, n);
-      const uint4* const myrow = (const uint4*)(rows + lane * LROW);
-      for (unsigned ch = 0; ch * 8 < mx; ++ch)
-        if (ch * 8 < n) p.nbr[(size_t)ch * p.N + gi] = myrow[ch];
-      if (lane < nb) {
+      if (act) {
+        if (n > p.cap) {  // reported as MDPD_EOVERFLOW; this particle's list is emptied
+          sover = true;
+          n = 0;
+        }
         p.nnbr[gi] = n;
-        p.self_loc[gi] = (unsigned short)(lb + b0 + lane);
+        p.self_loc[gi] = (unsigned short)self;
         smax = max(smax, n);
         ssum += n;
       }
-      __syncwarp();
     }
   }
   // statistics + overflow flag
@@ -1577,7 +1627,7 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
   }
   h->smem_pos = tile_smem_bytes(h->d.tile_cap, false, 0);
   h->smem_posvel = tile_smem_bytes(h->d.tile_cap, true, 0);
-  h->smem_build = tile_smem_bytes(h->d.tile_cap, false, (size_t)(BATCH * LROW + 2 * BATCH) * (h->block_build / 32));
+  h->smem_build = tile_smem_bytes(h->d.tile_cap, false, (size_t)BUILD_SCRATCH16 * (h->block_build / 32));
   if (h->smem_build > h->smem_limit) return set_err(h, MDPD_ENOMEM, "list build needs %zu bytes of shared memory", h->smem_build);
   CU_TRY(h, cudaFuncSetAttribute(k_build_list, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_build));
   CU_TRY(h, cudaFuncSetAttribute(k_density<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
