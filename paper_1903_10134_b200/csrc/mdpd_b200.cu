@@ -469,6 +469,9 @@ __global__ void __launch_bounds__(TPB) k_permute(const DevP p) {
 #ifndef MINB
 #define MINB 3
 #endif
+#ifndef TILE_TPB
+#define TILE_TPB 448  // most threads per CTA of the density / force passes
+#endif
 constexpr int HMAX = 216;                      // halo cells of the largest tile
 constexpr int HTAB = 224;                      // table size (HMAX + 1 rounded up)
 static_assert(HMAX + 1 <= HTAB, "halo table");
@@ -479,16 +482,19 @@ constexpr unsigned MSTRIDE = 17;                // words per particle slot of th
 constexpr unsigned BUILD_SCRATCH16 = (32 * MSTRIDE * 4 + 2 * MAXCAND * 2) / 2;  // per-warp scratch of the list build, in 16-bit units
 
 struct TileSmem {
-  float4* spos;      // [cap] (x_rel, y_rel, z_rel, bits(tag | type << 31))
-  float4* svel;      // [cap] (vx, vy, vz, rho)            (force pass only)
+  float4* spos;      // [cap + 1] (x_rel, y_rel, z_rel, bits(tag | type << 31)); slot cap = the far-away sentinel
+  float4* svel;      // [cap + 1] (vx, vy, vz, rho)            (force pass only)
+  float4* hshift;    // [HTAB] (sx, sy, sz, bits(delta)) of halo cell h: x_rel = x + s, global index = staged slot + delta
   unsigned* hbase;   // [HTAB] first staged slot of halo cell h; hbase[nh] = number of staged particles
-  unsigned* hstart;  // [HTAB] global index of the first particle of halo cell h
   unsigned short* queue;  // scratch behind the tables (list build: per-warp rows)
 };
 
+constexpr size_t TILE_SLOT_BYTES = 32;  // pos + vel: shared-memory bytes per staged slot of the force pass
+constexpr unsigned PERM_MAX = HTAB * 8; // own particles whose order fits the (dead after staging) hshift table
+
 // queue_entries: 16-bit scratch entries behind the tables (list build: rows per warp)
 __host__ __device__ inline size_t tile_smem_bytes(unsigned cap, bool with_vel, size_t queue_entries) {
-  return (size_t)(cap + 1) * 16 * (with_vel ? 2 : 1) + 2 * HTAB * 4 + queue_entries * 2;  // + sentinel slot
+  return (size_t)(cap + 1) * 16 * (with_vel ? 2 : 1) + HTAB * 16 + HTAB * 4 + queue_entries * 2;  // + sentinel slot
 }
 
 __device__ __forceinline__ TileSmem carve_smem(unsigned char* raw, unsigned cap, bool with_vel) {
@@ -497,29 +503,26 @@ __device__ __forceinline__ TileSmem carve_smem(unsigned char* raw, unsigned cap,
   raw += (size_t)(cap + 1) * 16;
   s.svel = (float4*)raw;
   if (with_vel) raw += (size_t)(cap + 1) * 16;
+  s.hshift = (float4*)raw;
+  raw += HTAB * 16;
   s.hbase = (unsigned*)raw;
-  raw += HTAB * 4;
-  s.hstart = (unsigned*)raw;
   raw += HTAB * 4;
   s.queue = (unsigned short*)raw;
   return s;
 }
 
-// coordinate of halo position hx in one dimension: wrapped cell index and the two addends of
-//   x_rel = (x + s1) + s2   (both additions exact for own-tile particles)
-__device__ __forceinline__ int halo_cell(int c0, int hx, int nc, float L, float o, float& s1, float& s2) {
+// coordinate of halo position hx in one dimension: wrapped cell index and the shift s of x_rel = x + s (tile origin
+// and periodic image folded into one addend; the addition is exact for own-tile particles)
+__device__ __forceinline__ int halo_cell(int c0, int hx, int nc, float L, float o, float& s) {
   int c = c0 + hx - 1;
-  if (c < 0) {            // image on the low side: only tiles with c0 == 0 (o == 0)
+  if (c < 0) {            // image on the low side: only tiles with c0 == 0, whose origin o is 0
     c += nc;
-    s1 = -L;
-    s2 = -o;
+    s = -L;
   } else if (c >= nc) {   // image on the high side
     c -= nc;
-    s1 = L - o;
-    s2 = 0.0f;
+    s = L - o;
   } else {
-    s1 = -o;
-    s2 = 0.0f;
+    s = -o;
   }
   return c;
 }
@@ -534,16 +537,16 @@ __device__ __forceinline__ unsigned stage_tile(const DevP& p, const TileInfo& T,
   const int hxn = T.ex + 2, hyn = T.ey + 2, hzn = T.ez + 2;
   const int nh = hxn * hyn * hzn;
   const float ox = tile_origin(T.c0x, p.edge_x), oy = tile_origin(T.c0y, p.edge_y), oz = tile_origin(T.c0z, p.edge_z);
-  for (int h = threadIdx.x; h < nh; h += blockDim.x) {
+  for (int h = threadIdx.x; h < nh; h += blockDim.x) {  // one halo cell per thread: where it is, how many, which shift
     const int hx = h % hxn, hy = (h / hxn) % hyn, hz = h / (hxn * hyn);
-    float a, b;
-    const int cx = halo_cell(T.c0x, hx, p.ncx, p.Lx, ox, a, b);
-    const int cy = halo_cell(T.c0y, hy, p.ncy, p.Ly, oy, a, b);
-    const int cz = halo_cell(T.c0z, hz, p.ncz, p.Lz, oz, a, b);
+    float sx, sy, sz;
+    const int cx = halo_cell(T.c0x, hx, p.ncx, p.Lx, ox, sx);
+    const int cy = halo_cell(T.c0y, hy, p.ncy, p.Ly, oy, sy);
+    const int cz = halo_cell(T.c0z, hz, p.ncz, p.Lz, oz, sz);
     const unsigned r = p.cell_rank[((unsigned)cz * p.ncy + cy) * p.ncx + cx];
     const unsigned s = p.cell_start[r];
-    sm.hstart[h] = s;
     sm.hbase[h] = p.cell_start[r + 1] - s;
+    sm.hshift[h] = make_float4(sx, sy, sz, u2f(s));
   }
   __syncthreads();
   if (threadIdx.x < 32) {  // exclusive scan of the counts by warp 0
@@ -566,27 +569,24 @@ __device__ __forceinline__ unsigned stage_tile(const DevP& p, const TileInfo& T,
   __syncthreads();
   const unsigned total = sm.hbase[nh];
   if (total > p.tile_cap) return 0xFFFFFFFFu;
-  // one staged slot per thread and iteration; the halo cell of a slot is found by bisection of hbase (loads of
-  // different iterations are independent: several are in flight per thread)
+  // slot -> halo cell map: one byte per slot, kept in the slot itself until the slot is filled (by the thread that
+  // reads the byte); and the slot -> global index offset of every cell
+  unsigned char* const cellof = (unsigned char*)sm.spos;
+  for (int h = threadIdx.x; h < nh; h += blockDim.x) {
+    const unsigned b = sm.hbase[h], e = sm.hbase[h + 1];
+    sm.hshift[h].w = u2f(f2u(sm.hshift[h].w) - b);
+    for (unsigned k = b; k < e; ++k) cellof[(size_t)k * 16] = (unsigned char)h;
+  }
+  __syncthreads();
+  // one staged slot per thread and iteration (loads of different iterations are independent: several are in flight)
 #pragma unroll 4
   for (unsigned sl = threadIdx.x; sl < total; sl += blockDim.x) {
-    int lo = 0, hi = nh;  // hbase[lo] <= sl < hbase[hi]
-    while (hi - lo > 1) {
-      const int mid = (lo + hi) >> 1;
-      if (sm.hbase[mid] <= sl) lo = mid;
-      else hi = mid;
-    }
-    const int h = lo;
-    const int hx = h % hxn, hy = (h / hxn) % hyn, hz = h / (hxn * hyn);
-    float ax, bx, ay, by, az, bz;
-    halo_cell(T.c0x, hx, p.ncx, p.Lx, ox, ax, bx);
-    halo_cell(T.c0y, hy, p.ncy, p.Ly, oy, ay, by);
-    halo_cell(T.c0z, hz, p.ncz, p.Lz, oz, az, bz);
-    const unsigned g = sm.hstart[h] + (sl - sm.hbase[h]);
+    const float4 sh = sm.hshift[cellof[(size_t)sl * 16]];
+    const unsigned g = sl + f2u(sh.w);
     float4 x = pos[g];
-    x.x = (x.x + ax) + bx;
-    x.y = (x.y + ay) + by;
-    x.z = (x.z + az) + bz;
+    x.x += sh.x;
+    x.y += sh.y;
+    x.z += sh.z;
     sm.spos[sl] = x;
     if (WITH_VEL) sm.svel[sl] = vel[g];
   }
@@ -609,9 +609,9 @@ __global__ void __launch_bounds__(128) k_tile_stats(const DevP p) {
   unsigned halo = 0;
   for (int h = lane; h < nh; h += 32) {
     const int hx = h % hxn, hy = (h / hxn) % hyn, hz = h / (hxn * hyn);
-    float a, b;
-    const int cx = halo_cell(T.c0x, hx, p.ncx, 0.f, 0.f, a, b), cy = halo_cell(T.c0y, hy, p.ncy, 0.f, 0.f, a, b),
-              cz = halo_cell(T.c0z, hz, p.ncz, 0.f, 0.f, a, b);
+    float a;
+    const int cx = halo_cell(T.c0x, hx, p.ncx, 0.f, 0.f, a), cy = halo_cell(T.c0y, hy, p.ncy, 0.f, 0.f, a),
+              cz = halo_cell(T.c0z, hz, p.ncz, 0.f, 0.f, a);
     const unsigned r = p.cell_rank[((unsigned)cz * p.ncy + cy) * p.ncx + cx];
     halo += p.cell_start[r + 1] - p.cell_start[r];
   }
@@ -680,7 +680,7 @@ __global__ void __launch_bounds__(256) k_build_list(const DevP p) {
         const int hown = ((lz + 1) * hyn + (ly + 1)) * hxn + lx + 1;
         c_lb[hh] = sm.hbase[hown];
         c_n[hh] = sm.hbase[hown + 1] - c_lb[hh];
-        c_gb[hh] = sm.hstart[hown];
+        c_gb[hh] = c_lb[hh] + f2u(sm.hshift[hown].w);
       }
     }
     const unsigned rounds = (max(c_n[0], c_n[1]) + 15u) >> 4;  // 16 particle slots per cell and round
@@ -848,7 +848,7 @@ __device__ __forceinline__ unsigned list_entry(const uint4& e, const int t) {  /
 // list is assembled 8 entries at a time in four registers (a 128-bit shift register) and stored as 16-byte chunks.
 // ----------------------------------------------------------------------------------------------------------------
 template <bool HAS_WALL>
-__global__ void __launch_bounds__(512, MINB) k_density(const DevP p) {
+__global__ void __launch_bounds__(TILE_TPB, MINB) k_density(const DevP p) {
   extern __shared__ __align__(16) unsigned char smraw[];
   const TileSmem sm = carve_smem(smraw, p.tile_cap, false);
   const unsigned cur = p.ctl->cur;
@@ -951,34 +951,80 @@ __device__ __forceinline__ void pair_force(const DevP& p, const float4 xi, const
   acc.z += Fr * dz;
 }
 
+// Own particles are handed to the threads in order of decreasing list length (a counting sort on the length, in shared
+// memory): the lanes of a warp then finish together, and the warp leaves the entry loop at its longest list instead
+// of at the next multiple of 8.  Which thread evaluates which particle does not change any result.
 template <bool ALL>  // ALL: also evaluate the (never used) forces on frozen particles, for parity checks
-__global__ void __launch_bounds__(512, MINB) k_force(const DevP p) {
+__global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
   extern __shared__ __align__(16) unsigned char smraw[];
   const TileSmem sm = carve_smem(smraw, p.tile_cap, true);
   const unsigned cur = p.ctl->cur;
   const TileInfo T = p.tiles[blockIdx.x];
   if (stage_tile<true>(p, T, p.pos[cur], p.vel[cur], sm) == 0xFFFFFFFFu) return;
   const unsigned os = p.cell_start[T.rank0], oe = p.cell_start[T.rank0 + T.ncell_own];
+  const unsigned nown = oe - os;
+  // counting sort of the own particles by list length, longest first: hist in the (dead) hbase table, order in map
+  unsigned* const hist = sm.hbase;            // [LCAP + 1] <= HTAB
+  unsigned short* const perm = (unsigned short*)sm.hshift;  // [nown] if nown <= PERM_MAX, else no sorting
+  const bool sorted = nown <= PERM_MAX;  // block-uniform
+  if (sorted) {
+    for (unsigned k = threadIdx.x; k <= LCAP; k += blockDim.x) hist[k] = 0u;
+    __syncthreads();
+    for (unsigned t = threadIdx.x; t < nown; t += blockDim.x) {
+      unsigned na = p.nact[os + t];
+      if (!ALL && (f2u(sm.spos[p.self_loc[os + t]].w) >> 31)) na = 0u;  // frozen: nothing to evaluate
+      atomicAdd(&hist[LCAP - min(na, LCAP)], 1u);                       // bin 0 = longest
+    }
+    __syncthreads();
+    if (threadIdx.x < 32) {  // exclusive scan of the LCAP + 1 bins by warp 0
+      const int lane = threadIdx.x;
+      unsigned run = 0;
+      for (unsigned b0 = 0; b0 <= LCAP; b0 += 32) {
+        const unsigned k = b0 + lane;
+        const unsigned c = k <= LCAP ? hist[k] : 0u;
+        unsigned incl = c;
+  #pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          const unsigned v = __shfl_up_sync(0xffffffffu, incl, o);
+          if (lane >= o) incl += v;
+        }
+        if (k <= LCAP) hist[k] = run + incl - c;
+        run += __shfl_sync(0xffffffffu, incl, 31);
+      }
+    }
+    __syncthreads();
+    for (unsigned t = threadIdx.x; t < nown; t += blockDim.x) {
+      unsigned na = p.nact[os + t];
+      if (!ALL && (f2u(sm.spos[p.self_loc[os + t]].w) >> 31)) na = 0u;
+      perm[atomicAdd(&hist[LCAP - min(na, LCAP)], 1u)] = (unsigned short)t;
+    }
+    __syncthreads();
+  }
   const HashKeys K = make_keys(p.ctl->step, p.seed);
-  for (unsigned i = os + threadIdx.x; i < oe; i += blockDim.x) {
+  for (unsigned t0 = 0; t0 < nown; t0 += blockDim.x) {  // every warp runs the same number of rounds
+    const unsigned t = t0 + threadIdx.x;
+    const bool valid = t < nown;
+    const unsigned i = os + (valid ? (sorted ? (unsigned)perm[t] : t) : 0u);
     const unsigned li = p.self_loc[i];
     const float4 xi = sm.spos[li];
     const unsigned wi = f2u(xi.w);
     const unsigned walli = wi >> 31;
-    if (!ALL && walli) continue;
+    const bool work = valid && (ALL || !walli);
     const unsigned tagi = wi & 0x7FFFFFFFu;
     const float4 vi = sm.svel[li];
-    const unsigned na = p.nact[i];
+    const unsigned na = work ? p.nact[i] : 0u;
+    const unsigned namax = __reduce_max_sync(0xffffffffu, na);
     ForceAcc acc = {0.f, 0.f, 0.f};
     const uint4* __restrict__ lst = p.act + i;
     uint4 nxt = na ? lst[0] : make_uint4(0, 0, 0, 0);
-    for (unsigned k0 = 0; k0 < na; k0 += 8) {
+    for (unsigned k0 = 0; k0 < namax; k0 += 8) {
       const uint4 e = nxt;
       if (k0 + 8 < na) nxt = lst[(size_t)((k0 >> 3) + 1) * p.N];  // next chunk in flight
 #pragma unroll
-      for (int t = 0; t < 8; ++t) {
-        if (k0 + t < na) {
-          const unsigned j = list_entry(e, t);
+      for (int q = 0; q < 8; ++q) {
+        if (k0 + q >= namax) break;  // warp-uniform
+        if (k0 + q < na) {
+          const unsigned j = list_entry(e, q);
           const float4 xj = sm.spos[j];
           const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
           const float r2 = dx * dx + dy * dy + dz * dz;
@@ -986,12 +1032,14 @@ __global__ void __launch_bounds__(512, MINB) k_force(const DevP p) {
         }
       }
     }
-    if (!walli) {
-      acc.x += p.fgx;
-      acc.y += p.fgy;
-      acc.z += p.fgz;
+    if (work) {
+      if (!walli) {
+        acc.x += p.fgx;
+        acc.y += p.fgy;
+        acc.z += p.fgz;
+      }
+      p.force[i] = make_float4(acc.x, acc.y, acc.z, 0.0f);
     }
-    p.force[i] = make_float4(acc.x, acc.y, acc.z, 0.0f);
   }
 }
 
@@ -1581,10 +1629,10 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
     memcpy(h->tile_dim, tdim, sizeof tdim);
     h->d.ntiles = (unsigned)tiles.size();
     const int vol = tdim[0] * tdim[1] * tdim[2];
-    h->block = 512u;  // upper bound while the capacity is probed; set from the tile population below
+    h->block = TILE_TPB;  // upper bound while the capacity is probed; set from the tile population below
     h->block_build = vol >= 32 ? 256u : 128u;
     const size_t fixed = tile_smem_bytes(0, true, 0);
-    const unsigned cap_limit = (unsigned)std::min<size_t>((h->smem_limit - fixed) / 32, 65535);
+    const unsigned cap_limit = (unsigned)std::min<size_t>((h->smem_limit - fixed) / TILE_SLOT_BYTES, 65535);
     h->d.tile_cap = cap_limit;
     LAUNCH(h, PS_OTHER, (k_ctl_init<<<1, 1, 0, h->stream>>>(h->d)));  // the initial sort reads buffer 0 and writes buffer 1
     CU_TRY(h, cudaMemcpyAsync(h->d.cell_rank, rank.data(), rank.size() * 4, cudaMemcpyHostToDevice, h->stream));
@@ -1603,10 +1651,10 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
       continue;  // try the next smaller tile shape
     }
     // density / force passes: one thread per own particle of the fullest tile (a tile with more loops)
-    h->block = std::min(512u, std::max(64u, (h->h_ctl->max_own + 31u) / 32u * 32u));
+    h->block = std::min<unsigned>(TILE_TPB, std::max(64u, (h->h_ctl->max_own + 31u) / 32u * 32u));
     if (const char* e = getenv("MDPD_BLOCK")) {
       int b = atoi(e);
-      if (b >= 32 && b <= 512 && b % 32 == 0) h->block = (unsigned)b;
+      if (b >= 32 && b <= TILE_TPB && b % 32 == 0) h->block = (unsigned)b;
     }
     if (const char* e = getenv("MDPD_BLOCK_BUILD")) {
       int b = atoi(e);
@@ -1621,7 +1669,7 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
       const size_t per_cta = tile_smem_bytes(want, true, 0) + 1024;
       const size_t ctas = std::max<size_t>(1, sm_total / per_cta);
       const size_t room = sm_total / ctas - 1024 - fixed;
-      h->d.tile_cap = std::max<unsigned>(want, std::min<unsigned>(cap_limit, (unsigned)(room / 32 / 64 * 64)));
+      h->d.tile_cap = std::max<unsigned>(want, std::min<unsigned>(cap_limit, (unsigned)(room / TILE_SLOT_BYTES / 64 * 64)));
     }
     break;
   }
