@@ -31,7 +31,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if force or needs_build():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         tmp = LIB + f".tmp{os.getpid()}"
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SRC
+        extra = os.environ.get("MDPD_NVCC_EXTRA", "").split()   # e.g. "-DTILE_TPB=448" for tuning experiments
+        cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SRC
         subprocess.check_call(cmd)
         os.replace(tmp, LIB)
     return LIB

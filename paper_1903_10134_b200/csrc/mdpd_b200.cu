@@ -45,6 +45,7 @@ struct Ctl {
   unsigned max_own;   // most particles in a tile at the last build
   unsigned has_wall;  // some particle is frozen (set by k_pack)
   unsigned long long steps, rebuilds, bounces, sum_nbr, overflow, nan_events, sum_act, dens_passes, graph_rebuilds, pad2;
+  unsigned long long ph[4];  // -DMDPD_PHASES: clock cycles of k_force's staging / sort / pair loop, summed over CTAs, and the CTA count
 };
 
 struct TileInfo {  // one CTA of the list / density / force passes
@@ -470,7 +471,7 @@ __global__ void __launch_bounds__(TPB) k_permute(const DevP p) {
 #define MINB 3
 #endif
 #ifndef TILE_TPB
-#define TILE_TPB 448  // most threads per CTA of the density / force passes
+#define TILE_TPB 224  // most threads per CTA of the density / force passes (7 warps x 2 rounds on a full tile)
 #endif
 constexpr int HMAX = 216;                      // halo cells of the largest tile
 constexpr int HTAB = 224;                      // table size (HMAX + 1 rounded up)
@@ -835,9 +836,58 @@ __global__ void k_reset_list_stats(const DevP p) {
   p.ctl->max_own = 0;
 }
 
-__device__ __forceinline__ unsigned list_entry(const uint4& e, const int t) {  // t is a compile-time constant
-  const unsigned w = t < 2 ? e.x : (t < 4 ? e.y : (t < 6 ? e.z : e.w));
-  return (t & 1) ? (w >> 16) : (w & 0xFFFFu);
+// Shared-memory gathers of the hot loops go through 32-bit shared addresses (one LEA per neighbour and array).
+__device__ __forceinline__ unsigned smem_addr(const void* ptr) { return (unsigned)__cvta_generic_to_shared(ptr); }
+__device__ __forceinline__ float4 lds4(unsigned addr) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ unsigned pin(unsigned v) {  // keeps a loop-invariant value in its register (no rematerialisation)
+  asm volatile("" : "+r"(v));
+  return v;
+}
+
+// Own particles are handed to the warps in order of decreasing list length (a counting sort on the length, in shared
+// memory): group g = sorted particles 32 g .. 32 g + 31, so the lanes of a warp finish together; warp w then takes the
+// groups w, 2W-1-w, 2W+w, 4W-1-w, ... (a long group is followed by a short one), so the warps of the CTA finish
+// together too.  Which thread evaluates which particle does not change any result.
+// hist = the (dead after staging) hbase table, perm = the (dead) hshift table.  Returns false (no sorting) if the
+// tile holds more own particles than perm has room for.  All threads of the CTA must call it.
+template <class LenFn>
+__device__ __forceinline__ bool sort_own_by_length(const TileSmem& sm, unsigned nown, LenFn len) {
+  unsigned* const hist = sm.hbase;                          // [LCAP + 1] <= HTAB
+  unsigned short* const perm = (unsigned short*)sm.hshift;  // [nown] if nown <= PERM_MAX
+  if (nown > PERM_MAX) return false;                        // block-uniform
+  for (unsigned k = threadIdx.x; k <= LCAP; k += blockDim.x) hist[k] = 0u;
+  __syncthreads();
+  for (unsigned t = threadIdx.x; t < nown; t += blockDim.x) atomicAdd(&hist[LCAP - min(len(t), LCAP)], 1u);  // bin 0 = longest
+  __syncthreads();
+  if (threadIdx.x < 32) {  // exclusive scan of the LCAP + 1 bins by warp 0
+    const int lane = threadIdx.x;
+    unsigned run = 0;
+    for (unsigned b0 = 0; b0 <= LCAP; b0 += 32) {
+      const unsigned k = b0 + lane;
+      const unsigned c = k <= LCAP ? hist[k] : 0u;
+      unsigned incl = c;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const unsigned v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
+      }
+      if (k <= LCAP) hist[k] = run + incl - c;
+      run += __shfl_sync(0xffffffffu, incl, 31);
+    }
+  }
+  __syncthreads();
+  for (unsigned t = threadIdx.x; t < nown; t += blockDim.x) perm[atomicAdd(&hist[LCAP - min(len(t), LCAP)], 1u)] = (unsigned short)t;
+  __syncthreads();
+  return true;
+}
+
+// group of 32 sorted own particles that warp `warp` of W takes in its round r (see above)
+__device__ __forceinline__ unsigned group_of_round(unsigned r, unsigned warp, unsigned W) {
+  return (r & 1u) ? (r + 1u) * W - 1u - warp : r * W + warp;
 }
 
 // ----------------------------------------------------------------------------------------------------------------
@@ -845,8 +895,33 @@ __device__ __forceinline__ unsigned list_entry(const uint4& e, const int t) {  /
 // CTA = tile; thread = own particle; neighbours are shared-memory loads through the 16-bit list.  The same sweep
 // also emits, for the force pass that follows, the compact list of the entries that are inside rc at THIS step
 // (positions do not change between the two passes): the force pass then touches in-range pairs only.  The compact
-// list is assembled 8 entries at a time in four registers (a 128-bit shift register) and stored as 16-byte chunks.
+// list is assembled 8 entries at a time in four registers (a 128-bit shift register that moves by 16 bits for an
+// in-range entry and by 0 otherwise: no branch) and stored as 16-byte chunks.
 // ----------------------------------------------------------------------------------------------------------------
+template <bool HAS_WALL>
+__device__ __forceinline__ void density_entry(const DevP& p, const unsigned pbase, const float4 xi, const unsigned walli,
+                                              const unsigned j, float& rho, unsigned& a0, unsigned& a1, unsigned& a2,
+                                              unsigned& a3, unsigned& na, uint4*& ao) {
+  const float4 xj = lds4(pbase + (j << 4));  // padding entries hit the far-away sentinel
+  const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
+  const float r2 = dx * dx + dy * dy + dz * dz;
+  const float rr = fmaxf(r2, 1e-30f);
+  const float w = fmaxf(0.0f, 1.0f - (rr * rsqrt_fast(rr)) * p.inv_rd);  // branch-free: 0 beyond rd
+  rho += w * w;
+  bool in = r2 < p.rc2 && r2 > 1e-12f;  // interacts at this step (R10)
+  if (HAS_WALL) in = in && !(walli & (f2u(xj.w) >> 31));  // frozen-frozen pairs do not (R8)
+  const unsigned sh = in ? 16u : 0u;
+  a0 = __funnelshift_r(a0, a1, sh);
+  a1 = __funnelshift_r(a1, a2, sh);
+  a2 = __funnelshift_r(a2, a3, sh);
+  a3 = __funnelshift_r(a3, j, sh);
+  na += sh >> 4;
+  if (in && (na & 7u) == 0u) {
+    *ao = make_uint4(a0, a1, a2, a3);
+    ao += p.N;
+  }
+}
+
 template <bool HAS_WALL>
 __global__ void __launch_bounds__(TILE_TPB, MINB) k_density(const DevP p) {
   extern __shared__ __align__(16) unsigned char smraw[];
@@ -855,44 +930,39 @@ __global__ void __launch_bounds__(TILE_TPB, MINB) k_density(const DevP p) {
   const TileInfo T = p.tiles[blockIdx.x];
   if (stage_tile<false>(p, T, p.pos[cur], nullptr, sm) == 0xFFFFFFFFu) return;  // flagged by k_build_list
   const unsigned os = p.cell_start[T.rank0], oe = p.cell_start[T.rank0 + T.ncell_own];
+  const unsigned nown = oe - os;
+  const bool sorted = sort_own_by_length(sm, nown, [&](unsigned t) { return p.nnbr[os + t]; });
+  const unsigned short* const perm = (const unsigned short*)sm.hshift;
   float4* __restrict__ vel = p.vel[cur];
   const unsigned sent = p.tile_cap;
+  const unsigned pbase = smem_addr(sm.spos);
+  const unsigned warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
+  const unsigned ngroups = (nown + 31u) >> 5;
   unsigned na_sum = 0;
-  for (unsigned i = os + threadIdx.x; i < oe; i += blockDim.x) {
+  for (unsigned r = 0; r * W < ngroups; ++r) {
+    const unsigned g = group_of_round(r, warp, W);
+    const unsigned t = g * 32u + lane;
+    if (g >= ngroups || t >= nown) continue;
+    const unsigned i = os + (sorted ? (unsigned)perm[t] : t);
     const float4 xi = sm.spos[p.self_loc[i]];
     const unsigned walli = f2u(xi.w) >> 31;
     const unsigned nn = p.nnbr[i];
     const uint4* __restrict__ lst = p.nbr + i;
-    uint4* __restrict__ ao = p.act + i;  // next chunk to write
+    uint4* ao = p.act + i;  // next chunk to write
     float rho = 0.0f;
     unsigned a0 = 0, a1 = 0, a2 = 0, a3 = 0, na = 0;
     uint4 nxt = nn ? lst[0] : make_uint4(0, 0, 0, 0);
     for (unsigned k0 = 0; k0 < nn; k0 += 8) {
       const uint4 e = nxt;
       if (k0 + 8 < nn) nxt = lst[(size_t)((k0 >> 3) + 1) * p.N];  // next chunk in flight while this one is evaluated
-#pragma unroll
-      for (int t = 0; t < 8; ++t) {
-        const unsigned j = list_entry(e, t);
-        const float4 xj = sm.spos[j];  // padding entries hit the far-away sentinel
-        const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
-        const float r2 = dx * dx + dy * dy + dz * dz;
-        const float rr = fmaxf(r2, 1e-30f);
-        const float w = fmaxf(0.0f, 1.0f - (rr * rsqrt_fast(rr)) * p.inv_rd);  // branch-free: 0 beyond rd
-        rho += w * w;
-        bool in = r2 < p.rc2 && r2 > 1e-12f;  // interacts at this step (R10)
-        if (HAS_WALL) in = in && !(walli & (f2u(xj.w) >> 31));  // frozen-frozen pairs do not (R8)
-        if (in) {
-          a0 = __funnelshift_r(a0, a1, 16);
-          a1 = __funnelshift_r(a1, a2, 16);
-          a2 = __funnelshift_r(a2, a3, 16);
-          a3 = __funnelshift_r(a3, j, 16);
-          ++na;
-          if ((na & 7u) == 0u) {
-            *ao = make_uint4(a0, a1, a2, a3);
-            ao += p.N;
-          }
-        }
-      }
+      density_entry<HAS_WALL>(p, pbase, xi, walli, e.x & 0xFFFFu, rho, a0, a1, a2, a3, na, ao);
+      density_entry<HAS_WALL>(p, pbase, xi, walli, e.x >> 16, rho, a0, a1, a2, a3, na, ao);
+      density_entry<HAS_WALL>(p, pbase, xi, walli, e.y & 0xFFFFu, rho, a0, a1, a2, a3, na, ao);
+      density_entry<HAS_WALL>(p, pbase, xi, walli, e.y >> 16, rho, a0, a1, a2, a3, na, ao);
+      density_entry<HAS_WALL>(p, pbase, xi, walli, e.z & 0xFFFFu, rho, a0, a1, a2, a3, na, ao);
+      density_entry<HAS_WALL>(p, pbase, xi, walli, e.z >> 16, rho, a0, a1, a2, a3, na, ao);
+      density_entry<HAS_WALL>(p, pbase, xi, walli, e.w & 0xFFFFu, rho, a0, a1, a2, a3, na, ao);
+      density_entry<HAS_WALL>(p, pbase, xi, walli, e.w >> 16, rho, a0, a1, a2, a3, na, ao);
     }
     if (na & 7u) {  // last, partial chunk: pad with the sentinel
       for (unsigned q = na & 7u; q < 8u; ++q) {
@@ -925,18 +995,23 @@ __global__ void __launch_bounds__(TILE_TPB, MINB) k_density(const DevP p) {
 // a6: pair-force pass (Eq. (1); L186 body force)
 //   F_ij = [A wC + B (rho_i + rho_j) wd - gamma wC^2 (e.v_ij) + sigma wC xi_ij / sqrt(dt)] e_ij ,  s = 1
 // Full list: every pair is evaluated from both ends; the symmetric hash makes F_ij = -F_ji bitwise.
-// Walks the compact in-range list the density pass wrote for this step: every evaluated pair interacts.
+// Walks the compact in-range list the density pass wrote for this step: every evaluated pair interacts.  The loop body
+// has no branch: the padding of a particle's last chunk points at the far-away sentinel slot, whose weights clamp to 0.
 // ----------------------------------------------------------------------------------------------------------------
 struct ForceAcc {
   float x, y, z;
 };
 
-__device__ __forceinline__ void pair_force(const DevP& p, const float4 xi, const float4 vi, const unsigned tagi,
-                                           const float4 xj, const float4 vj, const float dx, const float dy,
-                                           const float dz, const float r2, const HashKeys& K, ForceAcc& acc) {
-  const float rinv = rsqrt_fast(r2);  // r2 > 1e-12 here
+__device__ __forceinline__ void force_entry(const DevP& p, const unsigned pbase, const unsigned vbase, const float4 xi,
+                                            const float4 vi, const unsigned tagi, const unsigned j, const HashKeys& K,
+                                            ForceAcc& acc) {
+  const float4 xj = lds4(pbase + (j << 4));
+  const float4 vj = lds4(vbase + (j << 4));
+  const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
+  const float r2 = dx * dx + dy * dy + dz * dz;  // > 1e-12 for list entries; 3e18 for the sentinel
+  const float rinv = rsqrt_fast(r2);
   const float r = r2 * rinv;
-  const float w = 1.0f - r * p.inv_rc;
+  const float w = fmaxf(0.0f, 1.0f - r * p.inv_rc);  // > 0 for in-range entries, 0 for the sentinel
   float F = p.A * w;
   const float wd = fmaxf(0.0f, 1.0f - r * p.inv_rd);
   F += p.B * (vi.w + vj.w) * wd;
@@ -951,96 +1026,84 @@ __device__ __forceinline__ void pair_force(const DevP& p, const float4 xi, const
   acc.z += Fr * dz;
 }
 
-// Own particles are handed to the threads in order of decreasing list length (a counting sort on the length, in shared
-// memory): the lanes of a warp then finish together, and the warp leaves the entry loop at its longest list instead
-// of at the next multiple of 8.  Which thread evaluates which particle does not change any result.
 template <bool ALL>  // ALL: also evaluate the (never used) forces on frozen particles, for parity checks
 __global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
   extern __shared__ __align__(16) unsigned char smraw[];
   const TileSmem sm = carve_smem(smraw, p.tile_cap, true);
   const unsigned cur = p.ctl->cur;
   const TileInfo T = p.tiles[blockIdx.x];
+#ifdef MDPD_PHASES
+  const long long ph_t0 = clock64();
+#endif
   if (stage_tile<true>(p, T, p.pos[cur], p.vel[cur], sm) == 0xFFFFFFFFu) return;
   const unsigned os = p.cell_start[T.rank0], oe = p.cell_start[T.rank0 + T.ncell_own];
   const unsigned nown = oe - os;
-  // counting sort of the own particles by list length, longest first: hist in the (dead) hbase table, order in map
-  unsigned* const hist = sm.hbase;            // [LCAP + 1] <= HTAB
-  unsigned short* const perm = (unsigned short*)sm.hshift;  // [nown] if nown <= PERM_MAX, else no sorting
-  const bool sorted = nown <= PERM_MAX;  // block-uniform
-  if (sorted) {
-    for (unsigned k = threadIdx.x; k <= LCAP; k += blockDim.x) hist[k] = 0u;
-    __syncthreads();
-    for (unsigned t = threadIdx.x; t < nown; t += blockDim.x) {
-      unsigned na = p.nact[os + t];
-      if (!ALL && (f2u(sm.spos[p.self_loc[os + t]].w) >> 31)) na = 0u;  // frozen: nothing to evaluate
-      atomicAdd(&hist[LCAP - min(na, LCAP)], 1u);                       // bin 0 = longest
-    }
-    __syncthreads();
-    if (threadIdx.x < 32) {  // exclusive scan of the LCAP + 1 bins by warp 0
-      const int lane = threadIdx.x;
-      unsigned run = 0;
-      for (unsigned b0 = 0; b0 <= LCAP; b0 += 32) {
-        const unsigned k = b0 + lane;
-        const unsigned c = k <= LCAP ? hist[k] : 0u;
-        unsigned incl = c;
-  #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-          const unsigned v = __shfl_up_sync(0xffffffffu, incl, o);
-          if (lane >= o) incl += v;
-        }
-        if (k <= LCAP) hist[k] = run + incl - c;
-        run += __shfl_sync(0xffffffffu, incl, 31);
-      }
-    }
-    __syncthreads();
-    for (unsigned t = threadIdx.x; t < nown; t += blockDim.x) {
-      unsigned na = p.nact[os + t];
-      if (!ALL && (f2u(sm.spos[p.self_loc[os + t]].w) >> 31)) na = 0u;
-      perm[atomicAdd(&hist[LCAP - min(na, LCAP)], 1u)] = (unsigned short)t;
-    }
-    __syncthreads();
-  }
-  const HashKeys K = make_keys(p.ctl->step, p.seed);
-  for (unsigned t0 = 0; t0 < nown; t0 += blockDim.x) {  // every warp runs the same number of rounds
-    const unsigned t = t0 + threadIdx.x;
-    const bool valid = t < nown;
-    const unsigned i = os + (valid ? (sorted ? (unsigned)perm[t] : t) : 0u);
+#ifdef MDPD_PHASES
+  const long long ph_t1 = clock64();
+#endif
+  const bool sorted = sort_own_by_length(sm, nown, [&](unsigned t) {
+    unsigned na = p.nact[os + t];
+    if (!ALL && (f2u(sm.spos[p.self_loc[os + t]].w) >> 31)) na = 0u;  // frozen: nothing to evaluate
+    return na;
+  });
+  const unsigned short* const perm = (const unsigned short*)sm.hshift;
+#ifdef MDPD_PHASES
+  const long long ph_t2 = clock64();
+#endif
+  HashKeys K = make_keys(p.ctl->step, p.seed);
+#pragma unroll
+  for (int q = 0; q < 6; ++q) K.k[q] = pin(K.k[q]);
+  const unsigned pbase = smem_addr(sm.spos), vbase = smem_addr(sm.svel);
+  const unsigned sentw = p.tile_cap | (p.tile_cap << 16);
+  const unsigned warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
+  const unsigned ngroups = (nown + 31u) >> 5;
+  for (unsigned r = 0; r * W < ngroups; ++r) {
+    const unsigned g = group_of_round(r, warp, W);
+    const unsigned t = g * 32u + lane;
+    if (g >= ngroups || t >= nown) continue;
+    const unsigned i = os + (sorted ? (unsigned)perm[t] : t);
     const unsigned li = p.self_loc[i];
     const float4 xi = sm.spos[li];
     const unsigned wi = f2u(xi.w);
     const unsigned walli = wi >> 31;
-    const bool work = valid && (ALL || !walli);
+    if (!ALL && walli) continue;  // frozen particles are never integrated (R8): their force is not needed
     const unsigned tagi = wi & 0x7FFFFFFFu;
     const float4 vi = sm.svel[li];
-    const unsigned na = work ? p.nact[i] : 0u;
-    const unsigned namax = __reduce_max_sync(0xffffffffu, na);
+    const unsigned na = p.nact[i];
     ForceAcc acc = {0.f, 0.f, 0.f};
     const uint4* __restrict__ lst = p.act + i;
-    uint4 nxt = na ? lst[0] : make_uint4(0, 0, 0, 0);
-    for (unsigned k0 = 0; k0 < namax; k0 += 8) {
+    uint4 nxt = na ? lst[0] : make_uint4(sentw, sentw, sentw, sentw);
+    for (unsigned k0 = 0; k0 < na; k0 += 8) {
       const uint4 e = nxt;
       if (k0 + 8 < na) nxt = lst[(size_t)((k0 >> 3) + 1) * p.N];  // next chunk in flight
-#pragma unroll
-      for (int q = 0; q < 8; ++q) {
-        if (k0 + q >= namax) break;  // warp-uniform
-        if (k0 + q < na) {
-          const unsigned j = list_entry(e, q);
-          const float4 xj = sm.spos[j];
-          const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
-          const float r2 = dx * dx + dy * dy + dz * dz;
-          pair_force(p, xi, vi, tagi, xj, sm.svel[j], dx, dy, dz, r2, K, acc);
-        }
+      force_entry(p, pbase, vbase, xi, vi, tagi, e.x & 0xFFFFu, K, acc);
+      force_entry(p, pbase, vbase, xi, vi, tagi, e.x >> 16, K, acc);
+      force_entry(p, pbase, vbase, xi, vi, tagi, e.y & 0xFFFFu, K, acc);
+      force_entry(p, pbase, vbase, xi, vi, tagi, e.y >> 16, K, acc);
+      if (k0 + 4 < na) {  // the second half of the chunk holds at least one entry
+        force_entry(p, pbase, vbase, xi, vi, tagi, e.z & 0xFFFFu, K, acc);
+        force_entry(p, pbase, vbase, xi, vi, tagi, e.z >> 16, K, acc);
+        force_entry(p, pbase, vbase, xi, vi, tagi, e.w & 0xFFFFu, K, acc);
+        force_entry(p, pbase, vbase, xi, vi, tagi, e.w >> 16, K, acc);
       }
     }
-    if (work) {
-      if (!walli) {
-        acc.x += p.fgx;
-        acc.y += p.fgy;
-        acc.z += p.fgz;
-      }
-      p.force[i] = make_float4(acc.x, acc.y, acc.z, 0.0f);
+    if (!walli) {
+      acc.x += p.fgx;
+      acc.y += p.fgy;
+      acc.z += p.fgz;
     }
+    p.force[i] = make_float4(acc.x, acc.y, acc.z, 0.0f);
   }
+#ifdef MDPD_PHASES
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    const long long ph_t3 = clock64();
+    atomicAdd(&p.ctl->ph[0], (unsigned long long)(ph_t1 - ph_t0));
+    atomicAdd(&p.ctl->ph[1], (unsigned long long)(ph_t2 - ph_t1));
+    atomicAdd(&p.ctl->ph[2], (unsigned long long)(ph_t3 - ph_t2));
+    atomicAdd(&p.ctl->ph[3], 1ull);
+  }
+#endif
 }
 
 // ----------------------------------------------------------------------------------------------------------------
@@ -1827,6 +1890,7 @@ int mdpd_get_counters(mdpd_ctx* h, uint64_t out[MDPD_NCOUNTERS]) {
   out[9] = c->dens_passes;
   out[10] = (uint64_t)h->tile_dim[0] | ((uint64_t)h->tile_dim[1] << 8) | ((uint64_t)h->tile_dim[2] << 16);
   out[11] = h->d.ntiles;
+  for (int k = 0; k < 4; ++k) out[12 + k] = c->ph[k];  // zero unless built with -DMDPD_PHASES
   return rc;
 }
 
