@@ -73,10 +73,15 @@ struct DevP {  // passed by value to every kernel
   uint4* act;                // [cap / 8][N] this step's in-range (r < rc) subset of the list, written by the density pass
   unsigned short* nact;      // [N] its length
   const TileInfo* tiles;     // [ntiles]
+  uint4* runs;               // [ntiles][run_stride] staging recipe of every tile, written by k_build_list (see stage_fast)
+  uint2* dinfo;              // [N] hand-out records of the density pass: own particles of every tile in order of decreasing
+                             //     list length; x = index in the tile | own staged slot << 16, y = list length
+  uint2* finfo;              // [N] ... of the force pass: in order of decreasing in-range count of this step (y = count,
+                             //     bit 31: frozen particle whose force is not needed), written by the density pass
   const unsigned char* mask;
   Ctl* ctl;
   // sizes
-  unsigned N, ncell, cap, ntiles, tile_cap;
+  unsigned N, ncell, cap, ntiles, tile_cap, run_stride;
   int ncx, ncy, ncz;
   int mx, my, mz;
   // geometry
@@ -101,6 +106,18 @@ __device__ __forceinline__ float rsqrt_fast(float x) {  // one MUFU.RSQ (2 ulp);
   return y;
 }
 __device__ __forceinline__ float u2f(unsigned u) { return __uint_as_float(u); }
+
+// Shared-memory gathers of the hot loops go through 32-bit shared addresses (one LEA per neighbour and array).
+__device__ __forceinline__ unsigned smem_addr(const void* ptr) { return (unsigned)__cvta_generic_to_shared(ptr); }
+__device__ __forceinline__ float4 lds4(unsigned addr) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ unsigned pin(unsigned v) {  // keeps a loop-invariant value in its register (no rematerialisation)
+  asm volatile("" : "+r"(v));
+  return v;
+}
 
 // Positions are kept UNWRAPPED between list rebuilds (they leave [0, L) by at most skin / 2) so that a particle stays
 // geometrically inside the cell it was sorted into; they are wrapped when the sort runs, for the voxel-mask lookup
@@ -471,7 +488,7 @@ __global__ void __launch_bounds__(TPB) k_permute(const DevP p) {
 #define MINB 3
 #endif
 #ifndef TILE_TPB
-#define TILE_TPB 224  // most threads per CTA of the density / force passes (7 warps x 2 rounds on a full tile)
+#define TILE_TPB 256  // most threads per CTA of the density / force passes (8 warps; long and short groups paired: two rounds on a full tile)
 #endif
 constexpr int HMAX = 216;                      // halo cells of the largest tile
 constexpr int HTAB = 224;                      // table size (HMAX + 1 rounded up)
@@ -491,7 +508,6 @@ struct TileSmem {
 };
 
 constexpr size_t TILE_SLOT_BYTES = 32;  // pos + vel: shared-memory bytes per staged slot of the force pass
-constexpr unsigned PERM_MAX = HTAB * 8; // own particles whose order fits the (dead after staging) hshift table
 
 // queue_entries: 16-bit scratch entries behind the tables (list build: rows per warp)
 __host__ __device__ inline size_t tile_smem_bytes(unsigned cap, bool with_vel, size_t queue_entries) {
@@ -599,6 +615,119 @@ __device__ __forceinline__ unsigned stage_tile(const DevP& p, const TileInfo& T,
   return total;
 }
 
+// ----------------------------------------------------------------------------------------------------------------
+// Staging recipe.  The per-step passes (density, force) do not rediscover the tile's geometry: at every list build
+// k_build_list writes, per tile, a header and one record per RUN of halo cells that is contiguous both in the staged
+// image and in the sorted particle arrays (per (y, z) halo row: the cell at x = -1, the tile-aligned cells, the cell
+// at x = ex).  Header: x = staged particles (0xFFFFFFFF: tile does not fit), y = runs, z = items | own particles << 16,
+// w = first own particle.  Record: x = first global index, y = first staged slot | particles << 16, z = shift code
+// cx + 3 cy + 9 cz (per dimension 0 -> -origin, 1 -> -L, 2 -> L - origin), w = index of the run's first item; an ITEM is a
+// piece of at most 32 particles of a run: one coalesced load per warp.
+// stage_fast: records -> item list in shared memory (one global-memory latency), barrier, every warp copies its
+// items in batches of independent loads (one more latency), barrier.  The staged image is bit-identical to stage_tile's.
+// ----------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void cp_async16(unsigned dst_smem, const void* src) {  // LDGSTS: no register staging
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst_smem), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+template <bool WITH_VEL>
+__device__ __forceinline__ bool stage_fast(const DevP& p, const TileInfo& T, const uint4 hdr,
+                                           const float4* __restrict__ pos, const float4* __restrict__ vel,
+                                           const TileSmem& sm) {
+  uint2* const items = (uint2*)sm.hshift;   // [nitems] <= 3 * 36 + tile_cap / 32 <= 2 * HTAB
+  float4* const shtab = (float4*)sm.hbase;  // [27] shift of every code
+  // the records are requested together with the header (whose nruns bounds them): one latency for both
+  const uint4* __restrict__ rec = p.runs + (size_t)blockIdx.x * p.run_stride + 1;
+  const unsigned nrec = p.run_stride - 1u;
+  const unsigned total = hdr.x, nruns = hdr.y, nitems = hdr.z & 0xFFFFu;
+  for (unsigned r = threadIdx.x; r < nrec; r += blockDim.x) {
+    const uint4 R = rec[r];
+    if (r < nruns && total <= p.tile_cap) {
+      const unsigned cnt = R.y >> 16, sb = R.y & 0xFFFFu;
+      unsigned io = R.w;
+      for (unsigned c = 0; c < cnt; c += 32, ++io)
+        items[io] = make_uint2(R.x + c, (sb + c) | ((min(32u, cnt - c) - 1u) << 16) | (R.z << 21));
+    }
+  }
+  if (total > p.tile_cap) return false;  // flagged by k_build_list (block-uniform)
+  if (threadIdx.x < 27) {
+    const unsigned c = threadIdx.x, cx = c % 3u, cy = (c / 3u) % 3u, cz = c / 9u;
+    const float ox = tile_origin(T.c0x, p.edge_x), oy = tile_origin(T.c0y, p.edge_y), oz = tile_origin(T.c0z, p.edge_z);
+    shtab[c] = make_float4(cx == 0u ? -ox : (cx == 1u ? -p.Lx : p.Lx - ox), cy == 0u ? -oy : (cy == 1u ? -p.Ly : p.Ly - oy),
+                           cz == 0u ? -oz : (cz == 1u ? -p.Lz : p.Lz - oz), 0.f);
+  }
+  __syncthreads();
+  const unsigned warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
+  const unsigned pbase = smem_addr(sm.spos), vbase = smem_addr(sm.svel);
+  // asynchronous copies global -> shared of every item of the warp: all in flight at once
+  for (unsigned q = warp; q < nitems; q += W) {
+    const uint2 it = items[q];
+    if (lane <= ((it.y >> 16) & 31u)) {
+      const unsigned dst = ((it.y & 0xFFFFu) + lane) << 4;
+      cp_async16(pbase + dst, pos + it.x + lane);
+      if (WITH_VEL) cp_async16(vbase + dst, vel + it.x + lane);
+    }
+  }
+  cp_async_wait_all();
+  __syncwarp();
+  // to tile-relative coordinates, in place (a warp touches only what it copied itself)
+  for (unsigned q = warp; q < nitems; q += W) {
+    const uint2 it = items[q];
+    if (lane <= ((it.y >> 16) & 31u)) {
+      const float4 sh = shtab[it.y >> 21];
+      float4* const xp = sm.spos + (it.y & 0xFFFFu) + lane;
+      float4 x = *xp;
+      x.x += sh.x;
+      x.y += sh.y;
+      x.z += sh.z;
+      *xp = x;
+    }
+  }
+  if (threadIdx.x == 0) {  // sentinel slot: list padding points here; it is out of range of everything
+    sm.spos[p.tile_cap] = make_float4(1e9f, 1e9f, 1e9f, 0.f);
+    if (WITH_VEL) sm.svel[p.tile_cap] = make_float4(0.f, 0.f, 0.f, 0.f);
+  }
+  __syncthreads();
+  return true;
+}
+
+// Written by warp 0 of k_build_list right after stage_tile (hbase = first staged slot of every halo cell, hshift.w =
+// global index - staged slot of the cell's particles).
+__device__ __forceinline__ void write_tile_runs(const DevP& p, const TileInfo& T, const TileSmem& sm, unsigned total,
+                                                unsigned os, unsigned nown) {
+  const int lane = threadIdx.x & 31;
+  const int hxn = T.ex + 2, hyn = T.ey + 2, hzn = T.ez + 2;
+  const unsigned nruns = 3u * hyn * hzn;
+  uint4* const out = p.runs + (size_t)blockIdx.x * p.run_stride;
+  unsigned run_items = 0;
+  for (unsigned r0 = 0; r0 < nruns; r0 += 32) {
+    const unsigned r = r0 + lane;
+    unsigned cnt = 0, sb = 0, g = 0, code = 0;
+    if (r < nruns) {
+      const int seg = r % 3, hy = (r / 3) % hyn, hz = r / (3 * hyn);
+      const int hx = seg == 0 ? 0 : (seg == 1 ? 1 : hxn - 1), len = seg == 1 ? T.ex : 1;
+      const int h0 = (hz * hyn + hy) * hxn + hx;
+      sb = sm.hbase[h0];
+      cnt = sm.hbase[h0 + len] - sb;
+      g = sb + f2u(sm.hshift[h0].w);
+      const int cx = T.c0x + hx - 1, cy = T.c0y + hy - 1, cz = T.c0z + hz - 1;
+      code = (cx < 0 ? 1u : (cx >= p.ncx ? 2u : 0u)) + 3u * (cy < 0 ? 1u : (cy >= p.ncy ? 2u : 0u)) +
+             9u * (cz < 0 ? 1u : (cz >= p.ncz ? 2u : 0u));
+    }
+    const unsigned nit = (cnt + 31u) >> 5;
+    unsigned incl = nit;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const unsigned t = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += t;
+    }
+    if (r < nruns) out[1 + r] = make_uint4(g, sb | (cnt << 16), code, run_items + incl - nit);
+    run_items += __shfl_sync(0xffffffffu, incl, 31);
+  }
+  if (lane == 0) out[0] = make_uint4(total, nruns, run_items | (nown << 16), os);
+}
+
 // per-tile statistics after the first sort (load time): largest halo population (shared-memory capacity) and largest
 // tile.  One warp per tile, lanes over the halo cells.  During stepping k_build_list keeps the same two maxima.
 __global__ void __launch_bounds__(128) k_tile_stats(const DevP p) {
@@ -621,6 +750,46 @@ __global__ void __launch_bounds__(128) k_tile_stats(const DevP p) {
     atomicMax(&p.ctl->max_halo, halo);
     atomicMax(&p.ctl->max_own, p.cell_start[T.rank0 + T.ncell_own] - p.cell_start[T.rank0]);
   }
+}
+
+// Own particles are handed to the warps in order of decreasing list length (a counting sort on the length in shared
+// memory, the order written to `out`): group g = sorted particles 32 g .. 32 g + 31, so the lanes of a warp finish
+// together; warp w then takes the groups w, 2W-1-w, 2W+w, 4W-1-w, ... (a long group is followed by a short one), so
+// the warps of the CTA finish together too.  Which thread evaluates which particle does not change any result.
+// The order for the density pass (key: list length) is made once per list build, the order for the force pass (key:
+// in-range count of the step) by the density pass that precedes it.  hist = the hbase table (dead by then).
+// All threads of the CTA must call it.
+template <class LenFn, class RecFn>
+__device__ __forceinline__ void sort_own_by_length(const TileSmem& sm, unsigned nown, uint2* out, LenFn len, RecFn rec) {
+  unsigned* const hist = sm.hbase;  // [LCAP + 1] <= HTAB
+  __syncthreads();
+  for (unsigned k = threadIdx.x; k <= LCAP; k += blockDim.x) hist[k] = 0u;
+  __syncthreads();
+  for (unsigned t = threadIdx.x; t < nown; t += blockDim.x) atomicAdd(&hist[LCAP - min(len(t), LCAP)], 1u);  // bin 0 = longest
+  __syncthreads();
+  if (threadIdx.x < 32) {  // exclusive scan of the LCAP + 1 bins by warp 0
+    const int lane = threadIdx.x;
+    unsigned run = 0;
+    for (unsigned b0 = 0; b0 <= LCAP; b0 += 32) {
+      const unsigned k = b0 + lane;
+      const unsigned c = k <= LCAP ? hist[k] : 0u;
+      unsigned incl = c;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const unsigned v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
+      }
+      if (k <= LCAP) hist[k] = run + incl - c;
+      run += __shfl_sync(0xffffffffu, incl, 31);
+    }
+  }
+  __syncthreads();
+  for (unsigned t = threadIdx.x; t < nown; t += blockDim.x) out[atomicAdd(&hist[LCAP - min(len(t), LCAP)], 1u)] = rec(t);
+}
+
+// group of 32 sorted own particles that warp `warp` of W takes in its round r (see above)
+__device__ __forceinline__ unsigned group_of_round(unsigned r, unsigned warp, unsigned W) {
+  return (r & 1u) ? (r + 1u) * W - 1u - warp : r * W + warp;
 }
 
 // ----------------------------------------------------------------------------------------------------------------
@@ -649,18 +818,20 @@ __global__ void __launch_bounds__(256) k_build_list(const DevP p) {
     atomicMax(&p.ctl->max_halo, total == 0xFFFFFFFFu ? sm.hbase[(T.ex + 2) * (T.ey + 2) * (T.ez + 2)] : total);
     atomicMax(&p.ctl->max_own, p.cell_start[T.rank0 + T.ncell_own] - p.cell_start[T.rank0]);
   }
-  if (total == 0xFFFFFFFFu) {  // does not fit: flag it, leave empty lists
-    const unsigned os = p.cell_start[T.rank0], oe = p.cell_start[T.rank0 + T.ncell_own];
-    for (unsigned i = os + threadIdx.x; i < oe; i += blockDim.x) {
+  const unsigned own_s = p.cell_start[T.rank0], own_n = p.cell_start[T.rank0 + T.ncell_own] - own_s;
+  if (total == 0xFFFFFFFFu) {  // does not fit: flag it, leave empty lists; the per-step passes skip the tile
+    for (unsigned i = own_s + threadIdx.x; i < own_s + own_n; i += blockDim.x) {
       p.nnbr[i] = 0u;
       p.self_loc[i] = 0;
     }
     if (threadIdx.x == 0) {
+      p.runs[(size_t)blockIdx.x * p.run_stride] = make_uint4(0xFFFFFFFFu, 0u, own_n << 16, own_s);
       atomicOr(&p.ctl->err, ERR_TILE);
       atomicAdd(&p.ctl->overflow, 1ull);
     }
     return;
   }
+  if (warp == 0) write_tile_runs(p, T, sm, total, own_s, own_n);  // staging recipe of the per-step passes
   const int hxn = T.ex + 2, hyn = T.ey + 2;
   // per-warp scratch behind the tables: hit masks [32 particle slots][MSTRIDE] and two candidate tables [MAXCAND]
   unsigned* const masks = (unsigned*)(sm.queue + (size_t)warp * BUILD_SCRATCH16);
@@ -813,6 +984,9 @@ __global__ void __launch_bounds__(256) k_build_list(const DevP p) {
       }
     }
   }
+  // hand-out order of the density pass: own particles by decreasing list length (uses the now dead hbase table)
+  sort_own_by_length(sm, own_n, p.dinfo + own_s, [&](unsigned t) { return p.nnbr[own_s + t]; },
+                     [&](unsigned t) { return make_uint2(t | ((unsigned)p.self_loc[own_s + t] << 16), p.nnbr[own_s + t]); });
   // statistics + overflow flag
   smax = __reduce_max_sync(0xffffffffu, smax);
   ssum = __reduce_add_sync(0xffffffffu, ssum);
@@ -834,60 +1008,6 @@ __global__ void k_reset_list_stats(const DevP p) {
   p.ctl->sum_nbr = 0;
   p.ctl->max_halo = 0;
   p.ctl->max_own = 0;
-}
-
-// Shared-memory gathers of the hot loops go through 32-bit shared addresses (one LEA per neighbour and array).
-__device__ __forceinline__ unsigned smem_addr(const void* ptr) { return (unsigned)__cvta_generic_to_shared(ptr); }
-__device__ __forceinline__ float4 lds4(unsigned addr) {
-  float4 v;
-  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
-  return v;
-}
-__device__ __forceinline__ unsigned pin(unsigned v) {  // keeps a loop-invariant value in its register (no rematerialisation)
-  asm volatile("" : "+r"(v));
-  return v;
-}
-
-// Own particles are handed to the warps in order of decreasing list length (a counting sort on the length, in shared
-// memory): group g = sorted particles 32 g .. 32 g + 31, so the lanes of a warp finish together; warp w then takes the
-// groups w, 2W-1-w, 2W+w, 4W-1-w, ... (a long group is followed by a short one), so the warps of the CTA finish
-// together too.  Which thread evaluates which particle does not change any result.
-// hist = the (dead after staging) hbase table, perm = the (dead) hshift table.  Returns false (no sorting) if the
-// tile holds more own particles than perm has room for.  All threads of the CTA must call it.
-template <class LenFn>
-__device__ __forceinline__ bool sort_own_by_length(const TileSmem& sm, unsigned nown, LenFn len) {
-  unsigned* const hist = sm.hbase;                          // [LCAP + 1] <= HTAB
-  unsigned short* const perm = (unsigned short*)sm.hshift;  // [nown] if nown <= PERM_MAX
-  if (nown > PERM_MAX) return false;                        // block-uniform
-  for (unsigned k = threadIdx.x; k <= LCAP; k += blockDim.x) hist[k] = 0u;
-  __syncthreads();
-  for (unsigned t = threadIdx.x; t < nown; t += blockDim.x) atomicAdd(&hist[LCAP - min(len(t), LCAP)], 1u);  // bin 0 = longest
-  __syncthreads();
-  if (threadIdx.x < 32) {  // exclusive scan of the LCAP + 1 bins by warp 0
-    const int lane = threadIdx.x;
-    unsigned run = 0;
-    for (unsigned b0 = 0; b0 <= LCAP; b0 += 32) {
-      const unsigned k = b0 + lane;
-      const unsigned c = k <= LCAP ? hist[k] : 0u;
-      unsigned incl = c;
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        const unsigned v = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= o) incl += v;
-      }
-      if (k <= LCAP) hist[k] = run + incl - c;
-      run += __shfl_sync(0xffffffffu, incl, 31);
-    }
-  }
-  __syncthreads();
-  for (unsigned t = threadIdx.x; t < nown; t += blockDim.x) perm[atomicAdd(&hist[LCAP - min(len(t), LCAP)], 1u)] = (unsigned short)t;
-  __syncthreads();
-  return true;
-}
-
-// group of 32 sorted own particles that warp `warp` of W takes in its round r (see above)
-__device__ __forceinline__ unsigned group_of_round(unsigned r, unsigned warp, unsigned W) {
-  return (r & 1u) ? (r + 1u) * W - 1u - warp : r * W + warp;
 }
 
 // ----------------------------------------------------------------------------------------------------------------
@@ -922,36 +1042,60 @@ __device__ __forceinline__ void density_entry(const DevP& p, const unsigned pbas
   }
 }
 
-template <bool HAS_WALL>
+constexpr int PRE = 2;  // rounds whose hand-out record and first list chunk are requested before the tile is staged
+
+template <bool HAS_WALL, bool ALL>
 __global__ void __launch_bounds__(TILE_TPB, MINB) k_density(const DevP p) {
   extern __shared__ __align__(16) unsigned char smraw[];
   const TileSmem sm = carve_smem(smraw, p.tile_cap, false);
   const unsigned cur = p.ctl->cur;
   const TileInfo T = p.tiles[blockIdx.x];
-  if (stage_tile<false>(p, T, p.pos[cur], nullptr, sm) == 0xFFFFFFFFu) return;  // flagged by k_build_list
-  const unsigned os = p.cell_start[T.rank0], oe = p.cell_start[T.rank0 + T.ncell_own];
-  const unsigned nown = oe - os;
-  const bool sorted = sort_own_by_length(sm, nown, [&](unsigned t) { return p.nnbr[os + t]; });
-  const unsigned short* const perm = (const unsigned short*)sm.hshift;
+  const uint4 hdr = p.runs[(size_t)blockIdx.x * p.run_stride];
+  const unsigned os = hdr.w, nown = hdr.z >> 16;
+  const unsigned warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
+  const unsigned ngroups = (nown + 31u) >> 5;
+  // the first rounds' records and list heads are in flight while the tile is staged
+  uint2 info[PRE];
+  uint4 head[PRE];
+#pragma unroll
+  for (int r = 0; r < PRE; ++r) {
+    const unsigned g = group_of_round(r, warp, W), t = g * 32u + lane;
+    info[r] = (g < ngroups && t < nown) ? p.dinfo[os + t] : make_uint2(0u, 0u);
+  }
+#pragma unroll
+  for (int r = 0; r < PRE; ++r) head[r] = info[r].y ? p.nbr[os + (info[r].x & 0xFFFFu)] : make_uint4(0, 0, 0, 0);
+  if (!stage_fast<false>(p, T, hdr, p.pos[cur], nullptr, sm)) return;  // flagged by k_build_list
   float4* __restrict__ vel = p.vel[cur];
   const unsigned sent = p.tile_cap;
   const unsigned pbase = smem_addr(sm.spos);
-  const unsigned warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
-  const unsigned ngroups = (nown + 31u) >> 5;
+  unsigned* const hist = sm.hbase;  // [LCAP + 1] bins of the sort below (bin 0 = longest) + the in-range pair count; the
+                                    // shift table that lived here is dead after staging
+  for (unsigned k = threadIdx.x; k < HTAB; k += blockDim.x) hist[k] = 0u;
   unsigned na_sum = 0;
+  uint2 frec[PRE];  // this thread's records for the force pass: x as in dinfo, y = in-range count (bit 31: frozen, skip)
+#pragma unroll
+  for (int r = 0; r < PRE; ++r) frec[r] = make_uint2(0u, 0u);
   for (unsigned r = 0; r * W < ngroups; ++r) {
     const unsigned g = group_of_round(r, warp, W);
     const unsigned t = g * 32u + lane;
     if (g >= ngroups || t >= nown) continue;
-    const unsigned i = os + (sorted ? (unsigned)perm[t] : t);
-    const float4 xi = sm.spos[p.self_loc[i]];
+    uint2 rec;
+    uint4 nxt;
+    if (r < PRE) {
+      rec = r == 0 ? info[0] : info[PRE - 1];
+      nxt = r == 0 ? head[0] : head[PRE - 1];
+    } else {
+      rec = p.dinfo[os + t];
+      nxt = rec.y ? p.nbr[os + (rec.x & 0xFFFFu)] : make_uint4(0, 0, 0, 0);
+    }
+    const unsigned i = os + (rec.x & 0xFFFFu);
+    const float4 xi = sm.spos[rec.x >> 16];
     const unsigned walli = f2u(xi.w) >> 31;
-    const unsigned nn = p.nnbr[i];
+    const unsigned nn = rec.y;
     const uint4* __restrict__ lst = p.nbr + i;
     uint4* ao = p.act + i;  // next chunk to write
     float rho = 0.0f;
     unsigned a0 = 0, a1 = 0, a2 = 0, a3 = 0, na = 0;
-    uint4 nxt = nn ? lst[0] : make_uint4(0, 0, 0, 0);
     for (unsigned k0 = 0; k0 < nn; k0 += 8) {
       const uint4 e = nxt;
       if (k0 + 8 < nn) nxt = lst[(size_t)((k0 >> 3) + 1) * p.N];  // next chunk in flight while this one is evaluated
@@ -976,18 +1120,57 @@ __global__ void __launch_bounds__(TILE_TPB, MINB) k_density(const DevP p) {
     p.nact[i] = (unsigned short)na;
     na_sum += na;
     vel[i].w = rho * p.Krho;
+    const unsigned fy = (HAS_WALL && !ALL && walli) ? 0x80000000u : na;  // frozen: force not needed (R8)
+    if (r == 0) frec[0] = make_uint2(rec.x, fy);
+    else if (r < PRE) frec[PRE - 1] = make_uint2(rec.x, fy);
   }
-  // statistics: in-range pairs evaluated per step (the force pass's algorithmic work)
-  __syncthreads();  // the staged image is dead: reuse its first word
-  unsigned* acc = (unsigned*)smraw;
-  if (threadIdx.x == 0) *acc = 0u;
-  __syncthreads();
+  // Hand-out records of the force pass that follows: own particles by decreasing in-range count of this step (counting
+  // sort; the keys of the first PRE rounds are still in registers).  The in-range pair count of the tile (the force
+  // pass's algorithmic work, a statistic) rides on the same barriers.
+  auto round_record = [&](unsigned r, uint2& out) {
+    const unsigned g = group_of_round(r, warp, W), t = g * 32u + lane;
+    if (g >= ngroups || t >= nown) return false;
+    if (r == 0) out = frec[0];
+    else if (r < PRE) out = frec[PRE - 1];
+    else {
+      const uint2 d = p.dinfo[os + t];
+      const bool skip = HAS_WALL && !ALL && (f2u(sm.spos[d.x >> 16].w) >> 31);
+      out = make_uint2(d.x, skip ? 0x80000000u : (unsigned)p.nact[os + (d.x & 0xFFFFu)]);
+    }
+    return true;
+  };
   na_sum = __reduce_add_sync(0xffffffffu, na_sum);
-  if ((threadIdx.x & 31) == 0 && na_sum) atomicAdd(acc, na_sum);
+  __syncthreads();  // hist is zero, every particle of the tile is done
+  if (lane == 0 && na_sum) atomicAdd(&hist[HTAB - 1], na_sum);
+  for (unsigned r = 0; r * W < ngroups; ++r) {
+    uint2 fr;
+    if (round_record(r, fr)) atomicAdd(&hist[LCAP - min(fr.y & 0x7FFFFFFFu, LCAP)], 1u);
+  }
   __syncthreads();
-  if (threadIdx.x == 0) {
-    atomicAdd(&p.ctl->sum_act, (unsigned long long)*acc);
-    if (blockIdx.x == 0) atomicAdd(&p.ctl->dens_passes, 1ull);
+  if (threadIdx.x < 32) {  // exclusive scan of the LCAP + 1 bins by warp 0
+    unsigned run = 0;
+    for (unsigned b0 = 0; b0 <= LCAP; b0 += 32) {
+      const unsigned k = b0 + lane;
+      const unsigned c = k <= LCAP ? hist[k] : 0u;
+      unsigned incl = c;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const unsigned v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
+      }
+      if (k <= LCAP) hist[k] = run + incl - c;
+      run += __shfl_sync(0xffffffffu, incl, 31);
+    }
+    if (lane == 0) {
+      atomicAdd(&p.ctl->sum_act, (unsigned long long)hist[HTAB - 1]);
+      if (blockIdx.x == 0) atomicAdd(&p.ctl->dens_passes, 1ull);
+    }
+  }
+  __syncthreads();
+  uint2* __restrict__ fout = p.finfo + os;
+  for (unsigned r = 0; r * W < ngroups; ++r) {
+    uint2 fr;
+    if (round_record(r, fr)) fout[atomicAdd(&hist[LCAP - min(fr.y & 0x7FFFFFFFu, LCAP)], 1u)] = fr;
   }
 }
 
@@ -1035,44 +1218,54 @@ __global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
 #ifdef MDPD_PHASES
   const long long ph_t0 = clock64();
 #endif
-  if (stage_tile<true>(p, T, p.pos[cur], p.vel[cur], sm) == 0xFFFFFFFFu) return;
-  const unsigned os = p.cell_start[T.rank0], oe = p.cell_start[T.rank0 + T.ncell_own];
-  const unsigned nown = oe - os;
+  const uint4 hdr = p.runs[(size_t)blockIdx.x * p.run_stride];
+  const unsigned os = hdr.w, nown = hdr.z >> 16;
+  const unsigned warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
+  const unsigned ngroups = (nown + 31u) >> 5;
+  const unsigned sentw = p.tile_cap | (p.tile_cap << 16);
+  // the first rounds' records (written by the density pass of this step) and list heads are in flight while the
+  // tile is staged
+  uint2 info[PRE];
+  uint4 head[PRE];
+#pragma unroll
+  for (int r = 0; r < PRE; ++r) {
+    const unsigned g = group_of_round(r, warp, W), t = g * 32u + lane;
+    info[r] = (g < ngroups && t < nown) ? p.finfo[os + t] : make_uint2(0u, 0x80000000u);
+  }
+#pragma unroll
+  for (int r = 0; r < PRE; ++r)
+    head[r] = (info[r].y & 0x7FFFFFFFu) ? p.act[os + (info[r].x & 0xFFFFu)] : make_uint4(sentw, sentw, sentw, sentw);
+  if (!stage_fast<true>(p, T, hdr, p.pos[cur], p.vel[cur], sm)) return;
 #ifdef MDPD_PHASES
   const long long ph_t1 = clock64();
-#endif
-  const bool sorted = sort_own_by_length(sm, nown, [&](unsigned t) {
-    unsigned na = p.nact[os + t];
-    if (!ALL && (f2u(sm.spos[p.self_loc[os + t]].w) >> 31)) na = 0u;  // frozen: nothing to evaluate
-    return na;
-  });
-  const unsigned short* const perm = (const unsigned short*)sm.hshift;
-#ifdef MDPD_PHASES
-  const long long ph_t2 = clock64();
 #endif
   HashKeys K = make_keys(p.ctl->step, p.seed);
 #pragma unroll
   for (int q = 0; q < 6; ++q) K.k[q] = pin(K.k[q]);
   const unsigned pbase = smem_addr(sm.spos), vbase = smem_addr(sm.svel);
-  const unsigned sentw = p.tile_cap | (p.tile_cap << 16);
-  const unsigned warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
-  const unsigned ngroups = (nown + 31u) >> 5;
   for (unsigned r = 0; r * W < ngroups; ++r) {
     const unsigned g = group_of_round(r, warp, W);
     const unsigned t = g * 32u + lane;
     if (g >= ngroups || t >= nown) continue;
-    const unsigned i = os + (sorted ? (unsigned)perm[t] : t);
-    const unsigned li = p.self_loc[i];
+    uint2 rec;
+    uint4 nxt;
+    if (r < PRE) {
+      rec = r == 0 ? info[0] : info[PRE - 1];
+      nxt = r == 0 ? head[0] : head[PRE - 1];
+    } else {
+      rec = p.finfo[os + t];
+      nxt = (rec.y & 0x7FFFFFFFu) ? p.act[os + (rec.x & 0xFFFFu)] : make_uint4(sentw, sentw, sentw, sentw);
+    }
+    if (rec.y >> 31) continue;  // frozen particles are never integrated (R8): their force is not needed
+    const unsigned i = os + (rec.x & 0xFFFFu);
+    const unsigned li = rec.x >> 16;
     const float4 xi = sm.spos[li];
     const unsigned wi = f2u(xi.w);
-    const unsigned walli = wi >> 31;
-    if (!ALL && walli) continue;  // frozen particles are never integrated (R8): their force is not needed
     const unsigned tagi = wi & 0x7FFFFFFFu;
     const float4 vi = sm.svel[li];
-    const unsigned na = p.nact[i];
+    const unsigned na = rec.y;
     ForceAcc acc = {0.f, 0.f, 0.f};
     const uint4* __restrict__ lst = p.act + i;
-    uint4 nxt = na ? lst[0] : make_uint4(sentw, sentw, sentw, sentw);
     for (unsigned k0 = 0; k0 < na; k0 += 8) {
       const uint4 e = nxt;
       if (k0 + 8 < na) nxt = lst[(size_t)((k0 >> 3) + 1) * p.N];  // next chunk in flight
@@ -1087,7 +1280,7 @@ __global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
         force_entry(p, pbase, vbase, xi, vi, tagi, e.w >> 16, K, acc);
       }
     }
-    if (!walli) {
+    if (!(wi >> 31)) {
       acc.x += p.fgx;
       acc.y += p.fgy;
       acc.z += p.fgz;
@@ -1099,8 +1292,7 @@ __global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
   if (threadIdx.x == 0) {
     const long long ph_t3 = clock64();
     atomicAdd(&p.ctl->ph[0], (unsigned long long)(ph_t1 - ph_t0));
-    atomicAdd(&p.ctl->ph[1], (unsigned long long)(ph_t2 - ph_t1));
-    atomicAdd(&p.ctl->ph[2], (unsigned long long)(ph_t3 - ph_t2));
+    atomicAdd(&p.ctl->ph[2], (unsigned long long)(ph_t3 - ph_t1));
     atomicAdd(&p.ctl->ph[3], 1ull);
   }
 #endif
@@ -1155,7 +1347,7 @@ inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {
   size_t pos[2], vel[2], force, xbuild, cell_rank, cell_count, cell_start, scan_bsum, pcell, order, nbr,
-      act, nact, nnbr, self_loc, tiles, mask, ctl, stage, total;
+      act, nact, nnbr, self_loc, tiles, runs, dperm, fperm, mask, ctl, stage, total;
   unsigned ncx, ncy, ncz, ncell, cap, scan_blocks;
   float rlist;
 };
@@ -1214,6 +1406,9 @@ bool make_layout(const mdpd_params& p, uint64_t n, int has_mask, const uint32_t*
   L.nnbr = take(N * 4);
   L.self_loc = take(N * 2);
   L.tiles = take((size_t)L.ncell * sizeof(TileInfo));  // worst case: one cell per tile
+  L.runs = take(((size_t)L.ncell * 28 + 4096) * 16);   // worst case: one cell per tile, 1 + 27 records each
+  L.dperm = take(N * 8);
+  L.fperm = take(N * 8);
   L.stage = take(N * 40 + 64);  // load/unload staging: pos, vel, force [n][3] + rho [n] (+ type at load)
   size_t mbytes = 0;
   if (has_mask) {
@@ -1343,6 +1538,9 @@ void fill_devp(mdpd_ctx* h) {
   d.nnbr = (unsigned*)(w + L.nnbr);
   d.self_loc = (unsigned short*)(w + L.self_loc);
   d.tiles = (const TileInfo*)(w + L.tiles);
+  d.runs = (uint4*)(w + L.runs);
+  d.dinfo = (uint2*)(w + L.dperm);
+  d.finfo = (uint2*)(w + L.fperm);
   d.mask = (const unsigned char*)(w + L.mask);
   d.ctl = (Ctl*)(w + L.ctl);
   d.N = (unsigned)h->n;
@@ -1431,8 +1629,9 @@ int launch_rebuild_chain(mdpd_ctx* h, bool with_list = true) {
 
 int launch_forces(mdpd_ctx* h, bool all) {
   const DevP& d = h->d;
-  if (h->has_wall) LAUNCH(h, PS_DENSITY, (k_density<true><<<d.ntiles, h->block, h->smem_pos, h->ls>>>(d)));
-  else LAUNCH(h, PS_DENSITY, (k_density<false><<<d.ntiles, h->block, h->smem_pos, h->ls>>>(d)));
+  if (!h->has_wall) LAUNCH(h, PS_DENSITY, (k_density<false, false><<<d.ntiles, h->block, h->smem_pos, h->ls>>>(d)));
+  else if (all) LAUNCH(h, PS_DENSITY, (k_density<true, true><<<d.ntiles, h->block, h->smem_pos, h->ls>>>(d)));
+  else LAUNCH(h, PS_DENSITY, (k_density<true, false><<<d.ntiles, h->block, h->smem_pos, h->ls>>>(d)));
   if (all) LAUNCH(h, PS_FORCE, (k_force<true><<<d.ntiles, h->block, h->smem_posvel, h->ls>>>(d)));
   else LAUNCH(h, PS_FORCE, (k_force<false><<<d.ntiles, h->block, h->smem_posvel, h->ls>>>(d)));
   return MDPD_OK;
@@ -1691,6 +1890,9 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
     build_tile_ranks(L, tdim, rank, tiles);
     memcpy(h->tile_dim, tdim, sizeof tdim);
     h->d.ntiles = (unsigned)tiles.size();
+    h->d.run_stride = 1u + 3u * (unsigned)((tdim[1] + 2) * (tdim[2] + 2));
+    if ((size_t)h->d.ntiles * h->d.run_stride > (size_t)L.ncell * 28 + 4096)
+      return set_err(h, MDPD_ENOMEM, "tile run table does not fit its reservation");
     const int vol = tdim[0] * tdim[1] * tdim[2];
     h->block = TILE_TPB;  // upper bound while the capacity is probed; set from the tile population below
     h->block_build = vol >= 32 ? 256u : 128u;
@@ -1741,8 +1943,9 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
   h->smem_build = tile_smem_bytes(h->d.tile_cap, false, (size_t)BUILD_SCRATCH16 * (h->block_build / 32));
   if (h->smem_build > h->smem_limit) return set_err(h, MDPD_ENOMEM, "list build needs %zu bytes of shared memory", h->smem_build);
   CU_TRY(h, cudaFuncSetAttribute(k_build_list, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_build));
-  CU_TRY(h, cudaFuncSetAttribute(k_density<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
-  CU_TRY(h, cudaFuncSetAttribute(k_density<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
+  CU_TRY(h, cudaFuncSetAttribute(k_density<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
+  CU_TRY(h, cudaFuncSetAttribute(k_density<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
+  CU_TRY(h, cudaFuncSetAttribute(k_density<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
   CU_TRY(h, cudaFuncSetAttribute(k_pairs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
   CU_TRY(h, cudaFuncSetAttribute(k_force<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
   CU_TRY(h, cudaFuncSetAttribute(k_force<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
