@@ -485,10 +485,16 @@ __global__ void __launch_bounds__(TPB) k_permute(const DevP p) {
 // indices into this staged array, so every neighbour access of the hot loops is a shared-memory load.
 // ----------------------------------------------------------------------------------------------------------------
 #ifndef MINB
-#define MINB 3
+#define MINB 2   // resident CTAs per SM the force pass is compiled for
+#endif
+#ifndef DENS_TPB
+#define DENS_TPB 384  // most threads per CTA of the density pass
+#endif
+#ifndef DENS_MINB
+#define DENS_MINB 3
 #endif
 #ifndef TILE_TPB
-#define TILE_TPB 256  // most threads per CTA of the density / force passes (8 warps; long and short groups paired: two rounds on a full tile)
+#define TILE_TPB 512  // most threads per CTA of the density / force passes (8 warps; long and short groups paired: two rounds on a full tile)
 #endif
 constexpr int HMAX = 216;                      // halo cells of the largest tile
 constexpr int HTAB = 224;                      // table size (HMAX + 1 rounded up)
@@ -784,7 +790,11 @@ __device__ __forceinline__ void sort_own_by_length(const TileSmem& sm, unsigned 
     }
   }
   __syncthreads();
+#ifdef MDPD_DENS_NATURAL
+  for (unsigned t = threadIdx.x; t < nown; t += blockDim.x) out[t] = rec(t);
+#else
   for (unsigned t = threadIdx.x; t < nown; t += blockDim.x) out[atomicAdd(&hist[LCAP - min(len(t), LCAP)], 1u)] = rec(t);
+#endif
 }
 
 // group of 32 sorted own particles that warp `warp` of W takes in its round r (see above)
@@ -806,7 +816,10 @@ __device__ __forceinline__ unsigned group_of_round(unsigned r, unsigned warp, un
 // candidate table and pushes it through a 128-bit shift register; every 8 entries one 16-byte chunk is stored
 // straight to the list, layout [chunk][i], the last chunk padded with the sentinel slot.
 // ----------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_build_list(const DevP p) {
+#ifndef BUILD_TPB
+#define BUILD_TPB 384  // most threads per CTA of the list build
+#endif
+__global__ void __launch_bounds__(BUILD_TPB) k_build_list(const DevP p) {
   if (!p.ctl->rebuild) return;
   extern __shared__ __align__(16) unsigned char smraw[];
   const TileSmem sm = carve_smem(smraw, p.tile_cap, false);
@@ -1022,14 +1035,28 @@ template <bool HAS_WALL>
 __device__ __forceinline__ void density_entry(const DevP& p, const unsigned pbase, const float4 xi, const unsigned walli,
                                               const unsigned j, float& rho, unsigned& a0, unsigned& a1, unsigned& a2,
                                               unsigned& a3, unsigned& na, uint4*& ao) {
+#ifdef MDPD_ABL_NOGATHER
+  const float4 xj = make_float4(u2f(j), u2f(j << 3), u2f(j << 7), 0.f);
+#elif defined(MDPD_FAKE_NOCONFLICT)  // timing experiment only (wrong results): every quarter-warp hits 8 distinct bank groups
+  const float4 xj = lds4(pbase + ((((j & ~7u) | (threadIdx.x & 7u)) << 4)));
+#else
   const float4 xj = lds4(pbase + (j << 4));  // padding entries hit the far-away sentinel
+#endif
   const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
   const float r2 = dx * dx + dy * dy + dz * dz;
-  const float rr = fmaxf(r2, 1e-30f);
-  const float w = fmaxf(0.0f, 1.0f - (rr * rsqrt_fast(rr)) * p.inv_rd);  // branch-free: 0 beyond rd
-  rho += w * w;
-  bool in = r2 < p.rc2 && r2 > 1e-12f;  // interacts at this step (R10)
+  // The logic pipe (min/max, compares, shifts, selects) issues at half the rate of the FP32 pipe and bounds this loop:
+  // the clamps are saturate modifiers of the FMAs, the two-sided range test is one add and one unsigned compare.
+  const float rr = r2 + 1e-30f;  // r = 0 (coincident particles, R10) must not produce 0 * inf
+  const float w = __saturatef(fmaf(-(rr * rsqrt_fast(rr)), p.inv_rd, 1.0f));  // 0 beyond rd; never above 1
+  rho = fmaf(w, w, rho);
+  // 1e-12 < r2 < rc2 (R10): r2 - 1e-12 is negative below the lower bound (huge as an unsigned), and equals r2 wherever
+  // the upper bound could matter (1e-12 is far below half an ulp of rc2)
+  bool in = f2u(r2 - 1e-12f) < f2u(p.rc2 - 1e-12f);  // interacts at this step
   if (HAS_WALL) in = in && !(walli & (f2u(xj.w) >> 31));  // frozen-frozen pairs do not (R8)
+#ifdef MDPD_ABL_NOPUSH
+  na += in ? 1u : 0u;
+  return;
+#endif
   const unsigned sh = in ? 16u : 0u;
   a0 = __funnelshift_r(a0, a1, sh);
   a1 = __funnelshift_r(a1, a2, sh);
@@ -1045,7 +1072,7 @@ __device__ __forceinline__ void density_entry(const DevP& p, const unsigned pbas
 constexpr int PRE = 2;  // rounds whose hand-out record and first list chunk are requested before the tile is staged
 
 template <bool HAS_WALL, bool ALL>
-__global__ void __launch_bounds__(TILE_TPB, MINB) k_density(const DevP p) {
+__global__ void __launch_bounds__(DENS_TPB, DENS_MINB) k_density(const DevP p) {
   extern __shared__ __align__(16) unsigned char smraw[];
   const TileSmem sm = carve_smem(smraw, p.tile_cap, false);
   const unsigned cur = p.ctl->cur;
@@ -1065,6 +1092,9 @@ __global__ void __launch_bounds__(TILE_TPB, MINB) k_density(const DevP p) {
 #pragma unroll
   for (int r = 0; r < PRE; ++r) head[r] = info[r].y ? p.nbr[os + (info[r].x & 0xFFFFu)] : make_uint4(0, 0, 0, 0);
   if (!stage_fast<false>(p, T, hdr, p.pos[cur], nullptr, sm)) return;  // flagged by k_build_list
+#ifdef MDPD_ABL_STAGEONLY
+  if (p.N) return;
+#endif
   float4* __restrict__ vel = p.vel[cur];
   const unsigned sent = p.tile_cap;
   const unsigned pbase = smem_addr(sm.spos);
@@ -1139,6 +1169,9 @@ __global__ void __launch_bounds__(TILE_TPB, MINB) k_density(const DevP p) {
     }
     return true;
   };
+#ifdef MDPD_ABL_NOTAIL
+  if (p.N) return;
+#endif
   na_sum = __reduce_add_sync(0xffffffffu, na_sum);
   __syncthreads();  // hist is zero, every particle of the tile is done
   if (lane == 0 && na_sum) atomicAdd(&hist[HTAB - 1], na_sum);
@@ -1188,15 +1221,21 @@ struct ForceAcc {
 __device__ __forceinline__ void force_entry(const DevP& p, const unsigned pbase, const unsigned vbase, const float4 xi,
                                             const float4 vi, const unsigned tagi, const unsigned j, const HashKeys& K,
                                             ForceAcc& acc) {
+#ifdef MDPD_FAKE_NOCONFLICT
+  const unsigned jj = (j & ~7u) | (threadIdx.x & 7u);
+  const float4 xj = lds4(pbase + (jj << 4));
+  const float4 vj = lds4(vbase + (jj << 4));
+#else
   const float4 xj = lds4(pbase + (j << 4));
   const float4 vj = lds4(vbase + (j << 4));
+#endif
   const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
   const float r2 = dx * dx + dy * dy + dz * dz;  // > 1e-12 for list entries; 3e18 for the sentinel
   const float rinv = rsqrt_fast(r2);
   const float r = r2 * rinv;
-  const float w = fmaxf(0.0f, 1.0f - r * p.inv_rc);  // > 0 for in-range entries, 0 for the sentinel
+  const float w = __saturatef(fmaf(-r, p.inv_rc, 1.0f));  // > 0 for in-range entries, 0 for the sentinel
   float F = p.A * w;
-  const float wd = fmaxf(0.0f, 1.0f - r * p.inv_rd);
+  const float wd = __saturatef(fmaf(-r, p.inv_rd, 1.0f));
   F += p.B * (vi.w + vj.w) * wd;
   const float ev = (dx * (vi.x - vj.x) + dy * (vi.y - vj.y) + dz * (vi.z - vj.z)) * rinv;
   F -= p.gamma * w * w * ev;
@@ -1449,7 +1488,8 @@ struct mdpd_ctx {
   bool pending_B = false;        // the second half kick of the last step has not been applied yet
   uint64_t graph_steps = 0;
   int tile_dim[3] = {4, 4, 4};
-  unsigned block = 256;          // threads per CTA of the density / force passes
+  unsigned block = 256;          // threads per CTA of the force pass
+  unsigned block_dens = 256;     // threads per CTA of the density pass
   unsigned block_build = 256;    // threads per CTA of the list build
   size_t smem_pos = 0, smem_posvel = 0, smem_build = 0;
   size_t smem_limit = 0;         // cudaDevAttrMaxSharedMemoryPerBlockOptin
@@ -1629,9 +1669,9 @@ int launch_rebuild_chain(mdpd_ctx* h, bool with_list = true) {
 
 int launch_forces(mdpd_ctx* h, bool all) {
   const DevP& d = h->d;
-  if (!h->has_wall) LAUNCH(h, PS_DENSITY, (k_density<false, false><<<d.ntiles, h->block, h->smem_pos, h->ls>>>(d)));
-  else if (all) LAUNCH(h, PS_DENSITY, (k_density<true, true><<<d.ntiles, h->block, h->smem_pos, h->ls>>>(d)));
-  else LAUNCH(h, PS_DENSITY, (k_density<true, false><<<d.ntiles, h->block, h->smem_pos, h->ls>>>(d)));
+  if (!h->has_wall) LAUNCH(h, PS_DENSITY, (k_density<false, false><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
+  else if (all) LAUNCH(h, PS_DENSITY, (k_density<true, true><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
+  else LAUNCH(h, PS_DENSITY, (k_density<true, false><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
   if (all) LAUNCH(h, PS_FORCE, (k_force<true><<<d.ntiles, h->block, h->smem_posvel, h->ls>>>(d)));
   else LAUNCH(h, PS_FORCE, (k_force<false><<<d.ntiles, h->block, h->smem_posvel, h->ls>>>(d)));
   return MDPD_OK;
@@ -1870,7 +1910,7 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
   }
   // Tile shape: the largest candidate that still gives every SM work and whose most populated tile + halo fits in
   // shared memory (checked on the device after the sort); MDPD_TILE="tx,ty,tz" / MDPD_BLOCK override for experiments.
-  static const int kCand[][3] = {{4, 4, 2}, {4, 2, 2}, {2, 2, 2}, {2, 2, 1}, {2, 1, 1}, {1, 1, 1}};
+  static const int kCand[][3] = {{4, 4, 4}, {4, 4, 2}, {4, 2, 2}, {2, 2, 2}, {2, 2, 1}, {2, 1, 1}, {1, 1, 1}};
   const int ncand = (int)(sizeof kCand / sizeof kCand[0]);
   int first = 0;
   int forced[3] = {0, 0, 0};
@@ -1880,7 +1920,7 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
     auto ntiles_of = [&](const int* t) {
       return (size_t)((L.ncx + t[0] - 1) / t[0]) * ((L.ncy + t[1] - 1) / t[1]) * ((L.ncz + t[2] - 1) / t[2]);
     };
-    while (first < 2 && ntiles_of(kCand[first]) < 148) ++first;  // small boxes: down to 2 x 2 x 2
+    while (first < 3 && ntiles_of(kCand[first]) < 148) ++first;  // small boxes: down to 2 x 2 x 2
   }
   for (int ci = first; ci < ncand; ++ci) {
     const int* cand = force_tile ? forced : kCand[ci];
@@ -1895,7 +1935,7 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
       return set_err(h, MDPD_ENOMEM, "tile run table does not fit its reservation");
     const int vol = tdim[0] * tdim[1] * tdim[2];
     h->block = TILE_TPB;  // upper bound while the capacity is probed; set from the tile population below
-    h->block_build = vol >= 32 ? 256u : 128u;
+    h->block_build = vol >= 64 ? BUILD_TPB : (vol >= 32 ? std::min(256, BUILD_TPB) : 128u);
     const size_t fixed = tile_smem_bytes(0, true, 0);
     const unsigned cap_limit = (unsigned)std::min<size_t>((h->smem_limit - fixed) / TILE_SLOT_BYTES, 65535);
     h->d.tile_cap = cap_limit;
@@ -1916,14 +1956,17 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
       continue;  // try the next smaller tile shape
     }
     // density / force passes: one thread per own particle of the fullest tile (a tile with more loops)
-    h->block = std::min<unsigned>(TILE_TPB, std::max(64u, (h->h_ctl->max_own + 31u) / 32u * 32u));
+    // two rounds on the fullest tile: every warp gets a long and a short group of own particles (see sort_own_by_length)
+    const unsigned half_own = ((h->h_ctl->max_own + 1u) / 2u + 31u) / 32u * 32u;
+    h->block = std::min<unsigned>(TILE_TPB, std::max(64u, half_own));
+    h->block_dens = std::min<unsigned>(DENS_TPB, std::max(64u, half_own));
     if (const char* e = getenv("MDPD_BLOCK")) {
       int b = atoi(e);
       if (b >= 32 && b <= TILE_TPB && b % 32 == 0) h->block = (unsigned)b;
     }
     if (const char* e = getenv("MDPD_BLOCK_BUILD")) {
       int b = atoi(e);
-      if (b >= 32 && b <= 256 && b % 32 == 0) h->block_build = (unsigned)b;
+      if (b >= 32 && b <= BUILD_TPB && b % 32 == 0) h->block_build = (unsigned)b;
     }
     // head-room for density fluctuations between rebuilds of a long run
     {

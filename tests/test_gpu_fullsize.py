@@ -41,7 +41,7 @@ def test_config4b_one_million_particles_every_particle(gpu):
     s.step(8)
     st = s.get_state()
     ctr = s.counters()
-    assert ctr["faults"] == 0 and ctr["rebuilds"] >= 2 and ctr["tile_shape"] == (4 | 4 << 8 | 2 << 16)
+    assert ctr["faults"] == 0 and ctr["rebuilds"] >= 2 and ctr["tile_shape"] == (4 | 4 << 8 | 4 << 16)
     # pairwise forces are antisymmetric bitwise => total momentum only moves by fp32 rounding of the kicks
     p1 = st["vel"].astype(np.float64).sum(0)
     assert np.abs(p1 - p0).max() < 1e-6 * n, (p0, p1)
