@@ -170,10 +170,11 @@ def algorithmic_bytes(kernel, n, n_list, n_act):
     return None if per is None else per * n
 
 
-def algorithmic_ops(kernel, n, n_list, n_act):
+def algorithmic_ops(kernel, n, n_list, n_act, n_cand=0.0):
     """Thread-level arithmetic/logic operations the formulas need (FMA = 1, no address or loop
-    arithmetic): 13 per listed entry in the density pass (r^2, compare, weight), 48 per in-range pair in the force pass."""
-    per = {"k_density": 13 * n_list, "k_force": 48 * n_act}.get(kernel)
+    arithmetic): 13 per listed entry in the density pass (r^2, compare, weight), 48 per in-range pair in the force pass,
+    7 per candidate of the 27-cell stencil (r^2, compare) in the list build."""
+    per = {"k_density": 13 * n_list, "k_force": 48 * n_act, "k_build_list": 7 * n_cand}.get(kernel)
     return None if per is None else per * n
 
 
@@ -280,7 +281,13 @@ def main_ours(args, rank, world, local):
         (6650.0, "B200_PROFILING.md fallback")
     clocks = clk.summary()
     sm_mhz = clocks.get("sm_mhz") or clocks.get("sm_max_mhz") or 1965.0
-    alu_peak = 148 * 128 * sm_mhz * 1e6 / 1e9       # Gop/s: 148 SMs x 4 sub-partitions x 32 lanes x f_clk
+    # ALU peak: the FP32 FMA issue rate of this GPU measured in this run by the library's own probe kernels
+    # (mdpd_probe_issue_rates), x 32 lanes; the nominal figure 148 SMs x 128 lanes x f_clk is kept beside it
+    rates = pk.probe_issue_rates(local)
+    alu_nominal = 148 * 128 * sm_mhz * 1e6 / 1e9
+    alu_peak = rates["ffma"] * 32 / 1e9             # Gop/s (thread-level operations)
+    ncell = int(np.prod([int(np.floor(b / (c["params"]["rc"] + c["params"]["skin"]))) for b in c["params"]["box"]]))
+    n_cand = 27.0 * n / ncell                       # candidates per particle: the 27-cell stencil at the mean occupancy
 
     def launch_ms(k):   # mean duration of the launches that did work (rebuild-chain kernels: real rebuilds only)
         cnt = reb_prof if k == "k_build_list" else prof[k][1]
@@ -296,7 +303,7 @@ def main_ours(args, rank, world, local):
         if b:
             ent["hbm_gbs"] = round(b / (t * 1e-3) / 1e9, 1)
             ent["hbm_frac"] = round(ent["hbm_gbs"] / peak_gbs, 4)
-        o = algorithmic_ops(k, n, n_list, n_act)
+        o = algorithmic_ops(k, n, n_list, n_act, n_cand)
         if o:
             ent["alu_gops"] = round(o / (t * 1e-3) / 1e9, 1)
             ent["alu_frac"] = round(ent["alu_gops"] / alu_peak, 4)
@@ -306,12 +313,19 @@ def main_ours(args, rank, world, local):
     if d.get("alu_frac", 0) >= d.get("hbm_frac", 0) and "alu_gops" in d:
         roof = {"bound": "alu", "kernel": dom, "achieved": d["alu_gops"], "peak": round(alu_peak, 1), "unit": "Gop/s",
                 "frac": d["alu_frac"],
-                "peak_source": f"148 SMs x 128 lanes x {sm_mhz:.0f} MHz sampled in this run (DESIGN.md section 7)",
-                "algorithmic_ops_per_launch": algorithmic_ops(dom, n, n_list, n_act)}
+                "peak_source": "FP32 FMA issue rate measured in this run by mdpd_probe_issue_rates x 32 lanes "
+                               f"(nominal 148 SMs x 128 lanes x {sm_mhz:.0f} MHz = {alu_nominal:.0f} Gop/s; DESIGN.md section 7)",
+                "algorithmic_ops_per_launch": algorithmic_ops(dom, n, n_list, n_act, n_cand),
+                "issue_rates_gwinst_s": {k: round(v / 1e9, 1) for k, v in rates.items() if k != "sm_clock_hz"}}
     else:
         roof = {"bound": "hbm", "kernel": dom, "achieved": d.get("hbm_gbs"), "peak": peak_gbs, "unit": "GB/s",
                 "frac": d.get("hbm_frac"), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": algorithmic_bytes(dom, n, n_list, n_act)}
+    # the whole step against the same ALU peak: algorithmic operations of all launches of the profiled window / its time
+    win_ops = K * (algorithmic_ops("k_density", n, n_list, n_act) + algorithmic_ops("k_force", n, n_list, n_act)) + \
+        reb_prof * algorithmic_ops("k_build_list", n, n_list, n_act, n_cand)
+    roof["step"] = {"alu_gops": round(win_ops / (tot * 1e-3) / 1e9, 1), "alu_frac": round(win_ops / (tot * 1e-3) / 1e9 / alu_peak, 4),
+                    "ops_per_particle_step": round(win_ops / (n * K), 1)}
     roof["ms_per_launch"] = d.get("ms_per_launch")
     roof["traffic"] = None
     roof["hbm_peak_gbs"] = peak_gbs

@@ -129,7 +129,7 @@ int mdpd_rng_fill(mdpd_ctx* h, uint64_t npairs, const uint32_t* pairs, uint32_t 
  * tile (tile + halo) at the last build, [6] device fault events (list / tile overflows + non-finite coordinates; also
  * latched as an error code), [7] kernels launched by this handle so far, [8] sum over all density passes so far of
  * the in-range (r < rc) neighbour counts = pair evaluations of the force passes, [9] number of density passes so far,
- * [10] tile shape tx | ty << 8 | tz << 16 (cells), [11] number of tiles; [12..15] reserved (0).
+ * [10] tile shape tx | ty << 8 | tz << 16 (cells), [11] number of tiles; [12..15] see below (0 in a normal build).
  * Synchronises the stream. */
 int mdpd_get_counters(mdpd_ctx* h, uint64_t out[MDPD_NCOUNTERS]);
 
@@ -145,6 +145,16 @@ int mdpd_profile_begin(mdpd_ctx* h);
 int mdpd_profile_end(mdpd_ctx* h, double ms[MDPD_PROF_SLOTS], uint64_t launches[MDPD_PROF_SLOTS]);
 /* Name of a kernel slot ("k_force", "k_density", ...; "" past the last one).  Static storage. */
 const char* mdpd_profile_name(int slot);
+
+/* Issue-rate probe for the ALU roofline: runs three short register-only kernels on `device`
+ * (every SM, 64 resident warps, 8 independent dependency chains per thread), timed with CUDA events on `cuda_stream`, and
+ * returns warp-instructions per second of the whole GPU: out[0] FP32 FMA (FFMA), out[1] logic pipe (LOP3 + VIMNMX),
+ * out[2] 32 x 32 -> 64 integer multiply (IMAD.WIDE, the hash's multiply); out[3] = the SM clock [Hz] the runtime
+ * reports as maximum.  No handle needed.  Returns MDPD_OK or MDPD_ECUDA. */
+int mdpd_probe_issue_rates(int device, void* cuda_stream, double out[4]);
+
+/* [12..15] of mdpd_get_counters: clock cycles of k_force's staging and pair loop summed over CTAs, and the CTA count,
+ * when the library was built with -DMDPD_PHASES (a tuning aid); 0 otherwise. */
 
 #ifdef __cplusplus
 }

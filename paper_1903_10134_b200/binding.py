@@ -26,7 +26,7 @@ SYMBOLS = ("mdpd_create", "mdpd_destroy", "mdpd_set_params", "mdpd_workspace_byt
            "mdpd_load_particles", "mdpd_load_wall_mask", "mdpd_step", "mdpd_get_state", "mdpd_set_step_counter",
            "mdpd_set_forces",
            "mdpd_compute_forces", "mdpd_get_pairs", "mdpd_rng_fill", "mdpd_get_counters", "mdpd_last_error",
-           "mdpd_profile_begin", "mdpd_profile_end", "mdpd_profile_name")
+           "mdpd_profile_begin", "mdpd_profile_end", "mdpd_profile_name", "mdpd_probe_issue_rates")
 MDPD_PROF_SLOTS = 16
 
 
@@ -91,6 +91,7 @@ def lib():
         L.mdpd_profile_end.argtypes = [vp, vp, vp]
         L.mdpd_profile_name.argtypes = [i32]
         L.mdpd_profile_name.restype = C.c_char_p
+        L.mdpd_probe_issue_rates.argtypes = [i32, vp, vp]
         for s in SYMBOLS:
             getattr(L, s).restype = getattr(L, s).restype  # touch: AttributeError if a symbol is missing
         _lib = L
@@ -108,6 +109,17 @@ def _ptr(a):
 
 COUNTER_NAMES = ("steps", "rebuilds", "bounces", "max_nbr", "sum_nbr", "max_staged", "faults", "launches",
                  "sum_act", "density_passes", "tile_shape", "ntiles")
+
+
+def probe_issue_rates(device: int = 0, stream=None):
+    """mdpd_probe_issue_rates: measured warp-instructions/s of the whole GPU for FFMA, the logic pipe and IMAD.WIDE."""
+    import torch
+    st = (stream or torch.cuda.current_stream(device)).cuda_stream
+    out = np.zeros(4, np.float64)
+    rc = lib().mdpd_probe_issue_rates(int(device), C.c_void_p(st), out.ctypes.data)
+    if rc != MDPD_OK:
+        raise MdpdError(rc, "mdpd_probe_issue_rates")
+    return {"ffma": float(out[0]), "logic": float(out[1]), "imad_wide": float(out[2]), "sm_clock_hz": float(out[3])}
 
 
 class Simulation:

@@ -7,8 +7,8 @@
 // Device state: pos float4 = (x, y, z, bits(tag | type << 31)), vel float4 = (vx, vy, vz, rho),
 // both double-buffered for the counting sort into tiles of cells (tiles along the Z-curve, cells x-fastest inside a
 // tile); force float4; xbuild float4 (positions at the last list build); Verlet list of 16-bit indices into the
-// tile's staged shared-memory array, split in a near part (r < rd + skin at build: all the density pass needs) and a
-// far part, both stored column-major ([k][i]) so that a warp reads consecutive i at fixed k in one coalesced request.
+// tile's staged shared-memory image, stored in 16-byte chunks of 8 entries, layout [chunk][particle]; per tile a
+// staging recipe (runs of contiguous halo cells) and per particle the hand-out records of the two per-step passes.
 #include "mdpd.h"
 
 #include <cuda_runtime.h>
@@ -790,11 +790,7 @@ __device__ __forceinline__ void sort_own_by_length(const TileSmem& sm, unsigned 
     }
   }
   __syncthreads();
-#ifdef MDPD_DENS_NATURAL
-  for (unsigned t = threadIdx.x; t < nown; t += blockDim.x) out[t] = rec(t);
-#else
   for (unsigned t = threadIdx.x; t < nown; t += blockDim.x) out[atomicAdd(&hist[LCAP - min(len(t), LCAP)], 1u)] = rec(t);
-#endif
 }
 
 // group of 32 sorted own particles that warp `warp` of W takes in its round r (see above)
@@ -1035,13 +1031,7 @@ template <bool HAS_WALL>
 __device__ __forceinline__ void density_entry(const DevP& p, const unsigned pbase, const float4 xi, const unsigned walli,
                                               const unsigned j, float& rho, unsigned& a0, unsigned& a1, unsigned& a2,
                                               unsigned& a3, unsigned& na, uint4*& ao) {
-#ifdef MDPD_ABL_NOGATHER
-  const float4 xj = make_float4(u2f(j), u2f(j << 3), u2f(j << 7), 0.f);
-#elif defined(MDPD_FAKE_NOCONFLICT)  // timing experiment only (wrong results): every quarter-warp hits 8 distinct bank groups
-  const float4 xj = lds4(pbase + ((((j & ~7u) | (threadIdx.x & 7u)) << 4)));
-#else
   const float4 xj = lds4(pbase + (j << 4));  // padding entries hit the far-away sentinel
-#endif
   const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
   const float r2 = dx * dx + dy * dy + dz * dz;
   // The logic pipe (min/max, compares, shifts, selects) issues at half the rate of the FP32 pipe and bounds this loop:
@@ -1053,10 +1043,6 @@ __device__ __forceinline__ void density_entry(const DevP& p, const unsigned pbas
   // the upper bound could matter (1e-12 is far below half an ulp of rc2)
   bool in = f2u(r2 - 1e-12f) < f2u(p.rc2 - 1e-12f);  // interacts at this step
   if (HAS_WALL) in = in && !(walli & (f2u(xj.w) >> 31));  // frozen-frozen pairs do not (R8)
-#ifdef MDPD_ABL_NOPUSH
-  na += in ? 1u : 0u;
-  return;
-#endif
   const unsigned sh = in ? 16u : 0u;
   a0 = __funnelshift_r(a0, a1, sh);
   a1 = __funnelshift_r(a1, a2, sh);
@@ -1092,9 +1078,6 @@ __global__ void __launch_bounds__(DENS_TPB, DENS_MINB) k_density(const DevP p) {
 #pragma unroll
   for (int r = 0; r < PRE; ++r) head[r] = info[r].y ? p.nbr[os + (info[r].x & 0xFFFFu)] : make_uint4(0, 0, 0, 0);
   if (!stage_fast<false>(p, T, hdr, p.pos[cur], nullptr, sm)) return;  // flagged by k_build_list
-#ifdef MDPD_ABL_STAGEONLY
-  if (p.N) return;
-#endif
   float4* __restrict__ vel = p.vel[cur];
   const unsigned sent = p.tile_cap;
   const unsigned pbase = smem_addr(sm.spos);
@@ -1169,9 +1152,6 @@ __global__ void __launch_bounds__(DENS_TPB, DENS_MINB) k_density(const DevP p) {
     }
     return true;
   };
-#ifdef MDPD_ABL_NOTAIL
-  if (p.N) return;
-#endif
   na_sum = __reduce_add_sync(0xffffffffu, na_sum);
   __syncthreads();  // hist is zero, every particle of the tile is done
   if (lane == 0 && na_sum) atomicAdd(&hist[HTAB - 1], na_sum);
@@ -1221,14 +1201,8 @@ struct ForceAcc {
 __device__ __forceinline__ void force_entry(const DevP& p, const unsigned pbase, const unsigned vbase, const float4 xi,
                                             const float4 vi, const unsigned tagi, const unsigned j, const HashKeys& K,
                                             ForceAcc& acc) {
-#ifdef MDPD_FAKE_NOCONFLICT
-  const unsigned jj = (j & ~7u) | (threadIdx.x & 7u);
-  const float4 xj = lds4(pbase + (jj << 4));
-  const float4 vj = lds4(vbase + (jj << 4));
-#else
   const float4 xj = lds4(pbase + (j << 4));
   const float4 vj = lds4(vbase + (j << 4));
-#endif
   const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
   const float r2 = dx * dx + dy * dy + dz * dz;  // > 1e-12 for list entries; 3e18 for the sentinel
   const float rinv = rsqrt_fast(r2);
@@ -1377,6 +1351,37 @@ __global__ void k_rng_fill(unsigned long long n, const uint2* __restrict__ pairs
   if (q >= n) return;
   const HashKeys K = make_keys(step, seed);
   out[q] = pair_hash(pairs[q].x, pairs[q].y, K);
+}
+
+// ----------------------------------------------------------------------------------------------------------------
+// Issue-rate probe (mdpd_probe_issue_rates): register-only kernels, 8 independent chains per thread, so that the pipe
+// and not the dependency latency bounds them.  KIND 0: FFMA; 1: LOP3 + VIMNMX (the logic pipe); 2: IMAD.WIDE + the
+// add that closes its chain.  The unused result is stored under a condition that never holds.
+// ----------------------------------------------------------------------------------------------------------------
+constexpr int PROBE_CH = 8, PROBE_ITER = 2048, PROBE_TPB = 1024;
+template <int KIND>
+__global__ void __launch_bounds__(PROBE_TPB) k_probe(float* out, float a, float b, unsigned ua, unsigned ub) {
+  float x[PROBE_CH];
+  unsigned u[PROBE_CH];
+  unsigned long long w[PROBE_CH];
+#pragma unroll
+  for (int c = 0; c < PROBE_CH; ++c) {
+    x[c] = (float)threadIdx.x * 1e-3f + (float)c;
+    u[c] = threadIdx.x * 77u + (unsigned)c;
+    w[c] = u[c];
+  }
+  for (int it = 0; it < PROBE_ITER; ++it) {
+#pragma unroll
+    for (int c = 0; c < PROBE_CH; ++c) {
+      if (KIND == 0) x[c] = fmaf(x[c], a, b);
+      if (KIND == 1) u[c] = max(u[c], ua) ^ ub;
+      if (KIND == 2) w[c] = (unsigned long long)(unsigned)w[c] * 0xD256D193ull + (w[c] >> 32);
+    }
+  }
+  float sum = 0.f;
+#pragma unroll
+  for (int c = 0; c < PROBE_CH; ++c) sum += x[c] + (float)u[c] + (float)w[c];
+  if (sum == 12345.678f) out[0] = sum;
 }
 
 // ----------------------------------------------------------------------------------------------------------------
@@ -2242,5 +2247,44 @@ int mdpd_profile_end(mdpd_ctx* h, double ms[MDPD_PROF_SLOTS], uint64_t launches[
 }
 
 const char* mdpd_profile_name(int slot) { return (slot >= 0 && slot < PS_COUNT) ? kProfNames[slot] : ""; }
+
+int mdpd_probe_issue_rates(int device, void* cuda_stream, double out[4]) {
+  if (!out) return MDPD_EINVAL;
+  for (int k = 0; k < 4; ++k) out[k] = 0.0;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int sms = 0, khz = 0;
+  if (cudaSetDevice(device) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess ||
+      cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, device) != cudaSuccess)
+    return MDPD_ECUDA;
+  float* sink = nullptr;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (cudaMalloc((void**)&sink, 4) != cudaSuccess) return MDPD_ECUDA;
+  int rc = MDPD_OK;
+  if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) rc = MDPD_ECUDA;
+  const int blocks = sms * 2;  // 2 x 1024 threads = 64 resident warps per SM
+  const double per_iter[3] = {1.0, 2.0, 2.0};  // warp instructions per chain and iteration (FFMA; LOP3 + VIMNMX; IMAD.WIDE + IADD)
+  for (int kind = 0; kind < 3 && rc == MDPD_OK; ++kind) {
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {  // the first repetition warms up
+      cudaEventRecord(e0, st);
+      if (kind == 0) k_probe<0><<<blocks, PROBE_TPB, 0, st>>>(sink, 1.0001f, 0.5f, 0x9E3779B9u, 0x12345u);
+      if (kind == 1) k_probe<1><<<blocks, PROBE_TPB, 0, st>>>(sink, 1.0001f, 0.5f, 0x9E3779B9u, 0x12345u);
+      if (kind == 2) k_probe<2><<<blocks, PROBE_TPB, 0, st>>>(sink, 1.0001f, 0.5f, 0x9E3779B9u, 0x12345u);
+      cudaEventRecord(e1, st);
+      if (cudaEventSynchronize(e1) != cudaSuccess) { rc = MDPD_ECUDA; break; }
+      float ms = 0.f;
+      cudaEventElapsedTime(&ms, e0, e1);
+      if (rep > 0 && ms < best) best = ms;
+    }
+    const double winst = (double)blocks * (PROBE_TPB / 32) * PROBE_ITER * PROBE_CH * per_iter[kind];
+    out[kind] = winst / ((double)best * 1e-3);
+  }
+  out[3] = (double)khz * 1e3;
+  if (cudaGetLastError() != cudaSuccess) rc = MDPD_ECUDA;
+  if (e0) cudaEventDestroy(e0);
+  if (e1) cudaEventDestroy(e1);
+  cudaFree(sink);
+  return rc;
+}
 
 }  // extern "C"
