@@ -37,6 +37,8 @@
 #define REF_ESTATE (-5)
 #define REF_EINSOLID (-7)
 
+#define MDPD_REF_MAXTYPES 8
+
 typedef struct {
   double box[3];
   double rc, rd;
@@ -55,7 +57,15 @@ typedef struct mdpd_ref_ctx {
   int have_params;
   uint64_t n;
   double *x, *v, *f, *fpair, *rho; /* [n][3], [n] ; index == tag == load order */
-  uint8_t *type;
+  uint8_t *type;    /* 1: frozen (never integrated), 0: mobile */
+  uint8_t *species; /* material type of the particle: row / column of the pair-parameter matrices below */
+  /* Per-type-pair conservative parameters ("A_SL, B_SL"; Tables 1-2): ntypes == 0 means
+   * one material, A and B of mdpd_ref_params for every pair, type byte != 0 <=> frozen.  Otherwise the type byte of a
+   * particle is its species s in [0, ntypes), the pair (i, j) uses Am[s_i][s_j], Bm[s_i][s_j] (symmetric), and species s
+   * is frozen iff bit s of frozen_mask is set. */
+  int ntypes;
+  double Am[MDPD_REF_MAXTYPES * MDPD_REF_MAXTYPES], Bm[MDPD_REF_MAXTYPES * MDPD_REF_MAXTYPES];
+  uint32_t frozen_mask;
   uint8_t *mask; /* [nz][ny][nx], 1 = solid */
   uint32_t mdim[3];
   double voxel;
@@ -113,9 +123,9 @@ int mdpd_ref_create(mdpd_ref_ctx **out) {
 }
 
 static void free_particles(mdpd_ref_ctx *h) {
-  free(h->x); free(h->v); free(h->f); free(h->fpair); free(h->rho); free(h->type); free(h->next);
+  free(h->x); free(h->v); free(h->f); free(h->fpair); free(h->rho); free(h->type); free(h->species); free(h->next);
   h->x = h->v = h->f = h->fpair = h->rho = NULL;
-  h->type = NULL; h->next = NULL; h->n = 0;
+  h->type = NULL; h->species = NULL; h->next = NULL; h->n = 0;
 }
 
 int mdpd_ref_destroy(mdpd_ref_ctx *h) {
@@ -134,6 +144,23 @@ int mdpd_ref_set_params(mdpd_ref_ctx *h, const mdpd_ref_params *p) {
     if (!(p->box[d] >= 2.0 * p->rc)) return REF_EINVAL; /* minimum image needs L >= 2 rc */
   h->p = *p;
   h->have_params = 1;
+  return REF_OK;
+}
+
+/* Pair-parameter matrices ([ntypes][ntypes], symmetric) and the set of frozen species; before load_particles.
+ * ntypes == 0 returns to one material. */
+int mdpd_ref_set_pair_params(mdpd_ref_ctx *h, int ntypes, const double *A, const double *B, uint32_t frozen_mask) {
+  if (!h || ntypes < 0 || ntypes > MDPD_REF_MAXTYPES) return REF_EINVAL;
+  if (h->n) return REF_ESTATE;
+  if (ntypes && (!A || !B)) return REF_EINVAL;
+  for (int a = 0; a < ntypes; ++a)
+    for (int b = 0; b < ntypes; ++b) {
+      if (A[a * ntypes + b] != A[b * ntypes + a] || B[a * ntypes + b] != B[b * ntypes + a]) return REF_EINVAL;
+      h->Am[a * ntypes + b] = A[a * ntypes + b];
+      h->Bm[a * ntypes + b] = B[a * ntypes + b];
+    }
+  h->ntypes = ntypes;
+  h->frozen_mask = frozen_mask;
   return REF_OK;
 }
 
@@ -263,7 +290,12 @@ static void force_pair(mdpd_ref_ctx *h, uint64_t i, uint64_t j, const double d[3
   for (int k = 0; k < 3; ++k) ev += e[k] * (h->v[3 * i + k] - h->v[3 * j + k]);
   uint32_t hh = mdpd_ref_hash((uint32_t)i, (uint32_t)j, (uint32_t)h->step, p->seed); /* i < j here */
   double xi = mdpd_ref_xi(hh);
-  double FC = p->A * w + p->B * (h->rho[i] + h->rho[j]) * wd;          /* Eq. (1) */
+  double Aij = p->A, Bij = p->B;
+  if (h->ntypes) { /* per-type-pair parameters */
+    Aij = h->Am[h->species[i] * h->ntypes + h->species[j]];
+    Bij = h->Bm[h->species[i] * h->ntypes + h->species[j]];
+  }
+  double FC = Aij * w + Bij * (h->rho[i] + h->rho[j]) * wd;            /* Eq. (1) */
   double FD = -p->gamma * wR * wR * ev;                                /* P:L75, wD = wR^2 */
   double FR = p->sigma * wR * xi / sqrt(p->dt);                        /* P:L75; R2 */
   double F = FC + FD + FR;
@@ -315,10 +347,19 @@ int mdpd_ref_load_particles(mdpd_ref_ctx *h, uint64_t n, const double *pos, cons
   h->fpair = (double *)calloc(3 * m, sizeof(double));
   h->rho = (double *)calloc(m, sizeof(double));
   h->type = (uint8_t *)calloc(m, 1);
+  h->species = (uint8_t *)calloc(m, 1);
   h->next = (int64_t *)calloc(m, sizeof(int64_t));
-  if (!h->x || !h->v || !h->f || !h->fpair || !h->rho || !h->type || !h->next) return REF_ENOMEM;
+  if (!h->x || !h->v || !h->f || !h->fpair || !h->rho || !h->type || !h->species || !h->next) return REF_ENOMEM;
   for (uint64_t i = 0; i < n; ++i) {
-    h->type[i] = type ? (type[i] != 0) : 0;
+    if (h->ntypes) {
+      const uint8_t sp = type ? type[i] : 0;
+      if (sp >= h->ntypes) return REF_EINVAL;
+      h->species[i] = sp;
+      h->type[i] = (uint8_t)((h->frozen_mask >> sp) & 1u);
+    } else {
+      h->type[i] = type ? (type[i] != 0) : 0;
+      h->species[i] = h->type[i];
+    }
     for (int k = 0; k < 3; ++k) {
       h->x[3 * i + k] = wrap(pos[3 * i + k], h->p.box[k]);
       h->v[3 * i + k] = h->type[i] ? 0.0 : vel[3 * i + k]; /* frozen: v == 0 (R8) */

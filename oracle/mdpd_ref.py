@@ -51,6 +51,7 @@ def lib():
         L.mdpd_ref_destroy.argtypes = [vp]
         L.mdpd_ref_set_params.argtypes = [vp, C.POINTER(_Params)]
         L.mdpd_ref_set_brute_force.argtypes = [vp, C.c_int]
+        L.mdpd_ref_set_pair_params.argtypes = [vp, C.c_int, vp, vp, u32]
         L.mdpd_ref_compute_forces.argtypes = [vp]
         L.mdpd_ref_load_particles.argtypes = [vp, u64, vp, vp, vp]
         L.mdpd_ref_load_wall_mask.argtypes = [vp, vp, vp, C.c_double]
@@ -113,6 +114,19 @@ class RefSim:
             self.close()
         except Exception:
             pass
+
+    def set_pair_params(self, A, B, frozen_mask=0):
+        """Per-type-pair A_ij, B_ij ([nt][nt], symmetric; P:L152, Tables 1-2) and the set of frozen species (bit s);
+        call before load_particles, whose type byte is then the species index.  A = None: back to one material."""
+        if A is None:
+            _check(self._L.mdpd_ref_set_pair_params(self._h, 0, None, None, 0), "set_pair_params")
+            return
+        A = np.ascontiguousarray(A, np.float64)
+        B = np.ascontiguousarray(B, np.float64)
+        nt = A.shape[0]
+        assert A.shape == (nt, nt) and B.shape == (nt, nt)
+        _check(self._L.mdpd_ref_set_pair_params(self._h, nt, A.ctypes.data, B.ctypes.data, int(frozen_mask)),
+               "set_pair_params")
 
     def load_particles(self, pos, vel, type=None):
         pos = np.ascontiguousarray(pos, np.float64).reshape(-1, 3)

@@ -55,8 +55,9 @@ def brute_density(pos, box, rd):
     return w.sum(1)
 
 
-def brute_forces(pos, vel, typ, p, step, rho=None):
-    """O(N^2) total force per particle (pairwise part + m g on fluid), fp64, python-loop hash."""
+def brute_forces(pos, vel, typ, p, step, rho=None, species=None, Amat=None, Bmat=None):
+    """O(N^2) total force per particle (pairwise part + m g on fluid), fp64, python-loop hash.
+    typ: frozen flags.  species / Amat / Bmat: per-type-pair A_ij, B_ij (Tables 1-2); default one material."""
     pos = np.asarray(pos, np.float64)
     vel = np.asarray(vel, np.float64).copy()
     typ = np.asarray(typ).astype(bool)
@@ -80,7 +81,8 @@ def brute_forces(pos, vel, typ, p, step, rho=None):
         wd = max(0.0, 1.0 - r / p["rd"])
         wR = w ** p["s"]
         xi = xi_py(hash_py(i, j, step, p["seed"]))
-        F = (p["A"] * w + p["B"] * (rho[i] + rho[j]) * wd
+        A, B = (p["A"], p["B"]) if species is None else (Amat[species[i]][species[j]], Bmat[species[i]][species[j]])
+        F = (A * w + B * (rho[i] + rho[j]) * wd
              - p["gamma"] * wR * wR * float(e @ (vel[i] - vel[j]))
              + p["sigma"] * wR * xi / math.sqrt(p["dt"]))
         f[i] += F * e
