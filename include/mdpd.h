@@ -70,6 +70,17 @@ int mdpd_destroy(mdpd_ctx* h);
  * gamma, sigma, kT may change (box, cut-offs, skin, capacities are frozen: MDPD_ESTATE otherwise). */
 int mdpd_set_params(mdpd_ctx* h, const mdpd_params* p);
 
+/* Per-type-pair conservative parameters of Eq. (1) ("the particle interaction force between two types
+ * of materials such as solid and liquid can be modified by adjusting A_SL, B_SL"; Tables 1 and 2, PAPER.md L155-160,
+ * L188-192; five material types in the kerogen case, L247).  A, B: [ntypes][ntypes] float32 row-major HOST arrays,
+ * symmetric (else MDPD_EINVAL), ntypes <= 8.  After this call the `type` byte of mdpd_load_particles is the SPECIES
+ * index s in [0, ntypes) (a larger value: MDPD_EINVAL at load), the pair (i, j) uses A[s_i][s_j], B[s_i][s_j] in place
+ * of mdpd_params.A / .B, and species s is frozen (never integrated, v = 0, R8) iff bit s of frozen_mask is
+ * set.  gamma, sigma, rc, rd stay those of mdpd_params for every pair.  Call before mdpd_load_particles; afterwards
+ * only the VALUES may change (same ntypes and frozen_mask, else MDPD_ESTATE).  ntypes = 0 returns to one material
+ * (type byte != 0 <=> frozen wall). */
+int mdpd_set_pair_params(mdpd_ctx* h, uint32_t ntypes, const float* A, const float* B, uint32_t frozen_mask);
+
 /* Device bytes needed for n particles (+ an optional mask of mask_dims = {nx, ny, nz} voxels).  Returns 0 on bad input. */
 size_t mdpd_workspace_bytes(const mdpd_params* p, uint64_t n, int has_mask, const uint32_t mask_dims[3]);
 

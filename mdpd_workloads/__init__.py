@@ -19,6 +19,8 @@ from .generators import (  # noqa: F401
     make_slab,
     make_poiseuille,
     make_pore_network,
+    make_species_mixture,
+    make_slit_wetting,
     make_config,
     quantise_positions,
     maxwell_velocities,

@@ -196,6 +196,46 @@ def make_pore_network(nvox=128, voxel=0.5, corr=6.0, porosity=0.35, density=6.0,
                 pos=pos, vel=vel, type=typ, mask=mask, voxel=float(voxel))
 
 
+def make_species_mixture(box=(12.0, 10.0, 9.0), nspecies=5, frozen_mask=0b01010, density=6.0, seed=BASE_SEED + 5, **pover):
+    """A liquid of `nspecies` material types drawn uniformly (type byte = species index), the species of `frozen_mask`
+    frozen, with random symmetric pair matrices A_ij in [-40, -20], B_ij in [22, 28]: stands in for the five material
+    types of the paper's kerogen case, whose parameter table is not in the text."""
+    c = make_liquid(box, density=density, seed=seed, **pover)
+    rng = np.random.default_rng(seed + 1000)
+    n = len(c["pos"])
+    c["type"] = rng.integers(0, nspecies, n).astype(np.uint8)
+    A = (-40.0 + 20.0 * rng.random((nspecies, nspecies))).astype(np.float32)
+    B = (22.0 + 6.0 * rng.random((nspecies, nspecies))).astype(np.float32)
+    c["pair_A"] = np.maximum(A, A.T)
+    c["pair_B"] = np.maximum(B, B.T)
+    c["frozen_mask"] = int(frozen_mask)
+    frozen = ((c["frozen_mask"] >> c["type"]) & 1).astype(bool)
+    c["vel"][frozen] = 0.0
+    c["name"] = "species_mixture"
+    return c
+
+
+def make_slit_wetting(A_SL=-30.0, seed=BASE_SEED + 6, **pover):
+    """Section 4.2's slit pore shifted into [0, L): box 60 x 10 x 5, 3 500 solid particles (species 1,
+    frozen) uniformly random in each of the wall regions 0 <= y < 1 and 9 <= y < 10, 4 000 liquid particles (species 0)
+    in a block 20 <= x < 40, 1 < y < 9; A_SS = A_LL = -40, the unlike pair A_SL from Table 1, B = 25 (R19)."""
+    box = (60.0, 10.0, 5.0)
+    rng = np.random.default_rng(seed)
+    def block(n, lo, hi):
+        u = rng.random((n, 3), dtype=np.float32)
+        return (np.asarray(lo, np.float32) + u * (np.asarray(hi, np.float32) - np.asarray(lo, np.float32))).astype(np.float32)
+    w0 = block(3500, (0, 0, 0), (60, 1, 5))
+    w1 = block(3500, (0, 9, 0), (60, 10, 5))
+    liq = block(4000, (20, 1.05, 0), (40, 8.95, 5))
+    pos = _clip_into_box(np.concatenate([liq, w0, w1]), box)
+    vel = np.concatenate([maxwell_velocities(rng, 4000), np.zeros((7000, 3), np.float32)])
+    typ = np.concatenate([np.zeros(4000, np.uint8), np.ones(7000, np.uint8)])
+    A = np.array([[-40.0, A_SL], [A_SL, -40.0]], np.float32)
+    B = np.full((2, 2), 25.0, np.float32)
+    return dict(name="slit_wetting", params=default_params(box, **pover), pos=pos, vel=vel, type=typ,
+                pair_A=A, pair_B=B, frozen_mask=0b10)
+
+
 def quantise_positions(pos, box, bits=7):
     """Round coordinates to multiples of 2^-bits (and keep them inside the box): with boxes <= 16,
     every r^2 is then exact in fp32 and fp64 alike."""

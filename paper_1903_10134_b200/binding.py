@@ -22,7 +22,7 @@ _ERRNAME = {-1: "MDPD_EINVAL", -2: "MDPD_ENOMEM", -3: "MDPD_ECUDA", -4: "MDPD_EO
             -6: "MDPD_ENAN", -7: "MDPD_EINSOLID"}
 
 # every symbol include/mdpd.h declares
-SYMBOLS = ("mdpd_create", "mdpd_destroy", "mdpd_set_params", "mdpd_workspace_bytes", "mdpd_set_workspace",
+SYMBOLS = ("mdpd_create", "mdpd_destroy", "mdpd_set_params", "mdpd_set_pair_params", "mdpd_workspace_bytes", "mdpd_set_workspace",
            "mdpd_load_particles", "mdpd_load_wall_mask", "mdpd_step", "mdpd_get_state", "mdpd_set_step_counter",
            "mdpd_set_forces",
            "mdpd_compute_forces", "mdpd_get_pairs", "mdpd_rng_fill", "mdpd_get_counters", "mdpd_last_error",
@@ -72,6 +72,7 @@ def lib():
         L.mdpd_create.argtypes = [C.POINTER(vp), i32, vp]
         L.mdpd_destroy.argtypes = [vp]
         L.mdpd_set_params.argtypes = [vp, pp]
+        L.mdpd_set_pair_params.argtypes = [vp, u32, vp, vp, u32]
         L.mdpd_workspace_bytes.argtypes = [pp, u64, i32, vp]
         L.mdpd_workspace_bytes.restype = C.c_size_t
         L.mdpd_set_workspace.argtypes = [vp, vp, C.c_size_t]
@@ -174,6 +175,19 @@ class Simulation:
         self.params.update(changes)
         self._p = make_params(self.params)
         self._ck(self._L.mdpd_set_params(self._h, C.byref(self._p)), "mdpd_set_params")
+
+    def set_pair_params(self, A, B, frozen_mask=0):
+        """mdpd_set_pair_params: per-type-pair A_ij, B_ij ([nt][nt], symmetric) and the frozen species (bit s)."""
+        if A is None:
+            self._ck(self._L.mdpd_set_pair_params(self._h, 0, None, None, 0), "mdpd_set_pair_params")
+            return
+        A = np.ascontiguousarray(A, np.float32)
+        B = np.ascontiguousarray(B, np.float32)
+        nt = A.shape[0]
+        if A.shape != (nt, nt) or B.shape != (nt, nt):
+            raise ValueError("A, B must be [nt][nt]")
+        self._ck(self._L.mdpd_set_pair_params(self._h, nt, A.ctypes.data, B.ctypes.data, int(frozen_mask)),
+                 "mdpd_set_pair_params")
 
     def workspace_bytes(self, n, mask_dims=None):
         md = None if mask_dims is None else (C.c_uint32 * 3)(*[int(x) for x in mask_dims])

@@ -26,6 +26,9 @@ namespace {
 constexpr unsigned ERR_OVERFLOW = 1u;
 constexpr unsigned ERR_NAN = 2u;
 constexpr unsigned ERR_TILE = 4u;  // a tile + halo does not fit the shared-memory capacity
+constexpr unsigned ERR_TYPE = 8u;  // a particle's species index is not below the number of species
+// particle word (pos.w): tag (load-order index) | species << 28 | frozen << 31
+constexpr unsigned TAG_BITS = 28, TAG_MASK = (1u << TAG_BITS) - 1u, MAXTYPES = 8;
 constexpr int TPB = 128;           // threads per block of the per-particle kernels
 constexpr int SCAN_TPB = 256;      // scan: 256 threads x 8 items
 constexpr int SCAN_ITEMS = 8;
@@ -95,6 +98,9 @@ struct DevP {  // passed by value to every kernel
   float A, B, gamma, sig_c;  // sig_c = sigma * sqrt(3) * 2^-23 / sqrt(dt)
   float dt, hdt_m;           // dt, 0.5 dt / m
   float fgx, fgy, fgz;       // m g
+  unsigned ntypes;           // 0: one material (type byte != 0 <=> frozen); else the type byte is a species index
+  unsigned frozen_mask;      // bit s: species s is frozen
+  float2 AB[MAXTYPES * MAXTYPES];  // per-type-pair (A, B) of Eq. (1), row = species_i * MAXTYPES (Tables 1-2)
   float thr2;                // (skin / 2)^2
   unsigned seed;
 };
@@ -169,7 +175,19 @@ __global__ void k_pack(DevP p, const float* __restrict__ pos, const float* __res
                        const unsigned char* __restrict__ type, unsigned buf) {
   unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= p.N) return;
-  unsigned t = type ? (type[i] != 0) : 0u;
+  unsigned t = 0u, sp = 0u;  // frozen flag, species
+  if (type) {
+    if (p.ntypes) {
+      sp = type[i];
+      if (sp >= p.ntypes) {
+        atomicOr(&p.ctl->err, ERR_TYPE);
+        sp = 0u;
+      }
+      t = (p.frozen_mask >> sp) & 1u;
+    } else {
+      t = sp = type[i] != 0;
+    }
+  }
   float x = pos[3 * i], y = pos[3 * i + 1], z = pos[3 * i + 2];
   // general wrap at load time (inputs may be anywhere): x - L floor(x / L), result == L -> 0   (R12)
   x -= p.Lx * floorf(x / p.Lx);
@@ -182,7 +200,7 @@ __global__ void k_pack(DevP p, const float* __restrict__ pos, const float* __res
   if (y < 0.0f) y = 0.0f;
   if (z < 0.0f) z = 0.0f;
   if (t) atomicOr(&p.ctl->has_wall, 1u);
-  p.pos[buf][i] = make_float4(x, y, z, u2f(i | (t << 31)));
+  p.pos[buf][i] = make_float4(x, y, z, u2f(i | (sp << TAG_BITS) | (t << 31)));
   float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
   if (!t) {
     v.x = vel[3 * i];
@@ -193,12 +211,13 @@ __global__ void k_pack(DevP p, const float* __restrict__ pos, const float* __res
   p.force[i] = make_float4(0.f, 0.f, 0.f, 0.f);
 }
 
-// (re)start the control block for a fresh sort of buffer 0 into buffer 1; keeps has_wall
+// (re)start the control block for a fresh sort of buffer 0 into buffer 1; keeps has_wall and a bad-species fault
 __global__ void k_ctl_init(DevP p) {
   Ctl* c = p.ctl;
-  const unsigned hw = c->has_wall;
+  const unsigned hw = c->has_wall, et = c->err & ERR_TYPE;  // k_pack's findings survive the restart
   Ctl z;
   memset(&z, 0, sizeof z);
+  z.err = et;
   z.cur = 1;
   z.rebuild = 1;
   z.rebuilds = 1;
@@ -212,7 +231,7 @@ __global__ void k_unpack(DevP p, float* __restrict__ pos, float* __restrict__ ve
   if (i >= p.N) return;
   const unsigned cur = p.ctl->cur;
   float4 x = p.pos[cur][i], v = p.vel[cur][i], f = p.force[i];
-  unsigned tag = f2u(x.w) & 0x7FFFFFFFu;
+  unsigned tag = f2u(x.w) & TAG_MASK;
   if (pos) { pos[3 * tag] = wrap1(x.x, p.Lx); pos[3 * tag + 1] = wrap1(x.y, p.Ly); pos[3 * tag + 2] = wrap1(x.z, p.Lz); }
   if (vel) { vel[3 * tag] = v.x; vel[3 * tag + 1] = v.y; vel[3 * tag + 2] = v.z; }
   if (force) { force[3 * tag] = f.x; force[3 * tag + 1] = f.y; force[3 * tag + 2] = f.z; }
@@ -222,7 +241,7 @@ __global__ void k_unpack(DevP p, float* __restrict__ pos, float* __restrict__ ve
 __global__ void k_set_forces(DevP p, const float* __restrict__ force) {  // tag order -> sorted order
   unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= p.N) return;
-  const unsigned tag = f2u(p.pos[p.ctl->cur][i].w) & 0x7FFFFFFFu;
+  const unsigned tag = f2u(p.pos[p.ctl->cur][i].w) & TAG_MASK;
   p.force[i] = make_float4(force[3 * tag], force[3 * tag + 1], force[3 * tag + 2], 0.0f);
 }
 
@@ -464,10 +483,10 @@ __global__ void __launch_bounds__(TPB) k_permute(const DevP p) {
   x.x = wrap1(x.x, p.Lx);
   x.y = wrap1(x.y, p.Ly);
   x.z = wrap1(x.z, p.Lz);
-  const unsigned tag = f2u(x.w) & 0x7FFFFFFFu;
+  const unsigned tag = f2u(x.w) & TAG_MASK;
   unsigned rank = 0;
   for (unsigned t = cs; t < ce; ++t) {
-    unsigned ot = f2u(p.pos[src][p.order[t]].w) & 0x7FFFFFFFu;
+    unsigned ot = f2u(p.pos[src][p.order[t]].w) & TAG_MASK;
     rank += (ot < tag) ? 1u : 0u;
   }
   const unsigned dst = cs + rank;
@@ -1198,9 +1217,11 @@ struct ForceAcc {
   float x, y, z;
 };
 
+// MULTI: per-type-pair (A, B) from the table `ab` in shared memory (row = species of i), else the handle's A, B
+template <bool MULTI>
 __device__ __forceinline__ void force_entry(const DevP& p, const unsigned pbase, const unsigned vbase, const float4 xi,
                                             const float4 vi, const unsigned tagi, const unsigned j, const HashKeys& K,
-                                            ForceAcc& acc) {
+                                            const float2* ab, ForceAcc& acc) {
   const float4 xj = lds4(pbase + (j << 4));
   const float4 vj = lds4(vbase + (j << 4));
   const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
@@ -1208,12 +1229,18 @@ __device__ __forceinline__ void force_entry(const DevP& p, const unsigned pbase,
   const float rinv = rsqrt_fast(r2);
   const float r = r2 * rinv;
   const float w = __saturatef(fmaf(-r, p.inv_rc, 1.0f));  // > 0 for in-range entries, 0 for the sentinel
-  float F = p.A * w;
+  float Aij = p.A, Bij = p.B;
+  if (MULTI) {  // the species sits in bits 28..30 of the particle word (A_SL, B_SL)
+    const float2 t = ab[(f2u(xj.w) >> TAG_BITS) & (MAXTYPES - 1u)];
+    Aij = t.x;
+    Bij = t.y;
+  }
+  float F = Aij * w;
   const float wd = __saturatef(fmaf(-r, p.inv_rd, 1.0f));
-  F += p.B * (vi.w + vj.w) * wd;
+  F += Bij * (vi.w + vj.w) * wd;
   const float ev = (dx * (vi.x - vj.x) + dy * (vi.y - vj.y) + dz * (vi.z - vj.z)) * rinv;
   F -= p.gamma * w * w * ev;
-  const unsigned h = pair_hash(tagi, f2u(xj.w) & 0x7FFFFFFFu, K);
+  const unsigned h = pair_hash(tagi, f2u(xj.w) & TAG_MASK, K);
   const float xi_s = (float)((int)(h >> 8) - (1 << 23));  // exact
   F += p.sig_c * w * xi_s;
   const float Fr = F * rinv;
@@ -1222,9 +1249,13 @@ __device__ __forceinline__ void force_entry(const DevP& p, const unsigned pbase,
   acc.z += Fr * dz;
 }
 
-template <bool ALL>  // ALL: also evaluate the (never used) forces on frozen particles, for parity checks
+template <bool ALL, bool MULTI>  // ALL: also evaluate the (never used) forces on frozen particles, for parity checks
 __global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
   extern __shared__ __align__(16) unsigned char smraw[];
+  __shared__ float2 s_ab[MULTI ? MAXTYPES * MAXTYPES : 1];
+  if (MULTI) {
+    for (unsigned q = threadIdx.x; q < MAXTYPES * MAXTYPES; q += blockDim.x) s_ab[q] = p.AB[q];  // ordered by stage_fast's barriers
+  }
   const TileSmem sm = carve_smem(smraw, p.tile_cap, true);
   const unsigned cur = p.ctl->cur;
   const TileInfo T = p.tiles[blockIdx.x];
@@ -1274,7 +1305,8 @@ __global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
     const unsigned li = rec.x >> 16;
     const float4 xi = sm.spos[li];
     const unsigned wi = f2u(xi.w);
-    const unsigned tagi = wi & 0x7FFFFFFFu;
+    const unsigned tagi = wi & TAG_MASK;
+    const float2* const ab = s_ab + (MULTI ? ((wi >> TAG_BITS) & (MAXTYPES - 1u)) * MAXTYPES : 0u);
     const float4 vi = sm.svel[li];
     const unsigned na = rec.y;
     ForceAcc acc = {0.f, 0.f, 0.f};
@@ -1282,15 +1314,15 @@ __global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
     for (unsigned k0 = 0; k0 < na; k0 += 8) {
       const uint4 e = nxt;
       if (k0 + 8 < na) nxt = lst[(size_t)((k0 >> 3) + 1) * p.N];  // next chunk in flight
-      force_entry(p, pbase, vbase, xi, vi, tagi, e.x & 0xFFFFu, K, acc);
-      force_entry(p, pbase, vbase, xi, vi, tagi, e.x >> 16, K, acc);
-      force_entry(p, pbase, vbase, xi, vi, tagi, e.y & 0xFFFFu, K, acc);
-      force_entry(p, pbase, vbase, xi, vi, tagi, e.y >> 16, K, acc);
+      force_entry<MULTI>(p, pbase, vbase, xi, vi, tagi, e.x & 0xFFFFu, K, ab, acc);
+      force_entry<MULTI>(p, pbase, vbase, xi, vi, tagi, e.x >> 16, K, ab, acc);
+      force_entry<MULTI>(p, pbase, vbase, xi, vi, tagi, e.y & 0xFFFFu, K, ab, acc);
+      force_entry<MULTI>(p, pbase, vbase, xi, vi, tagi, e.y >> 16, K, ab, acc);
       if (k0 + 4 < na) {  // the second half of the chunk holds at least one entry
-        force_entry(p, pbase, vbase, xi, vi, tagi, e.z & 0xFFFFu, K, acc);
-        force_entry(p, pbase, vbase, xi, vi, tagi, e.z >> 16, K, acc);
-        force_entry(p, pbase, vbase, xi, vi, tagi, e.w & 0xFFFFu, K, acc);
-        force_entry(p, pbase, vbase, xi, vi, tagi, e.w >> 16, K, acc);
+        force_entry<MULTI>(p, pbase, vbase, xi, vi, tagi, e.z & 0xFFFFu, K, ab, acc);
+        force_entry<MULTI>(p, pbase, vbase, xi, vi, tagi, e.z >> 16, K, ab, acc);
+        force_entry<MULTI>(p, pbase, vbase, xi, vi, tagi, e.w & 0xFFFFu, K, ab, acc);
+        force_entry<MULTI>(p, pbase, vbase, xi, vi, tagi, e.w >> 16, K, ab, acc);
       }
     }
     if (!(wi >> 31)) {
@@ -1324,7 +1356,7 @@ __global__ void __launch_bounds__(512) k_pairs(const DevP p, float rcut2, uint2*
   const unsigned os = p.cell_start[T.rank0], oe = p.cell_start[T.rank0 + T.ncell_own];
   for (unsigned i = os + threadIdx.x; i < oe; i += blockDim.x) {
     const float4 xi = sm.spos[p.self_loc[i]];
-    const unsigned tagi = f2u(xi.w) & 0x7FFFFFFFu;
+    const unsigned tagi = f2u(xi.w) & TAG_MASK;
     const unsigned n = p.nnbr[i];
     {
       const uint4* lst = p.nbr + i;
@@ -1332,7 +1364,7 @@ __global__ void __launch_bounds__(512) k_pairs(const DevP p, float rcut2, uint2*
         const uint4 e = lst[(size_t)(k >> 3) * p.N];
         const unsigned w = (k & 4) ? ((k & 2) ? e.w : e.z) : ((k & 2) ? e.y : e.x);
         const float4 xj = sm.spos[(k & 1) ? (w >> 16) : (w & 0xFFFFu)];
-        const unsigned tagj = f2u(xj.w) & 0x7FFFFFFFu;
+        const unsigned tagj = f2u(xj.w) & TAG_MASK;
         if (tagi >= tagj) continue;
         const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
         const float r2 = dx * dx + dy * dy + dz * dz;
@@ -1406,7 +1438,7 @@ bool make_layout(const mdpd_params& p, uint64_t n, int has_mask, const uint32_t*
   if (!(p.dt > 0) || !(p.mass > 0)) return fail("dt and mass must be > 0");
   if (p.s != 1.0f) return fail("only s = 1 is implemented (DESIGN.md R15)");
   if (p.reorder_every > 1) return fail("only reorder_every = 0/1 is implemented (DESIGN.md R16)");
-  if (n >= (1ull << 31)) return fail("n must be < 2^31");
+  if (n >= (1ull << TAG_BITS)) return fail("n must be < 2^28");
   L.rlist = p.rc + p.skin;
   int nc[3];
   for (int d = 0; d < 3; ++d) {
@@ -1481,6 +1513,8 @@ struct mdpd_ctx {
   size_t mask_cap = 0;  // bytes reserved for the mask in the workspace
   bool has_mask = false;
   bool has_wall = false;  // some particle is frozen (type 1)
+  unsigned ntypes = 0, frozen_mask = 0;        // mdpd_set_pair_params
+  float pairA[MAXTYPES * MAXTYPES] = {}, pairB[MAXTYPES * MAXTYPES] = {};
   uint64_t launches = 0;         // kernels launched directly (graph replays are added from graph_steps / ctl)
   uint64_t host_step = 0;
   cudaStream_t ls = nullptr;     // stream the LAUNCH macro targets (the handle's stream, or the capture stream)
@@ -1617,6 +1651,13 @@ void fill_physics(mdpd_ctx* h) {
   d.fgx = p.mass * p.g[0]; d.fgy = p.mass * p.g[1]; d.fgz = p.mass * p.g[2];
   d.thr2 = 0.25f * p.skin * p.skin;
   d.seed = p.seed;
+  d.ntypes = h->ntypes;
+  d.frozen_mask = h->frozen_mask;
+  for (unsigned a = 0; a < MAXTYPES; ++a)
+    for (unsigned b = 0; b < MAXTYPES; ++b) {
+      const bool in = a < h->ntypes && b < h->ntypes;
+      d.AB[a * MAXTYPES + b] = make_float2(in ? h->pairA[a * h->ntypes + b] : p.A, in ? h->pairB[a * h->ntypes + b] : p.B);
+    }
 }
 
 // Sort order of the cells: tiles of tdim[0] x tdim[1] x tdim[2] cells enumerated along the Z-curve (Morton order of
@@ -1677,8 +1718,13 @@ int launch_forces(mdpd_ctx* h, bool all) {
   if (!h->has_wall) LAUNCH(h, PS_DENSITY, (k_density<false, false><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
   else if (all) LAUNCH(h, PS_DENSITY, (k_density<true, true><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
   else LAUNCH(h, PS_DENSITY, (k_density<true, false><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
-  if (all) LAUNCH(h, PS_FORCE, (k_force<true><<<d.ntiles, h->block, h->smem_posvel, h->ls>>>(d)));
-  else LAUNCH(h, PS_FORCE, (k_force<false><<<d.ntiles, h->block, h->smem_posvel, h->ls>>>(d)));
+  if (d.ntypes) {  // per-type-pair parameters
+    if (all) LAUNCH(h, PS_FORCE, (k_force<true, true><<<d.ntiles, h->block, h->smem_posvel, h->ls>>>(d)));
+    else LAUNCH(h, PS_FORCE, (k_force<false, true><<<d.ntiles, h->block, h->smem_posvel, h->ls>>>(d)));
+  } else {
+    if (all) LAUNCH(h, PS_FORCE, (k_force<true, false><<<d.ntiles, h->block, h->smem_posvel, h->ls>>>(d)));
+    else LAUNCH(h, PS_FORCE, (k_force<false, false><<<d.ntiles, h->block, h->smem_posvel, h->ls>>>(d)));
+  }
   return MDPD_OK;
 }
 
@@ -1760,6 +1806,8 @@ int sync_and_check(mdpd_ctx* h) {
   CU_TRY(h, cudaMemcpyAsync(h->h_ctl, h->d.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, h->stream));
   CU_TRY(h, cudaStreamSynchronize(h->stream));
   CU_TRY(h, cudaGetLastError());
+  if (h->h_ctl->err & ERR_TYPE)
+    return set_err(h, MDPD_EINVAL, "a particle's type is not below the number of species given to mdpd_set_pair_params");
   if (h->h_ctl->err & ERR_NAN)
     return set_err(h, MDPD_ENAN, "non-finite coordinates appeared (%llu events)", h->h_ctl->nan_events);
   if (h->h_ctl->err & ERR_TILE)
@@ -1849,6 +1897,31 @@ int mdpd_set_params(mdpd_ctx* h, const mdpd_params* p) {
   }
   h->prm = *p;
   h->have_params = true;
+  return MDPD_OK;
+}
+
+int mdpd_set_pair_params(mdpd_ctx* h, uint32_t ntypes, const float* A, const float* B, uint32_t frozen_mask) {
+  if (!h) return MDPD_EINVAL;
+  if (ntypes > MAXTYPES) return set_err(h, MDPD_EINVAL, "at most %u species", MAXTYPES);
+  if (ntypes && (!A || !B)) return set_err(h, MDPD_EINVAL, "A / B are NULL");
+  for (uint32_t a = 0; a < ntypes; ++a)
+    for (uint32_t b = 0; b < a; ++b)
+      if (A[a * ntypes + b] != A[b * ntypes + a] || B[a * ntypes + b] != B[b * ntypes + a])
+        return set_err(h, MDPD_EINVAL, "A and B must be symmetric");
+  if (h->loaded && (ntypes != h->ntypes || frozen_mask != h->frozen_mask))
+    return set_err(h, MDPD_ESTATE, "the number of species and the frozen set are fixed by load_particles");
+  h->ntypes = ntypes;
+  h->frozen_mask = frozen_mask;
+  for (uint32_t q = 0; q < ntypes * ntypes; ++q) {
+    h->pairA[q] = A[q];
+    h->pairB[q] = B[q];
+  }
+  if (h->loaded) {  // new values between steps: like mdpd_set_params
+    CU_TRY(h, cudaSetDevice(h->device));
+    if (h->pending_B) finalize_kick(h);
+    fill_physics(h);
+    h->graph_dirty = true;
+  }
   return MDPD_OK;
 }
 
@@ -1995,8 +2068,10 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
   CU_TRY(h, cudaFuncSetAttribute(k_density<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
   CU_TRY(h, cudaFuncSetAttribute(k_density<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
   CU_TRY(h, cudaFuncSetAttribute(k_pairs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
-  CU_TRY(h, cudaFuncSetAttribute(k_force<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
-  CU_TRY(h, cudaFuncSetAttribute(k_force<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
+  CU_TRY(h, cudaFuncSetAttribute(k_force<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
+  CU_TRY(h, cudaFuncSetAttribute(k_force<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
+  CU_TRY(h, cudaFuncSetAttribute(k_force<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
+  CU_TRY(h, cudaFuncSetAttribute(k_force<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
   if (n) {
     LAUNCH(h, PS_BUILD_LIST, (k_build_list<<<h->d.ntiles, h->block_build, h->smem_build, h->stream>>>(h->d)));
     launch_forces(h, true);
