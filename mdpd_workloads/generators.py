@@ -218,7 +218,9 @@ def make_species_mixture(box=(12.0, 10.0, 9.0), nspecies=5, frozen_mask=0b01010,
 def make_slit_wetting(A_SL=-30.0, seed=BASE_SEED + 6, **pover):
     """Section 4.2's slit pore shifted into [0, L): box 60 x 10 x 5, 3 500 solid particles (species 1,
     frozen) uniformly random in each of the wall regions 0 <= y < 1 and 9 <= y < 10, 4 000 liquid particles (species 0)
-    in a block 20 <= x < 40, 1 < y < 9; A_SS = A_LL = -40, the unlike pair A_SL from Table 1, B = 25 (R19)."""
+    in a block 20 <= x < 40, 1 < y < 9; A_SS = A_LL = -40, the unlike pair A_SL from Table 1, B = 25 (R19); the
+    wall regions are also solid voxels of a 0.5-voxel mask (the bounce-back wall of BASELINE.json in place of the paper's
+    anti-penetration model, R7)."""
     box = (60.0, 10.0, 5.0)
     rng = np.random.default_rng(seed)
     def block(n, lo, hi):
@@ -232,8 +234,12 @@ def make_slit_wetting(A_SL=-30.0, seed=BASE_SEED + 6, **pover):
     typ = np.concatenate([np.zeros(4000, np.uint8), np.ones(7000, np.uint8)])
     A = np.array([[-40.0, A_SL], [A_SL, -40.0]], np.float32)
     B = np.full((2, 2), 25.0, np.float32)
+    voxel = 0.5
+    mask = np.zeros((10, 20, 120), np.uint8)   # [nz][ny][nx]: the wall regions are solid voxels (no-slip bounce-back)
+    mask[:, :2, :] = 1
+    mask[:, 18:, :] = 1
     return dict(name="slit_wetting", params=default_params(box, **pover), pos=pos, vel=vel, type=typ,
-                pair_A=A, pair_B=B, frozen_mask=0b10)
+                pair_A=A, pair_B=B, frozen_mask=0b10, mask=mask, voxel=voxel)
 
 
 def quantise_positions(pos, box, bits=7):

@@ -46,7 +46,10 @@ def test_pair_params_density_force_parity(gpu, maker):
     c = maker()
     s = gpu.Simulation(c["params"])
     s.set_pair_params(c["pair_A"], c["pair_B"], c["frozen_mask"])
-    s.load_particles(c["pos"], c["vel"], c["type"])
+    md = None if c.get("mask") is None else c["mask"].shape[::-1]
+    s.load_particles(c["pos"], c["vel"], c["type"], mask_dims=md)
+    if md is not None:
+        s.load_wall_mask(c["mask"], c["voxel"])
     check(s.get_state(), oracle_for(c, c["pos"], c["vel"], 0).get_state(), "load")
     frozen = ((c["frozen_mask"] >> c["type"]) & 1).astype(bool)
     s.step(15)
@@ -103,3 +106,29 @@ def test_bad_pair_params_are_rejected(gpu):
     s.set_pair_params(c["pair_A"][:3, :3], c["pair_B"][:3, :3], 0)
     with pytest.raises(gpu.MdpdError):
         s.load_particles(c["pos"], c["vel"], c["type"])                     # species 3, 4 of 3
+
+
+def test_slit_pore_wetting_follows_A_SL(gpu):
+    """Section 4.2 / Figure 6: the liquid in the slit goes from wetting to non-wetting as the
+    solid-liquid attraction A_SL weakens from -35 to -20 (Table 1).  Observable: the liquid's contact with the walls,
+    i.e. the number of liquid particles within 1 rc of a wall face, and its extent along the walls, after 4000 steps."""
+    res = {}
+    for A_SL in (-35.0, -20.0):
+        c = wl.make_slit_wetting(A_SL)
+        s = gpu.Simulation(c["params"])
+        s.set_pair_params(c["pair_A"], c["pair_B"], c["frozen_mask"])
+        s.load_particles(c["pos"], c["vel"], c["type"], mask_dims=c["mask"].shape[::-1])
+        s.load_wall_mask(c["mask"], c["voxel"])
+        s.step(4000)
+        st = s.get_state()
+        liq = st["pos"][c["type"] == 0]
+        assert np.isfinite(liq).all() and s.counters()["faults"] == 0
+        assert (liq[:, 1] >= 1.0).all() and (liq[:, 1] < 9.0).all()         # the walls hold the liquid
+        near = int(((liq[:, 1] < 2.0) | (liq[:, 1] > 8.0)).sum())
+        x = liq[:, 0]
+        # extent along x of the liquid next to the walls (circular spread around the block's centre x = 30)
+        xw = x[(liq[:, 1] < 2.0) | (liq[:, 1] > 8.0)]
+        spread = float(np.sqrt(np.mean((xw - 30.0) ** 2))) if len(xw) else 0.0
+        res[A_SL] = (near, spread)
+    assert res[-35.0][0] > 1.15 * res[-20.0][0], res          # more liquid at the walls when they attract it more
+    assert res[-35.0][1] > res[-20.0][1], res                 # and it spreads further along them
