@@ -2015,7 +2015,10 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
     h->block = TILE_TPB;  // upper bound while the capacity is probed; set from the tile population below
     h->block_build = vol >= 64 ? BUILD_TPB : (vol >= 32 ? std::min(256, BUILD_TPB) : 128u);
     const size_t fixed = tile_smem_bytes(0, true, 0);
-    const unsigned cap_limit = (unsigned)std::min<size_t>((h->smem_limit - fixed) / TILE_SLOT_BYTES, 65535);
+    // capacity of a tile + halo in staged slots: what the force pass can hold in shared memory, what a 16-bit list entry can
+    // address, and what the item list of stage_fast (2 * HTAB items: 3 * 36 runs + one item per 32 slots) can describe
+    const unsigned cap_limit = (unsigned)std::min<size_t>(std::min<size_t>((h->smem_limit - fixed) / TILE_SLOT_BYTES, 65535),
+                                                          (size_t)(2 * HTAB - 3 * 36) * 32);
     h->d.tile_cap = cap_limit;
     LAUNCH(h, PS_OTHER, (k_ctl_init<<<1, 1, 0, h->stream>>>(h->d)));  // the initial sort reads buffer 0 and writes buffer 1
     CU_TRY(h, cudaMemcpyAsync(h->d.cell_rank, rank.data(), rank.size() * 4, cudaMemcpyHostToDevice, h->stream));
