@@ -89,8 +89,9 @@ size_t mdpd_workspace_bytes(const mdpd_params* p, uint64_t n, int has_mask, cons
  * and mdpd_destroy frees that allocation. */
 int mdpd_set_workspace(mdpd_ctx* h, void* dev_ptr, size_t bytes);
 
-/* Load n particles.  pos, vel: [n][3] float32, host or device.  type: [n] uint8 (0 = fluid, 1 = frozen wall) or NULL
- * (all fluid).  The tag of a particle is its index in this call and is permanent.  Positions are wrapped into the box;
+/* Load n < 2^28 particles.  pos, vel: [n][3] float32, host or device.  type: [n] uint8 (0 = fluid, any other value =
+ * frozen wall; after mdpd_set_pair_params: the species index) or NULL (all fluid / species 0).  The tag of a particle is
+ * its index in this call and is permanent.  Positions are wrapped into the box;
  * frozen particles get v = 0.  Builds the cell list / neighbour list and evaluates rho and f at step index 0.
  * n = 0 is allowed.  Synchronises the stream. */
 int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* vel, const uint8_t* type);

@@ -4,7 +4,7 @@
 // (x -> rho -> f -> v): PAPER.md L125-133; body force: L186; frozen walls: L162.  Readings R1..R18 and the hash
 // specification: DESIGN.md sections 3 and 4.  This file shares nothing with oracle/ (the fp64 CPU oracle).
 //
-// Device state: pos float4 = (x, y, z, bits(tag | type << 31)), vel float4 = (vx, vy, vz, rho),
+// Device state: pos float4 = (x, y, z, bits(tag | species << 28 | frozen << 31)), vel float4 = (vx, vy, vz, rho),
 // both double-buffered for the counting sort into tiles of cells (tiles along the Z-curve, cells x-fastest inside a
 // tile); force float4; xbuild float4 (positions at the last list build); Verlet list of 16-bit indices into the
 // tile's staged shared-memory image, stored in 16-byte chunks of 8 entries, layout [chunk][particle]; per tile a
@@ -525,7 +525,7 @@ constexpr unsigned MSTRIDE = 17;                // words per particle slot of th
 constexpr unsigned BUILD_SCRATCH16 = (32 * MSTRIDE * 4 + 2 * MAXCAND * 2) / 2;  // per-warp scratch of the list build, in 16-bit units
 
 struct TileSmem {
-  float4* spos;      // [cap + 1] (x_rel, y_rel, z_rel, bits(tag | type << 31)); slot cap = the far-away sentinel
+  float4* spos;      // [cap + 1] (x_rel, y_rel, z_rel, particle word); slot cap = the far-away sentinel
   float4* svel;      // [cap + 1] (vx, vy, vz, rho)            (force pass only)
   float4* hshift;    // [HTAB] (sx, sy, sz, bits(delta)) of halo cell h: x_rel = x + s, global index = staged slot + delta
   unsigned* hbase;   // [HTAB] first staged slot of halo cell h; hbase[nh] = number of staged particles
