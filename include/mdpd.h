@@ -53,6 +53,9 @@ typedef struct {
   float g[3];             /* body acceleration on fluid particles         */
   float skin;             /* Verlet-list skin (default 0.25); list radius = rc + skin; rebuild when the largest
                              displacement since the last build exceeds skin/2                   DESIGN.md R3, R4      */
+  float headroom;         /* capacity of a tile of cells (shared memory) = headroom x the fullest tile of the loaded
+                             state; 0 = default 1.15.  Raise it when the density will grow locally during the run (a
+                             contracting slab, a filling pore): outgrowing the capacity is MDPD_EOVERFLOW              */
   uint32_t seed;          /* seed of the pair hash      */
   uint32_t max_neigh;     /* list capacity per particle, <= 128; 0 = automatic                                       */
   uint32_t reorder_every; /* Morton reorder every N list rebuilds; only 0/1 (= every rebuild) is implemented (R16)    */

@@ -20,6 +20,7 @@ from .generators import (  # noqa: F401
     make_poiseuille,
     make_pore_network,
     make_species_mixture,
+    make_liquid_vacuum,
     make_slit_wetting,
     make_config,
     quantise_positions,

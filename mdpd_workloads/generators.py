@@ -196,6 +196,30 @@ def make_pore_network(nvox=128, voxel=0.5, corr=6.0, porosity=0.35, density=6.0,
                 pos=pos, vel=vel, type=typ, mask=mask, voxel=float(voxel))
 
 
+def make_liquid_vacuum(L=100.0, Lyz=None, half_width=10.0, A=-50.0, gamma=12.4, seed=BASE_SEED + 7, **pover):
+    """Section 4.1's liquid-vacuum interface: periodic box L x Lyz x Lyz, particles on an fcc lattice of
+    spacing rc in the slab |x - L/2| <= half_width (the paper's box [-50, 50]^3 shifted by +50: 820 000 particles for
+    L = Lyz = 100, half_width = 10), A = -50, B = 25, rd = 0.75, gamma = 12.4 (sigma^2 = 2 gamma kT), Maxwell velocities
+    at kT = 1."""
+    Lyz = L if Lyz is None else float(Lyz)
+    box = (float(L), Lyz, Lyz)
+    rng = np.random.default_rng(seed)
+    nx = int(round(2 * half_width + 0.5)) + 1                 # whole cells 0 .. 2 hw, the last one contributes half a cell
+    ny = int(round(Lyz))
+    ii, jj, kk = np.meshgrid(np.arange(nx), np.arange(ny), np.arange(ny), indexing="ij")
+    cells = np.stack([ii.ravel(), jj.ravel(), kk.ravel()], 1).astype(np.float32)
+    basis = np.array([[0, 0, 0], [0.5, 0.5, 0], [0.5, 0, 0.5], [0, 0.5, 0.5]], np.float32)
+    sites = (cells[:, None, :] + basis[None, :, :]).reshape(-1, 3)
+    sites = sites[sites[:, 0] < 2 * half_width + 0.5]          # x in [0, 20.5): 41 half-layers, 4 * ny^2 * 20.5 sites
+    pos = sites + np.array([L / 2 - half_width, 0.25, 0.25], np.float32)
+    pos = _clip_into_box(pos.astype(np.float32), box)
+    n = len(pos)
+    vel = maxwell_velocities(rng, n)
+    sigma = float(np.sqrt(2.0 * gamma * 1.0))
+    return dict(name="liquid_vacuum", params=default_params(box, A=A, gamma=gamma, sigma=sigma, **pover),
+                pos=pos, vel=vel, type=np.zeros(n, np.uint8))
+
+
 def make_species_mixture(box=(12.0, 10.0, 9.0), nspecies=5, frozen_mask=0b01010, density=6.0, seed=BASE_SEED + 5, **pover):
     """A liquid of `nspecies` material types drawn uniformly (type byte = species index), the species of `frozen_mask`
     frozen, with random symmetric pair matrices A_ij in [-40, -20], B_ij in [22, 28]: stands in for the five material

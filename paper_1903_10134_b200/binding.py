@@ -41,6 +41,7 @@ class mdpd_params(C.Structure):
     _fields_ = [("box", C.c_float * 3), ("rc", C.c_float), ("rd", C.c_float), ("A", C.c_float), ("B", C.c_float),
                 ("gamma", C.c_float), ("sigma", C.c_float), ("kT", C.c_float), ("s", C.c_float),
                 ("mass", C.c_float), ("dt", C.c_float), ("g", C.c_float * 3), ("skin", C.c_float),
+                ("headroom", C.c_float),
                 ("seed", C.c_uint32), ("max_neigh", C.c_uint32), ("reorder_every", C.c_uint32),
                 ("flags", C.c_uint32)]
 
@@ -51,6 +52,7 @@ def make_params(d: dict) -> mdpd_params:
     for k in ("rc", "rd", "A", "B", "gamma", "sigma", "kT", "s", "mass", "dt", "skin"):
         setattr(p, k, float(d[k]))
     p.g[:] = [float(b) for b in d["g"]]
+    p.headroom = float(d.get("headroom", 0.0))
     for k in ("seed", "max_neigh", "reorder_every", "flags"):
         setattr(p, k, int(d.get(k, 0)) & 0xFFFFFFFF)
     return p

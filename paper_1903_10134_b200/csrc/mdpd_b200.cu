@@ -1884,7 +1884,7 @@ int mdpd_set_params(mdpd_ctx* h, const mdpd_params* p) {
   if (h->loaded) {
     const mdpd_params& q = h->prm;
     if (memcmp(q.box, p->box, sizeof q.box) || q.rc != p->rc || q.rd != p->rd || q.skin != p->skin ||
-        q.max_neigh != p->max_neigh || q.mass != p->mass)
+        q.max_neigh != p->max_neigh || q.mass != p->mass || q.headroom != p->headroom)
       return set_err(h, MDPD_ESTATE, "box, cut-offs, skin, mass and capacities are frozen after load_particles");
     if (h->pending_B) {  // the outstanding half kick belongs to the old parameters
       CU_TRY(h, cudaSetDevice(h->device));
@@ -2030,10 +2030,11 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
     CU_TRY(h, cudaStreamSynchronize(h->stream));  // rank, tiles are locals
     h->has_wall = h->h_ctl->has_wall != 0;
     const unsigned max_halo = h->h_ctl->max_halo;
-    if (max_halo > cap_limit) {
+    const double headroom = h->prm.headroom > 0.0f ? std::max(1.0, (double)h->prm.headroom) : 1.15;  // mdpd_params.headroom
+    if ((double)max_halo * headroom > (double)cap_limit) {
       if (force_tile || ci + 1 == ncand)
-        return set_err(h, MDPD_EOVERFLOW, "a tile of %d x %d x %d cells plus halo holds %u particles; shared memory fits %u",
-                       tdim[0], tdim[1], tdim[2], max_halo, cap_limit);
+        return set_err(h, MDPD_EOVERFLOW, "a tile of %d x %d x %d cells plus halo holds %u particles (x head-room %.2f); shared memory fits %u",
+                       tdim[0], tdim[1], tdim[2], max_halo, headroom, cap_limit);
       continue;  // try the next smaller tile shape
     }
     // density / force passes: one thread per own particle of the fullest tile (a tile with more loops)
@@ -2051,9 +2052,9 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
     }
     // head-room for density fluctuations between rebuilds of a long run
     {
-      // at least 15 % over the fullest tile of the initial state; beyond that, all the shared memory that does not
+      // at least `headroom` (default 15 %) over the fullest tile of the initial state; beyond that, all the shared memory that does not
       // cost a resident CTA of the force pass (the tightest: it stages positions and velocities)
-      const unsigned want = std::min<unsigned>(cap_limit, ((unsigned)(max_halo * 1.15) + 64 + 63) / 64 * 64);
+      const unsigned want = std::min<unsigned>(cap_limit, ((unsigned)(max_halo * headroom) + 64 + 63) / 64 * 64);
       const size_t sm_total = h->smem_limit + 1024;  // per-SM shared memory; 1 KB is reserved per resident CTA
       const size_t per_cta = tile_smem_bytes(want, true, 0) + 1024;
       const size_t ctas = std::max<size_t>(1, sm_total / per_cta);

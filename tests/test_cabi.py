@@ -36,8 +36,8 @@ def test_every_declared_symbol_is_exported(pk):
 
 
 def test_params_struct_matches_header(pk):
-    """17 float + 4 uint32 fields in the header's order = 84 bytes, no padding."""
-    assert C.sizeof(pk.mdpd_params) == 21 * 4
+    """18 float + 4 uint32 fields in the header's order = 88 bytes, no padding."""
+    assert C.sizeof(pk.mdpd_params) == 22 * 4
     src = open(os.path.join(ROOT, "include", "mdpd.h")).read()
     body = re.search(r"typedef struct \{(.*?)\} mdpd_params;", src, flags=re.S).group(1)
     body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)

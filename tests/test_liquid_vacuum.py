@@ -1,0 +1,66 @@
+"""Section 4.1 of the paper: liquid-vacuum interface, A = -50, B = 25, rd = 0.75 rc, gamma = 12.4, fcc
+start in |x| <= 10 rc, 5 000 steps to equilibrate, 5 000 steps of averaging, density profile in 2 rc bins along x.
+The paper PRINTS the density at the centre of the slab: 6.88 ("for both USER-MESO 2.5 and our CPU code, matching the
+value reported in Ghoufi and Malfreyt").  The oracle is pinned to it on a reduced slab (CPU), the CUDA path reproduces
+the paper's full-size run (100^3 box, 820 000 particles).  Both give 6.81-6.82, 1 % below the printed value, inside the
+1.5 % tolerance used here (R20); the closed-form EOS of PAPER.md L89 puts the zero-pressure density at 6.85."""
+import numpy as np
+import pytest
+
+import mdpd_workloads as wl
+
+PAPER_CENTRE_DENSITY = 6.88
+TOL = 0.015
+
+
+def test_workload_is_the_papers():
+    c = wl.make_liquid_vacuum()
+    assert len(c["pos"]) == 820_000
+    assert c["params"]["A"] == -50.0 and c["params"]["B"] == 25.0 and c["params"]["rd"] == 0.75
+    assert abs(c["params"]["sigma"] ** 2 - 2 * 12.4 * 1.0) < 1e-9     # sigma^2 = 2 gamma kT
+    x = c["pos"][:, 0]
+    assert x.min() == 40.0 and x.max() == 60.0                        # |x - 50| <= 10
+
+
+def test_oracle_slab_centre_density_matches_the_paper():
+    """Reduced slab (24 x 7 x 7 box, 2 450 particles): the bulk density of the slab is intensive."""
+    from oracle.mdpd_ref import RefSim
+    c = wl.make_liquid_vacuum(L=24.0, Lyz=7.0, half_width=6.0)
+    s = RefSim(c["params"])
+    s.load_particles(c["pos"].astype(np.float64), c["vel"].astype(np.float64), c["type"])
+    s.step(2000)
+    dens = []
+    for _ in range(40):
+        s.step(50)
+        x = s.get_state()["pos"][:, 0]
+        dens.append((np.abs(x - x.mean()) < 1.5).sum() / (3.0 * 7.0 * 7.0))
+    rho = float(np.mean(dens))
+    assert abs(rho / PAPER_CENTRE_DENSITY - 1.0) < TOL, rho
+    assert abs(rho - 6.82) < 0.05, rho          # what this oracle gives (6.817 +- 0.007 over 50 samples): regression guard
+
+
+@pytest.mark.gpu
+def test_gpu_full_size_run_reproduces_the_papers_centre_density():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("the -m gpu suite needs a CUDA device (no CPU fallback exists)")
+    import paper_1903_10134_b200 as pk
+    pk.build()
+    c = wl.make_liquid_vacuum()
+    c["params"]["headroom"] = 2.0               # the fcc start (density 4) contracts to a liquid of density 6.9
+    sim = pk.Simulation(c["params"])
+    sim.load_particles(c["pos"], c["vel"], c["type"])
+    sim.step(5000)                              # equilibration
+    hist = np.zeros(50)
+    nsamp = 0
+    for _ in range(50):                         # 5 000 steps of averaging, one sample per 100 steps
+        sim.step(100)
+        x = sim.get_state(vel=False, force=False, rho=False)["pos"][:, 0]
+        hist += np.histogram(x, bins=50, range=(0.0, 100.0))[0]     # 2 rc bins along x
+        nsamp += 1
+    assert sim.counters()["faults"] == 0
+    prof = hist / nsamp / (2.0 * 100.0 * 100.0)
+    centre = float(prof[24:26].mean())          # the two bins around x = 50 (the paper's x = 0)
+    assert abs(centre / PAPER_CENTRE_DENSITY - 1.0) < TOL, (centre, prof[18:32])
+    assert prof[:18].sum() == 0.0 and prof[32:].sum() == 0.0        # vacuum outside the slab
+    assert abs(prof[23:27] - centre).max() < 0.02                   # flat plateau
