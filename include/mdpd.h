@@ -128,6 +128,12 @@ int mdpd_set_forces(mdpd_ctx* h, const float* force);
 /* rho and f (on every particle, frozen ones included) from the current x, v at the current step index. */
 int mdpd_compute_forces(mdpd_ctx* h);
 
+/* mdpd_compute_forces, and in the same pass the configurational (conservative-force) part of the stress:
+ * out = sum over interacting pairs of r_ij,a F^C_ij,b for ab = xx, yy, zz, xy, xz, yz (F^C of Eq. (1), PAPER.md L77-81;
+ * frozen-frozen pairs excluded as in the force).  With the kinetic part sum m v_a v_b from mdpd_get_state this gives the
+ * pressure tensor, and for a slab normal to x the interfacial tension of section 4.1. */
+int mdpd_compute_virial(mdpd_ctx* h, double out[6]);
+
 /* All tag pairs (a < b) with r < rcut, found through the Verlet list with the kernels' own fp32 predicate
  * (r^2 < rcut^2); rcut <= rc + skin.  For rcut > rc the result is complete only right after a list build
  * (load_particles, or any step that rebuilt).  *count receives the number found; up to cap pairs are written

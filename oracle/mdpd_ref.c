@@ -74,6 +74,7 @@ typedef struct mdpd_ref_ctx {
   uint64_t bounces;   /* cumulative bounce-back events */
   uint64_t npairs_rc; /* pairs with r < rc at the last force evaluation */
   double virial_c;    /* sum over pairs of r_ij . F^C_ij at the last force evaluation */
+  double vir_t[6];    /* its tensor: sum over pairs of r_ij,a F^C_ij,b for ab = xx, yy, zz, xy, xz, yz (symmetric) */
   /* scratch for the cell list */
   int64_t *cell_head, *next;
   uint64_t cell_cap;
@@ -304,6 +305,14 @@ static void force_pair(mdpd_ref_ctx *h, uint64_t i, uint64_t j, const double d[3
     h->fpair[3 * j + k] -= F * e[k];
   }
   h->virial_c += FC * r;
+  /* configurational part of the stress (conservative forces): r_a F_b = FC d_a d_b / r; the interfacial tension of
+   * section 4.1 is L_x < s_xx - (s_yy + s_zz) / 2 > */
+  h->vir_t[0] += FC * d[0] * d[0] / r;
+  h->vir_t[1] += FC * d[1] * d[1] / r;
+  h->vir_t[2] += FC * d[2] * d[2] / r;
+  h->vir_t[3] += FC * d[0] * d[1] / r;
+  h->vir_t[4] += FC * d[0] * d[2] / r;
+  h->vir_t[5] += FC * d[1] * d[2] / r;
 }
 
 int mdpd_ref_compute_forces(mdpd_ref_ctx *h) {
@@ -315,6 +324,7 @@ int mdpd_ref_compute_forces(mdpd_ref_ctx *h) {
   for (uint64_t i = 0; i < 3 * n; ++i) h->fpair[i] = 0.0;
   h->npairs_rc = 0;
   h->virial_c = 0.0;
+  for (int k = 0; k < 6; ++k) h->vir_t[k] = 0.0;
   if ((rcode = for_each_pair(h, h->p.rc, force_pair, NULL)) != REF_OK) return rcode;
   for (uint64_t i = 0; i < n; ++i)
     for (int k = 0; k < 3; ++k)
@@ -452,6 +462,13 @@ int mdpd_ref_get_pair_force(mdpd_ref_ctx *h, double *fpair) {
 }
 
 /* out[0] steps, [1] bounces, [2] pairs r<rc at last evaluation; out_f[0] = sum r_ij F^C_ij */
+/* sum over interacting pairs of r_ij,a F^C_ij,b at the last force evaluation: xx, yy, zz, xy, xz, yz */
+int mdpd_ref_get_virial(mdpd_ref_ctx *h, double out[6]) {
+  if (!h || !out) return REF_EINVAL;
+  for (int k = 0; k < 6; ++k) out[k] = h->vir_t[k];
+  return REF_OK;
+}
+
 int mdpd_ref_get_counters(mdpd_ref_ctx *h, uint64_t out[4], double out_f[2]) {
   if (!h) return REF_EINVAL;
   if (out) { out[0] = h->step; out[1] = h->bounces; out[2] = h->npairs_rc; out[3] = h->n; }

@@ -61,6 +61,7 @@ def lib():
         L.mdpd_ref_get_state.argtypes = [vp, vp, vp, vp, vp, vp]
         L.mdpd_ref_get_pair_force.argtypes = [vp, vp]
         L.mdpd_ref_get_counters.argtypes = [vp, vp, vp]
+        L.mdpd_ref_get_virial.argtypes = [vp, vp]
         L.mdpd_ref_get_pairs.argtypes = [vp, C.c_double, vp, vp, u64]
         _lib = L
     return _lib
@@ -172,6 +173,12 @@ class RefSim:
         f = np.empty((self.n, 3))
         _check(self._L.mdpd_ref_get_pair_force(self._h, f.ctypes.data), "get_pair_force")
         return f
+
+    def virial(self):
+        """sum over interacting pairs of r_a F^C_b at the last force evaluation: [xx, yy, zz, xy, xz, yz]."""
+        out = np.zeros(6, np.float64)
+        _check(self._L.mdpd_ref_get_virial(self._h, out.ctypes.data), "get_virial")
+        return out
 
     def counters(self):
         out = np.zeros(4, np.uint64); outf = np.zeros(2)

@@ -25,7 +25,7 @@ _ERRNAME = {-1: "MDPD_EINVAL", -2: "MDPD_ENOMEM", -3: "MDPD_ECUDA", -4: "MDPD_EO
 SYMBOLS = ("mdpd_create", "mdpd_destroy", "mdpd_set_params", "mdpd_set_pair_params", "mdpd_workspace_bytes", "mdpd_set_workspace",
            "mdpd_load_particles", "mdpd_load_wall_mask", "mdpd_step", "mdpd_get_state", "mdpd_set_step_counter",
            "mdpd_set_forces",
-           "mdpd_compute_forces", "mdpd_get_pairs", "mdpd_rng_fill", "mdpd_get_counters", "mdpd_last_error",
+           "mdpd_compute_forces", "mdpd_compute_virial", "mdpd_get_pairs", "mdpd_rng_fill", "mdpd_get_counters", "mdpd_last_error",
            "mdpd_profile_begin", "mdpd_profile_end", "mdpd_profile_name", "mdpd_probe_issue_rates")
 MDPD_PROF_SLOTS = 16
 
@@ -85,6 +85,7 @@ def lib():
         L.mdpd_set_step_counter.argtypes = [vp, u64]
         L.mdpd_set_forces.argtypes = [vp, vp]
         L.mdpd_compute_forces.argtypes = [vp]
+        L.mdpd_compute_virial.argtypes = [vp, vp]
         L.mdpd_get_pairs.argtypes = [vp, f32, vp, vp, u64]
         L.mdpd_rng_fill.argtypes = [vp, u64, vp, u32, vp]
         L.mdpd_get_counters.argtypes = [vp, vp]
@@ -231,6 +232,12 @@ class Simulation:
 
     def compute_forces(self):
         self._ck(self._L.mdpd_compute_forces(self._h), "mdpd_compute_forces")
+
+    def compute_virial(self):
+        """mdpd_compute_virial: [xx, yy, zz, xy, xz, yz] of sum over pairs r_a F^C_b (also refreshes rho and f)."""
+        out = np.zeros(6, np.float64)
+        self._ck(self._L.mdpd_compute_virial(self._h, out.ctypes.data), "mdpd_compute_virial")
+        return out
 
     def set_step_counter(self, k):
         self._ck(self._L.mdpd_set_step_counter(self._h, int(k)), "mdpd_set_step_counter")

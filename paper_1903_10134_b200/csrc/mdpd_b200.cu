@@ -48,6 +48,7 @@ struct Ctl {
   unsigned max_own;   // most particles in a tile at the last build
   unsigned has_wall;  // some particle is frozen (set by k_pack)
   unsigned long long steps, rebuilds, bounces, sum_nbr, overflow, nan_events, sum_act, dens_passes, graph_rebuilds, pad2;
+  double vir[6];             // k_force<.., VIRIAL>: sum over list entries of r_a F^C_b (xx, yy, zz, xy, xz, yz); each pair twice
   unsigned long long ph[4];  // -DMDPD_PHASES: clock cycles of k_force's staging / sort / pair loop, summed over CTAs, and the CTA count
 };
 
@@ -1218,10 +1219,11 @@ struct ForceAcc {
 };
 
 // MULTI: per-type-pair (A, B) from the table `ab` in shared memory (row = species of i), else the handle's A, B
-template <bool MULTI>
+// VIRIAL: also accumulate r_a F^C_b of the pair (conservative part of the stress, section 4.1 of the paper) into vir[6]
+template <bool MULTI, bool VIRIAL>
 __device__ __forceinline__ void force_entry(const DevP& p, const unsigned pbase, const unsigned vbase, const float4 xi,
                                             const float4 vi, const unsigned tagi, const unsigned j, const HashKeys& K,
-                                            const float2* ab, ForceAcc& acc) {
+                                            const float2* ab, ForceAcc& acc, float* vir) {
   const float4 xj = lds4(pbase + (j << 4));
   const float4 vj = lds4(vbase + (j << 4));
   const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
@@ -1238,6 +1240,15 @@ __device__ __forceinline__ void force_entry(const DevP& p, const unsigned pbase,
   float F = Aij * w;
   const float wd = __saturatef(fmaf(-r, p.inv_rd, 1.0f));
   F += Bij * (vi.w + vj.w) * wd;
+  if (VIRIAL) {  // F is the conservative force here; the sentinel contributes 0 * finite
+    const float c = F * rinv;
+    vir[0] += c * dx * dx;
+    vir[1] += c * dy * dy;
+    vir[2] += c * dz * dz;
+    vir[3] += c * dx * dy;
+    vir[4] += c * dx * dz;
+    vir[5] += c * dy * dz;
+  }
   const float ev = (dx * (vi.x - vj.x) + dy * (vi.y - vj.y) + dz * (vi.z - vj.z)) * rinv;
   F -= p.gamma * w * w * ev;
   const unsigned h = pair_hash(tagi, f2u(xj.w) & TAG_MASK, K);
@@ -1249,7 +1260,7 @@ __device__ __forceinline__ void force_entry(const DevP& p, const unsigned pbase,
   acc.z += Fr * dz;
 }
 
-template <bool ALL, bool MULTI>  // ALL: also evaluate the (never used) forces on frozen particles, for parity checks
+template <bool ALL, bool MULTI, bool VIRIAL = false>  // ALL: also evaluate the (never used) forces on frozen particles, for parity checks
 __global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
   extern __shared__ __align__(16) unsigned char smraw[];
   __shared__ float2 s_ab[MULTI ? MAXTYPES * MAXTYPES : 1];
@@ -1287,6 +1298,7 @@ __global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
 #pragma unroll
   for (int q = 0; q < 6; ++q) K.k[q] = pin(K.k[q]);
   const unsigned pbase = smem_addr(sm.spos), vbase = smem_addr(sm.svel);
+  double vsum[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
   for (unsigned r = 0; r * W < ngroups; ++r) {
     const unsigned g = group_of_round(r, warp, W);
     const unsigned t = g * 32u + lane;
@@ -1310,19 +1322,20 @@ __global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
     const float4 vi = sm.svel[li];
     const unsigned na = rec.y;
     ForceAcc acc = {0.f, 0.f, 0.f};
+    float vir[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
     const uint4* __restrict__ lst = p.act + i;
     for (unsigned k0 = 0; k0 < na; k0 += 8) {
       const uint4 e = nxt;
       if (k0 + 8 < na) nxt = lst[(size_t)((k0 >> 3) + 1) * p.N];  // next chunk in flight
-      force_entry<MULTI>(p, pbase, vbase, xi, vi, tagi, e.x & 0xFFFFu, K, ab, acc);
-      force_entry<MULTI>(p, pbase, vbase, xi, vi, tagi, e.x >> 16, K, ab, acc);
-      force_entry<MULTI>(p, pbase, vbase, xi, vi, tagi, e.y & 0xFFFFu, K, ab, acc);
-      force_entry<MULTI>(p, pbase, vbase, xi, vi, tagi, e.y >> 16, K, ab, acc);
+      force_entry<MULTI, VIRIAL>(p, pbase, vbase, xi, vi, tagi, e.x & 0xFFFFu, K, ab, acc, vir);
+      force_entry<MULTI, VIRIAL>(p, pbase, vbase, xi, vi, tagi, e.x >> 16, K, ab, acc, vir);
+      force_entry<MULTI, VIRIAL>(p, pbase, vbase, xi, vi, tagi, e.y & 0xFFFFu, K, ab, acc, vir);
+      force_entry<MULTI, VIRIAL>(p, pbase, vbase, xi, vi, tagi, e.y >> 16, K, ab, acc, vir);
       if (k0 + 4 < na) {  // the second half of the chunk holds at least one entry
-        force_entry<MULTI>(p, pbase, vbase, xi, vi, tagi, e.z & 0xFFFFu, K, ab, acc);
-        force_entry<MULTI>(p, pbase, vbase, xi, vi, tagi, e.z >> 16, K, ab, acc);
-        force_entry<MULTI>(p, pbase, vbase, xi, vi, tagi, e.w & 0xFFFFu, K, ab, acc);
-        force_entry<MULTI>(p, pbase, vbase, xi, vi, tagi, e.w >> 16, K, ab, acc);
+        force_entry<MULTI, VIRIAL>(p, pbase, vbase, xi, vi, tagi, e.z & 0xFFFFu, K, ab, acc, vir);
+        force_entry<MULTI, VIRIAL>(p, pbase, vbase, xi, vi, tagi, e.z >> 16, K, ab, acc, vir);
+        force_entry<MULTI, VIRIAL>(p, pbase, vbase, xi, vi, tagi, e.w & 0xFFFFu, K, ab, acc, vir);
+        force_entry<MULTI, VIRIAL>(p, pbase, vbase, xi, vi, tagi, e.w >> 16, K, ab, acc, vir);
       }
     }
     if (!(wi >> 31)) {
@@ -1331,6 +1344,19 @@ __global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
       acc.z += p.fgz;
     }
     p.force[i] = make_float4(acc.x, acc.y, acc.z, 0.0f);
+    if (VIRIAL) {
+#pragma unroll
+      for (int q = 0; q < 6; ++q) vsum[q] += (double)vir[q];
+    }
+  }
+  if (VIRIAL) {  // all lanes of the warp arrive here (the round loop has no early return)
+#pragma unroll
+    for (int q = 0; q < 6; ++q) {
+      double v = vsum[q];
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+      if (lane == 0 && v != 0.0) atomicAdd(&p.ctl->vir[q], v);
+    }
   }
 #ifdef MDPD_PHASES
   __syncthreads();
@@ -1713,12 +1739,15 @@ int launch_rebuild_chain(mdpd_ctx* h, bool with_list = true) {
   return MDPD_OK;
 }
 
-int launch_forces(mdpd_ctx* h, bool all) {
+int launch_forces(mdpd_ctx* h, bool all, bool virial = false) {
   const DevP& d = h->d;
   if (!h->has_wall) LAUNCH(h, PS_DENSITY, (k_density<false, false><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
   else if (all) LAUNCH(h, PS_DENSITY, (k_density<true, true><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
   else LAUNCH(h, PS_DENSITY, (k_density<true, false><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
-  if (d.ntypes) {  // per-type-pair parameters
+  if (virial) {  // mdpd_compute_virial: forces on every particle + the conservative virial tensor
+    if (d.ntypes) LAUNCH(h, PS_FORCE, (k_force<true, true, true><<<d.ntiles, h->block, h->smem_posvel, h->ls>>>(d)));
+    else LAUNCH(h, PS_FORCE, (k_force<true, false, true><<<d.ntiles, h->block, h->smem_posvel, h->ls>>>(d)));
+  } else if (d.ntypes) {  // per-type-pair parameters
     if (all) LAUNCH(h, PS_FORCE, (k_force<true, true><<<d.ntiles, h->block, h->smem_posvel, h->ls>>>(d)));
     else LAUNCH(h, PS_FORCE, (k_force<false, true><<<d.ntiles, h->block, h->smem_posvel, h->ls>>>(d)));
   } else {
@@ -2075,6 +2104,8 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
   CU_TRY(h, cudaFuncSetAttribute(k_force<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
   CU_TRY(h, cudaFuncSetAttribute(k_force<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
   CU_TRY(h, cudaFuncSetAttribute(k_force<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
+  CU_TRY(h, (cudaFuncSetAttribute(k_force<true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel)));
+  CU_TRY(h, (cudaFuncSetAttribute(k_force<true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel)));
   CU_TRY(h, cudaFuncSetAttribute(k_force<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
   if (n) {
     LAUNCH(h, PS_BUILD_LIST, (k_build_list<<<h->d.ntiles, h->block_build, h->smem_build, h->stream>>>(h->d)));
@@ -2152,6 +2183,20 @@ int mdpd_compute_forces(mdpd_ctx* h) {
   finalize_kick(h);
   launch_forces(h, true);
   return sync_and_check(h);
+}
+
+int mdpd_compute_virial(mdpd_ctx* h, double out[6]) {
+  if (!h || !out) return MDPD_EINVAL;
+  if (!h->loaded) return set_err(h, MDPD_ESTATE, "load_particles first");
+  for (int k = 0; k < 6; ++k) out[k] = 0.0;
+  if (h->n == 0) return MDPD_OK;
+  CU_TRY(h, cudaSetDevice(h->device));
+  finalize_kick(h);
+  CU_TRY(h, cudaMemsetAsync(h->d.ctl->vir, 0, sizeof(double) * 6, h->stream));
+  launch_forces(h, true, true);
+  int rc = sync_and_check(h);
+  for (int k = 0; k < 6; ++k) out[k] = 0.5 * h->h_ctl->vir[k];  // the full list visits every pair from both ends
+  return rc;
 }
 
 int mdpd_set_step_counter(mdpd_ctx* h, uint64_t step) {
