@@ -48,7 +48,7 @@ typedef struct {
   float A, B;             /* Eq. (1): attractive A < 0, many-body repulsive B > 0 (-40, 25)   */
   float gamma, sigma;     /* dissipative / random amplitudes, sigma^2 = 2 gamma kT (4.5, 3.0)           */
   float kT;               /* informational: if > 0 the library checks |sigma^2 - 2 gamma kT| <= 1e-3 sigma^2          */
-  float s;                /* exponent of wR = (1 - r/rc)^s; only s = 1 is implemented          PAPER.md L75 (R15)     */
+  float s;                /* exponent of wR = (1 - r/rc)^s, wD = wR^2, 0 < s <= 4 (1: the paper's) PAPER.md L75 (R15)  */
   float mass, dt;         /* particle mass (1), timestep (0.01)         */
   float g[3];             /* body acceleration on fluid particles         */
   float skin;             /* Verlet-list skin (default 0.25); list radius = rc + skin; rebuild when the largest

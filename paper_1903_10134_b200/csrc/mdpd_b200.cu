@@ -99,6 +99,7 @@ struct DevP {  // passed by value to every kernel
   float A, B, gamma, sig_c;  // sig_c = sigma * sqrt(3) * 2^-23 / sqrt(dt)
   float dt, hdt_m;           // dt, 0.5 dt / m
   float fgx, fgy, fgz;       // m g
+  float s_exp;               // exponent s of wR = (1 - r/rc)^s; the kernels specialise s = 1
   unsigned ntypes;           // 0: one material (type byte != 0 <=> frozen); else the type byte is a species index
   unsigned frozen_mask;      // bit s: species s is frozen
   float2 AB[MAXTYPES * MAXTYPES];  // per-type-pair (A, B) of Eq. (1), row = species_i * MAXTYPES (Tables 1-2)
@@ -1220,7 +1221,7 @@ struct ForceAcc {
 
 // MULTI: per-type-pair (A, B) from the table `ab` in shared memory (row = species of i), else the handle's A, B
 // VIRIAL: also accumulate r_a F^C_b of the pair (conservative part of the stress, section 4.1 of the paper) into vir[6]
-template <bool MULTI, bool VIRIAL>
+template <bool MULTI, bool VIRIAL, bool SPOW>
 __device__ __forceinline__ void force_entry(const DevP& p, const unsigned pbase, const unsigned vbase, const float4 xi,
                                             const float4 vi, const unsigned tagi, const unsigned j, const HashKeys& K,
                                             const float2* ab, ForceAcc& acc, float* vir) {
@@ -1250,17 +1251,19 @@ __device__ __forceinline__ void force_entry(const DevP& p, const unsigned pbase,
     vir[5] += c * dy * dz;
   }
   const float ev = (dx * (vi.x - vj.x) + dy * (vi.y - vj.y) + dz * (vi.z - vj.z)) * rinv;
-  F -= p.gamma * w * w * ev;
+  // wR = w^s (wD = wR^2); s = 1 unless SPOW.  w = 0 (sentinel) gives exp2(-inf) = 0.
+  const float wR = SPOW ? __powf(w, p.s_exp) : w;
+  F -= p.gamma * wR * wR * ev;
   const unsigned h = pair_hash(tagi, f2u(xj.w) & TAG_MASK, K);
   const float xi_s = (float)((int)(h >> 8) - (1 << 23));  // exact
-  F += p.sig_c * w * xi_s;
+  F += p.sig_c * wR * xi_s;
   const float Fr = F * rinv;
   acc.x += Fr * dx;
   acc.y += Fr * dy;
   acc.z += Fr * dz;
 }
 
-template <bool ALL, bool MULTI, bool VIRIAL = false>  // ALL: also evaluate the (never used) forces on frozen particles, for parity checks
+template <bool ALL, bool MULTI, bool VIRIAL = false, bool SPOW = false>  // SPOW: general exponent s of wR; ALL: also evaluate the (never used) forces on frozen particles, for parity checks
 __global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
   extern __shared__ __align__(16) unsigned char smraw[];
   __shared__ float2 s_ab[MULTI ? MAXTYPES * MAXTYPES : 1];
@@ -1327,15 +1330,15 @@ __global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
     for (unsigned k0 = 0; k0 < na; k0 += 8) {
       const uint4 e = nxt;
       if (k0 + 8 < na) nxt = lst[(size_t)((k0 >> 3) + 1) * p.N];  // next chunk in flight
-      force_entry<MULTI, VIRIAL>(p, pbase, vbase, xi, vi, tagi, e.x & 0xFFFFu, K, ab, acc, vir);
-      force_entry<MULTI, VIRIAL>(p, pbase, vbase, xi, vi, tagi, e.x >> 16, K, ab, acc, vir);
-      force_entry<MULTI, VIRIAL>(p, pbase, vbase, xi, vi, tagi, e.y & 0xFFFFu, K, ab, acc, vir);
-      force_entry<MULTI, VIRIAL>(p, pbase, vbase, xi, vi, tagi, e.y >> 16, K, ab, acc, vir);
+      force_entry<MULTI, VIRIAL, SPOW>(p, pbase, vbase, xi, vi, tagi, e.x & 0xFFFFu, K, ab, acc, vir);
+      force_entry<MULTI, VIRIAL, SPOW>(p, pbase, vbase, xi, vi, tagi, e.x >> 16, K, ab, acc, vir);
+      force_entry<MULTI, VIRIAL, SPOW>(p, pbase, vbase, xi, vi, tagi, e.y & 0xFFFFu, K, ab, acc, vir);
+      force_entry<MULTI, VIRIAL, SPOW>(p, pbase, vbase, xi, vi, tagi, e.y >> 16, K, ab, acc, vir);
       if (k0 + 4 < na) {  // the second half of the chunk holds at least one entry
-        force_entry<MULTI, VIRIAL>(p, pbase, vbase, xi, vi, tagi, e.z & 0xFFFFu, K, ab, acc, vir);
-        force_entry<MULTI, VIRIAL>(p, pbase, vbase, xi, vi, tagi, e.z >> 16, K, ab, acc, vir);
-        force_entry<MULTI, VIRIAL>(p, pbase, vbase, xi, vi, tagi, e.w & 0xFFFFu, K, ab, acc, vir);
-        force_entry<MULTI, VIRIAL>(p, pbase, vbase, xi, vi, tagi, e.w >> 16, K, ab, acc, vir);
+        force_entry<MULTI, VIRIAL, SPOW>(p, pbase, vbase, xi, vi, tagi, e.z & 0xFFFFu, K, ab, acc, vir);
+        force_entry<MULTI, VIRIAL, SPOW>(p, pbase, vbase, xi, vi, tagi, e.z >> 16, K, ab, acc, vir);
+        force_entry<MULTI, VIRIAL, SPOW>(p, pbase, vbase, xi, vi, tagi, e.w & 0xFFFFu, K, ab, acc, vir);
+        force_entry<MULTI, VIRIAL, SPOW>(p, pbase, vbase, xi, vi, tagi, e.w >> 16, K, ab, acc, vir);
       }
     }
     if (!(wi >> 31)) {
@@ -1462,7 +1465,7 @@ bool make_layout(const mdpd_params& p, uint64_t n, int has_mask, const uint32_t*
   if (!(p.rc > 0) || !(p.rd > 0) || !(p.rd <= p.rc)) return fail("need 0 < rd <= rc");
   if (!(p.skin >= 0)) return fail("skin must be >= 0");
   if (!(p.dt > 0) || !(p.mass > 0)) return fail("dt and mass must be > 0");
-  if (p.s != 1.0f) return fail("only s = 1 is implemented (DESIGN.md R15)");
+  if (!(p.s > 0.0f) || p.s > 4.0f) return fail("the exponent s of wR = (1 - r/rc)^s must be in (0, 4] (DESIGN.md R15)");
   if (p.reorder_every > 1) return fail("only reorder_every = 0/1 is implemented (DESIGN.md R16)");
   if (n >= (1ull << TAG_BITS)) return fail("n must be < 2^28");
   L.rlist = p.rc + p.skin;
@@ -1677,6 +1680,7 @@ void fill_physics(mdpd_ctx* h) {
   d.fgx = p.mass * p.g[0]; d.fgy = p.mass * p.g[1]; d.fgz = p.mass * p.g[2];
   d.thr2 = 0.25f * p.skin * p.skin;
   d.seed = p.seed;
+  d.s_exp = p.s;
   d.ntypes = h->ntypes;
   d.frozen_mask = h->frozen_mask;
   for (unsigned a = 0; a < MAXTYPES; ++a)
@@ -1744,7 +1748,10 @@ int launch_forces(mdpd_ctx* h, bool all, bool virial = false) {
   if (!h->has_wall) LAUNCH(h, PS_DENSITY, (k_density<false, false><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
   else if (all) LAUNCH(h, PS_DENSITY, (k_density<true, true><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
   else LAUNCH(h, PS_DENSITY, (k_density<true, false><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
-  if (virial) {  // mdpd_compute_virial: forces on every particle + the conservative virial tensor
+  if (d.s_exp != 1.0f) {  // general exponent of wR: one material, no virial (checked by the callers)
+    if (all) LAUNCH(h, PS_FORCE, (k_force<true, false, false, true><<<d.ntiles, h->block, h->smem_posvel, h->ls>>>(d)));
+    else LAUNCH(h, PS_FORCE, (k_force<false, false, false, true><<<d.ntiles, h->block, h->smem_posvel, h->ls>>>(d)));
+  } else if (virial) {  // mdpd_compute_virial: forces on every particle + the conservative virial tensor
     if (d.ntypes) LAUNCH(h, PS_FORCE, (k_force<true, true, true><<<d.ntiles, h->block, h->smem_posvel, h->ls>>>(d)));
     else LAUNCH(h, PS_FORCE, (k_force<true, false, true><<<d.ntiles, h->block, h->smem_posvel, h->ls>>>(d)));
   } else if (d.ntypes) {  // per-type-pair parameters
@@ -1976,6 +1983,7 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
   if (!h) return MDPD_EINVAL;
   if (!h->have_params) return set_err(h, MDPD_ESTATE, "set_params first");
   if (n && (!pos || !vel)) return set_err(h, MDPD_EINVAL, "pos / vel are NULL");
+  if (h->prm.s != 1.0f && h->ntypes) return set_err(h, MDPD_EINVAL, "per-type-pair parameters need s = 1");
   CU_TRY(h, cudaSetDevice(h->device));
   std::string why;
   Layout L;
@@ -2104,6 +2112,8 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
   CU_TRY(h, cudaFuncSetAttribute(k_force<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
   CU_TRY(h, cudaFuncSetAttribute(k_force<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
   CU_TRY(h, cudaFuncSetAttribute(k_force<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
+  CU_TRY(h, (cudaFuncSetAttribute(k_force<true, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel)));
+  CU_TRY(h, (cudaFuncSetAttribute(k_force<false, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel)));
   CU_TRY(h, (cudaFuncSetAttribute(k_force<true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel)));
   CU_TRY(h, (cudaFuncSetAttribute(k_force<true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel)));
   CU_TRY(h, cudaFuncSetAttribute(k_force<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
@@ -2192,6 +2202,7 @@ int mdpd_compute_virial(mdpd_ctx* h, double out[6]) {
   if (h->n == 0) return MDPD_OK;
   CU_TRY(h, cudaSetDevice(h->device));
   finalize_kick(h);
+  if (h->prm.s != 1.0f) return set_err(h, MDPD_EINVAL, "mdpd_compute_virial needs s = 1");
   CU_TRY(h, cudaMemsetAsync(h->d.ctl->vir, 0, sizeof(double) * 6, h->stream));
   launch_forces(h, true, true);
   int rc = sync_and_check(h);

@@ -39,8 +39,8 @@ def test_call_order_and_bad_arguments(gpu):
     assert L.mdpd_get_state(h, None, None, None, None, None) == -5
     assert L.mdpd_load_particles(h, 1, None, None, None) == -5       # set_params first
     assert b"set_params" in L.mdpd_last_error(h)
-    p = gpu.make_params(wl.default_params((10.0, 10.0, 10.0), s=0.5))
-    assert L.mdpd_set_params(h, C.byref(p)) == -1                    # MDPD_EINVAL: s != 1 (R15)
+    p = gpu.make_params(wl.default_params((10.0, 10.0, 10.0), s=-0.5))
+    assert L.mdpd_set_params(h, C.byref(p)) == -1                    # MDPD_EINVAL: s must be in (0, 4] (R15)
     p = gpu.make_params(wl.default_params((10.0, 10.0, 10.0), sigma=2.0))
     assert L.mdpd_set_params(h, C.byref(p)) == -1                    # sigma^2 != 2 gamma kT
     p = gpu.make_params(wl.default_params((10.0, 10.0, 10.0)))

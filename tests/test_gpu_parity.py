@@ -260,3 +260,40 @@ def test_verlet_list_stays_valid_over_rebuilds(gpu):
     assert rebuilds[-1] > 3, rebuilds            # the trigger fired several times in 36 steps
     assert rebuilds[-1] < 36, rebuilds           # ... but not every step
     g.close()
+
+
+@pytest.mark.parametrize("s_exp", [0.5, 0.25, 2.0])
+def test_density_force_parity_general_exponent_s(gpu, s_exp):
+    """wR = (1 - r/rc)^s, wD = wR^2 with s != 1 (R15): rho and F against the oracle at load and after stepping."""
+    from oracle.mdpd_ref import RefSim
+    c = wl.make_config(0, s=s_exp)
+    g = gpu.Simulation(c["params"])
+    g.load_particles(c["pos"], c["vel"], c["type"])
+    r = RefSim(c["params"])
+    r.load_particles(c["pos"].astype(np.float64), c["vel"].astype(np.float64), c["type"])
+
+    # For s < 1/2 the random force sigma w^s xi / sqrt(dt) is ill-conditioned at the cut-off in ANY fp32 evaluation:
+    # d(w^s) = s w^(s-1) dw with dw ~ 1e-7 from r itself, so the few pairs with w ~ 1e-5 carry errors ~1e-3 of the RMS
+    # force.  The maximum norm is therefore relaxed to 2e-3 for s = 1/4 and the RMS error to 5e-5 (DESIGN.md R15).
+    tol_max, tol_rms = (TOL, 1e-5) if s_exp >= 0.5 else (2e-3, 5e-5)
+
+    def check(a, b, what):
+        f_rms = np.sqrt(np.mean((b["force"] ** 2).sum(1)))
+        err = np.sqrt(((a["force"] - b["force"]) ** 2).sum(1))
+        e_rho = np.abs(a["rho"] - b["rho"]).max() / np.sqrt(np.mean(b["rho"] ** 2))
+        assert err.max() / f_rms <= tol_max and np.sqrt(np.mean(err ** 2)) / f_rms <= tol_rms and e_rho <= TOL, \
+            (what, s_exp, err.max() / f_rms, np.sqrt(np.mean(err ** 2)) / f_rms, e_rho)
+
+    check(g.get_state(), r.get_state(), "load")
+    # the exponent really enters: the s = 1 forces of the same state differ
+    g1 = gpu.Simulation(dict(c["params"], s=1.0))
+    g1.load_particles(c["pos"], c["vel"], c["type"])
+    assert np.abs(g1.get_state()["force"] - g.get_state()["force"]).max() > 1.0
+    g.step(12)
+    st = g.get_state()
+    g.compute_forces()
+    r2 = RefSim(c["params"])
+    r2.load_particles(st["pos"].astype(np.float64), st["vel"].astype(np.float64), c["type"])
+    r2.set_step(st["step"])
+    r2.compute_forces()
+    check(g.get_state(), r2.get_state(), "after 12 steps")
