@@ -63,7 +63,7 @@ def test_workspace_bytes_host_logic(pk):
     p = pk.make_params(wl.default_params((175.0, 175.0, 175.0)))
     assert pk.lib().mdpd_workspace_bytes(C.byref(p), 32_156_250, 0, None) < 60e9
     # invalid parameters -> 0
-    for bad in (dict(rd=1.5), dict(s=0.5), dict(skin=-1.0), dict(dt=0.0), dict(reorder_every=3)):
+    for bad in (dict(rd=1.5), dict(s=-0.5), dict(s=5.0), dict(skin=-1.0), dict(dt=0.0), dict(reorder_every=3)):
         q = pk.make_params(wl.default_params((10.0, 10.0, 10.0), **bad))
         assert pk.lib().mdpd_workspace_bytes(C.byref(q), 100, 0, None) == 0, bad
     q = pk.make_params(wl.default_params((3.0, 10.0, 10.0)))     # fewer than 3 cells of rc + skin along x (R4)
