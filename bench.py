@@ -328,7 +328,13 @@ def main_ours(args, rank, world, local):
     roof["step"] = {"alu_gops": round(win_ops / (tot * 1e-3) / 1e9, 1), "alu_frac": round(win_ops / (tot * 1e-3) / 1e9 / alu_peak, 4),
                     "ops_per_particle_step": round(win_ops / (n * K), 1)}
     roof["ms_per_launch"] = d.get("ms_per_launch")
-    roof["traffic"] = None
+    # DRAM bytes per launch of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum) from the committed
+    # ncu --set full capture of this workload, scaled per particle: profiles/r1k_fast_staging_4x4x4.md (config 4a / 4b)
+    ncu_dram_bytes_per_particle = {"4a": {"k_build_list": 149.6, "k_density": 265.5, "k_force": 126.3, "k_integrate": 94.7},
+                                   "4b": {"k_build_list": 88.0, "k_density": 232.7, "k_force": 113.0, "k_integrate": 64.5}}
+    tpp = ncu_dram_bytes_per_particle.get(args.workload, {}).get(dom)
+    roof["traffic"] = None if tpp is None else tpp * n
+    roof["traffic_source"] = None if tpp is None else "ncu --set full capture in profiles/r1k_fast_staging_4x4x4.md"
     roof["hbm_peak_gbs"] = peak_gbs
     roof["per_kernel"] = per_kernel
 
