@@ -698,8 +698,11 @@ __device__ __forceinline__ bool stage_fast(const DevP& p, const TileInfo& T, con
   }
   cp_async_wait_all();
   __syncwarp();
-  // to tile-relative coordinates, in place (a warp touches only what it copied itself)
-  for (unsigned q = warp; q < nitems; q += W) {
+  // To tile-relative coordinates, in place (a warp touches only what it copied itself).  A tile that does not touch the
+  // periodic boundary needs no periodic images: its staged coordinates stay the global ones (differences of nearby
+  // fp32 coordinates are as exact as differences of their translates) and the pass over the image is skipped.
+  const bool interior = T.c0x > 0 && T.c0x + T.ex < p.ncx && T.c0y > 0 && T.c0y + T.ey < p.ncy && T.c0z > 0 && T.c0z + T.ez < p.ncz;
+  for (unsigned q = warp; q < nitems && !interior; q += W) {
     const uint2 it = items[q];
     if (lane <= ((it.y >> 16) & 31u)) {
       const float4 sh = shtab[it.y >> 21];
