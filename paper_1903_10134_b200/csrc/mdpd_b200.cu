@@ -524,6 +524,7 @@ constexpr unsigned LCAP = 128;                 // per-particle list capacity
 constexpr int SCH = 4;                         // candidate chunks (of 32) held in registers at a time
 constexpr unsigned MAXCAND = 512;               // candidates (particles of a cell's 27-cell stencil) per window of the list build
 constexpr unsigned MSTRIDE = 17;                // words per particle slot of the hit masks (MAXCAND / 32 + 1: bank spread)
+constexpr unsigned BUILD_HIST = 132;  // LCAP + 1 bins of the list-length histogram of k_build_list, padded to 16 bytes
 constexpr unsigned BUILD_SCRATCH16 = (32 * MSTRIDE * 4 + 2 * MAXCAND * 2) / 2;  // per-warp scratch of the list build, in 16-bit units
 
 struct TileSmem {
@@ -845,6 +846,10 @@ __global__ void __launch_bounds__(BUILD_TPB) k_build_list(const DevP p) {
   const TileSmem sm = carve_smem(smraw, p.tile_cap, false);
   const unsigned cur = p.ctl->cur;
   const TileInfo T = p.tiles[blockIdx.x];
+  {  // the list-length histogram lives behind the warps' scratch; stage_tile's barriers order this before its first use
+    unsigned* const lh = (unsigned*)(sm.queue + (size_t)(blockDim.x >> 5) * BUILD_SCRATCH16);
+    for (unsigned k = threadIdx.x; k < BUILD_HIST; k += blockDim.x) lh[k] = 0u;
+  }
   const unsigned total = stage_tile<false>(p, T, p.pos[cur], nullptr, sm);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
   if (threadIdx.x == 0) {
@@ -869,6 +874,9 @@ __global__ void __launch_bounds__(BUILD_TPB) k_build_list(const DevP p) {
   // per-warp scratch behind the tables: hit masks [32 particle slots][MSTRIDE] and two candidate tables [MAXCAND]
   unsigned* const masks = (unsigned*)(sm.queue + (size_t)warp * BUILD_SCRATCH16);
   unsigned short* const tables = (unsigned short*)(masks + 32 * MSTRIDE);
+  // behind the warps' scratch: histogram of the list lengths, filled as the lengths become known, for the hand-out order
+  // of the density pass (counting sort at the end: one pass over the lengths instead of two)
+  unsigned* const lhist = (unsigned*)(sm.queue + (size_t)nwarps * BUILD_SCRATCH16);  // [LCAP + 1] (+ padding)
   const unsigned sent = p.tile_cap;
   unsigned smax = 0, ssum = 0;
   bool sover = false;
@@ -1012,14 +1020,37 @@ __global__ void __launch_bounds__(BUILD_TPB) k_build_list(const DevP p) {
         }
         p.nnbr[gi] = n;
         p.self_loc[gi] = (unsigned short)self;
+        atomicAdd(&lhist[LCAP - min(n, LCAP)], 1u);  // bin 0 = longest
         smax = max(smax, n);
         ssum += n;
       }
     }
   }
   // hand-out order of the density pass: own particles by decreasing list length (uses the now dead hbase table)
-  sort_own_by_length(sm, own_n, p.dinfo + own_s, [&](unsigned t) { return p.nnbr[own_s + t]; },
-                     [&](unsigned t) { return make_uint2(t | ((unsigned)p.self_loc[own_s + t] << 16), p.nnbr[own_s + t]); });
+  {  // the histogram is complete: scan it, then scatter the records (lengths and own slots were just written: L1 / L2)
+    __syncthreads();
+    if (threadIdx.x < 32) {  // exclusive scan of the LCAP + 1 bins by warp 0
+      unsigned run = 0;
+      for (unsigned b0 = 0; b0 <= LCAP; b0 += 32) {
+        const unsigned k = b0 + lane;
+        const unsigned c = k <= LCAP ? lhist[k] : 0u;
+        unsigned incl = c;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          const unsigned v = __shfl_up_sync(0xffffffffu, incl, o);
+          if (lane >= o) incl += v;
+        }
+        if (k <= LCAP) lhist[k] = run + incl - c;
+        run += __shfl_sync(0xffffffffu, incl, 31);
+      }
+    }
+    __syncthreads();
+    uint2* __restrict__ dout = p.dinfo + own_s;
+    for (unsigned t = threadIdx.x; t < own_n; t += blockDim.x) {
+      const unsigned n = p.nnbr[own_s + t];
+      dout[atomicAdd(&lhist[LCAP - min(n, LCAP)], 1u)] = make_uint2(t | ((unsigned)p.self_loc[own_s + t] << 16), n);
+    }
+  }
   // statistics + overflow flag
   smax = __reduce_max_sync(0xffffffffu, smax);
   ssum = __reduce_add_sync(0xffffffffu, ssum);
@@ -2105,7 +2136,8 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
   }
   h->smem_pos = tile_smem_bytes(h->d.tile_cap, false, 0);
   h->smem_posvel = tile_smem_bytes(h->d.tile_cap, true, 0);
-  h->smem_build = tile_smem_bytes(h->d.tile_cap, false, (size_t)BUILD_SCRATCH16 * (h->block_build / 32));
+  h->smem_build = tile_smem_bytes(h->d.tile_cap, false, (size_t)BUILD_SCRATCH16 * (h->block_build / 32)) +
+                  4 * (size_t)BUILD_HIST;  // + the list-length histogram
   if (h->smem_build > h->smem_limit) return set_err(h, MDPD_ENOMEM, "list build needs %zu bytes of shared memory", h->smem_build);
   CU_TRY(h, cudaFuncSetAttribute(k_build_list, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_build));
   CU_TRY(h, cudaFuncSetAttribute(k_density<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
