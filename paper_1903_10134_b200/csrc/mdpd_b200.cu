@@ -1027,8 +1027,27 @@ __global__ void __launch_bounds__(BUILD_TPB) k_build_list(const DevP p) {
     }
   }
   // hand-out order of the density pass: own particles by decreasing list length (uses the now dead hbase table)
+  // statistics of the tile: per warp into shared memory (lhist[LCAP + 1 ..]), one set of global atomics per CTA
+  smax = __reduce_max_sync(0xffffffffu, smax);
+  ssum = __reduce_add_sync(0xffffffffu, ssum);
+  const unsigned wover = __any_sync(0xffffffffu, sover);
+  if (lane == 0) {
+    atomicMax(&lhist[LCAP + 1], smax);
+    atomicAdd(&lhist[LCAP + 2], ssum);
+    if (wover) atomicOr(&lhist[LCAP + 1], 0x80000000u);
+  }
   {  // the histogram is complete: scan it, then scatter the records (lengths and own slots were just written: L1 / L2)
     __syncthreads();
+    if (threadIdx.x == 0) {
+      Ctl* c = p.ctl;
+      const unsigned mx = lhist[LCAP + 1];
+      atomicMax(&c->max_nbr, mx & 0x7FFFFFFFu);
+      atomicAdd(&c->sum_nbr, (unsigned long long)lhist[LCAP + 2]);
+      if (mx >> 31) {
+        atomicOr(&c->err, ERR_OVERFLOW);
+        atomicAdd(&c->overflow, 1ull);
+      }
+    }
     if (threadIdx.x < 32) {  // exclusive scan of the LCAP + 1 bins by warp 0
       unsigned run = 0;
       for (unsigned b0 = 0; b0 <= LCAP; b0 += 32) {
@@ -1049,19 +1068,6 @@ __global__ void __launch_bounds__(BUILD_TPB) k_build_list(const DevP p) {
     for (unsigned t = threadIdx.x; t < own_n; t += blockDim.x) {
       const unsigned n = p.nnbr[own_s + t];
       dout[atomicAdd(&lhist[LCAP - min(n, LCAP)], 1u)] = make_uint2(t | ((unsigned)p.self_loc[own_s + t] << 16), n);
-    }
-  }
-  // statistics + overflow flag
-  smax = __reduce_max_sync(0xffffffffu, smax);
-  ssum = __reduce_add_sync(0xffffffffu, ssum);
-  const unsigned wover = __any_sync(0xffffffffu, sover);
-  if (lane == 0) {
-    Ctl* c = p.ctl;
-    atomicMax(&c->max_nbr, smax);
-    atomicAdd(&c->sum_nbr, (unsigned long long)ssum);
-    if (wover) {
-      atomicOr(&c->err, ERR_OVERFLOW);
-      atomicAdd(&c->overflow, 1ull);
     }
   }
 }
