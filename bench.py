@@ -330,11 +330,11 @@ def main_ours(args, rank, world, local):
     roof["ms_per_launch"] = d.get("ms_per_launch")
     # DRAM bytes per launch of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum) from the committed
     # ncu --set full capture of this workload, scaled per particle: profiles/r1k_fast_staging_4x4x4.md (config 4a / 4b)
-    ncu_dram_bytes_per_particle = {"4a": {"k_build_list": 149.6, "k_density": 265.5, "k_force": 126.3, "k_integrate": 94.7},
+    ncu_dram_bytes_per_particle = {"4a": {"k_build_list": 149.6, "k_density": 268.1, "k_force": 126.2, "k_integrate": 94.8},
                                    "4b": {"k_build_list": 88.0, "k_density": 232.7, "k_force": 113.0, "k_integrate": 64.5}}
     # l1tex__data_pipe_lsu_wavefronts_mem_shared (% of peak) of the same captures: the unit that actually limits the two
     # per-step passes (16-byte gathers from the staged tile); static, from profiles/, not measured live
-    ncu_smem_pipe_frac = {"4a": {"k_density": 0.686, "k_force": 0.723, "k_build_list": 0.381},
+    ncu_smem_pipe_frac = {"4a": {"k_density": 0.668, "k_force": 0.729, "k_build_list": 0.390},
                           "4b": {"k_density": 0.549, "k_force": 0.656, "k_build_list": 0.341}}
     for k, v in ncu_smem_pipe_frac.get(args.workload, {}).items():
         if k in per_kernel:
