@@ -167,7 +167,7 @@ def algorithmic_bytes(kernel, n, n_list, n_act):
     rho 4 + compact list 2 n_act; force = pos 16 + (vel, rho) 16 + compact list 2 n_act + force 16; integrate = pos r/w
     32 + vel r/w 32 + force 16 + xbuild 16; list build = pos 16 + list 2 n_list + length and own slot 6."""
     per = {"k_density": 16 + 2 * n_list + 4 + 2 * n_act, "k_force": 16 + 16 + 2 * n_act + 16, "k_integrate": 96,
-           "k_build_list": 16 + 2 * n_list + 6}.get(kernel)
+           "k_cells_list": 16 + 2 * n_list + 6, "k_cells_direct": 16 + 4 + 2 * n_act + 8}.get(kernel)
     return None if per is None else per * n
 
 
@@ -175,7 +175,8 @@ def algorithmic_ops(kernel, n, n_list, n_act, n_cand=0.0):
     """Thread-level arithmetic/logic operations the formulas need (FMA = 1, no address or loop
     arithmetic): 13 per listed entry in the density pass (r^2, compare, weight), 48 per in-range pair in the force pass,
     7 per candidate of the 27-cell stencil (r^2, compare) in the list build."""
-    per = {"k_density": 13 * n_list, "k_force": 48 * n_act, "k_build_list": 7 * n_cand}.get(kernel)
+    per = {"k_density": 13 * n_list, "k_force": 48 * n_act, "k_cells_list": 7 * n_cand,
+           "k_cells_direct": 7 * n_cand + 13 * n_act}.get(kernel)
     return None if per is None else per * n
 
 
@@ -216,6 +217,7 @@ def main_ours(args, rank, world, local):
     c = wl.make_config(args.workload if args.workload in ("4a", "4b") else int(args.workload))
     if args.skin is not None:
         c["params"]["skin"] = float(args.skin)
+    c["params"]["flags"] = (2 if args.direct else 0) | (1 if args.no_graph else 0)
     n = len(c["pos"])
     md = None if c.get("mask") is None else c["mask"].shape[::-1]
     # pinned host buffers (inputs of the e2e leg, outputs of get_state)
@@ -272,7 +274,7 @@ def main_ours(args, rank, world, local):
     dom = max(hot, key=lambda k: prof[k][0])
     kernels = {k: {"ms_total": round(prof[k][0], 4), "launches": prof[k][1],
                    "share": round(prof[k][0] / tot, 4) if tot else None} for k in prof}
-    kernels["k_build_list"]["real_rebuilds"] = reb_prof
+    kernels["k_permute"]["real_rebuilds"] = reb_prof
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
@@ -291,11 +293,11 @@ def main_ours(args, rank, world, local):
     n_cand = 27.0 * n / ncell                       # candidates per particle: the 27-cell stencil at the mean occupancy
 
     def launch_ms(k):   # mean duration of the launches that did work (rebuild-chain kernels: real rebuilds only)
-        cnt = reb_prof if k == "k_build_list" else prof[k][1]
+        cnt = reb_prof if k == "k_cells_list" else prof[k][1]
         return prof[k][0] / max(1, cnt)
 
     per_kernel = {}
-    for k in ("k_force", "k_density", "k_build_list", "k_integrate"):
+    for k in ("k_force", "k_density", "k_cells_list", "k_cells_direct", "k_integrate"):
         t = launch_ms(k)
         if t <= 0:
             continue
@@ -323,19 +325,22 @@ def main_ours(args, rank, world, local):
                 "frac": d.get("hbm_frac"), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": algorithmic_bytes(dom, n, n_list, n_act)}
     # the whole step against the same ALU peak: algorithmic operations of all launches of the profiled window / its time
-    win_ops = K * (algorithmic_ops("k_density", n, n_list, n_act) + algorithmic_ops("k_force", n, n_list, n_act)) + \
-        reb_prof * algorithmic_ops("k_build_list", n, n_list, n_act, n_cand)
+    if args.direct:
+        win_ops = K * (algorithmic_ops("k_cells_direct", n, n_list, n_act, n_cand) + algorithmic_ops("k_force", n, n_list, n_act))
+    else:
+        win_ops = K * (algorithmic_ops("k_density", n, n_list, n_act) + algorithmic_ops("k_force", n, n_list, n_act)) + \
+            reb_prof * algorithmic_ops("k_cells_list", n, n_list, n_act, n_cand)
     roof["step"] = {"alu_gops": round(win_ops / (tot * 1e-3) / 1e9, 1), "alu_frac": round(win_ops / (tot * 1e-3) / 1e9 / alu_peak, 4),
                     "ops_per_particle_step": round(win_ops / (n * K), 1)}
     roof["ms_per_launch"] = d.get("ms_per_launch")
     # DRAM bytes per launch of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum) from the committed
     # ncu --set full capture of this workload, scaled per particle: profiles/r1k_fast_staging_4x4x4.md (config 4a / 4b)
-    ncu_dram_bytes_per_particle = {"4a": {"k_build_list": 149.6, "k_density": 268.1, "k_force": 126.2, "k_integrate": 94.8},
-                                   "4b": {"k_build_list": 88.0, "k_density": 232.7, "k_force": 113.0, "k_integrate": 64.5}}
+    ncu_dram_bytes_per_particle = {"4a": {"k_cells_list": 149.6, "k_density": 268.1, "k_force": 126.2, "k_integrate": 94.8},
+                                   "4b": {"k_cells_list": 88.0, "k_density": 232.7, "k_force": 113.0, "k_integrate": 64.5}}
     # l1tex__data_pipe_lsu_wavefronts_mem_shared (% of peak) of the same captures: the unit that actually limits the two
     # per-step passes (16-byte gathers from the staged tile); static, from profiles/, not measured live
-    ncu_smem_pipe_frac = {"4a": {"k_density": 0.668, "k_force": 0.729, "k_build_list": 0.390},
-                          "4b": {"k_density": 0.549, "k_force": 0.656, "k_build_list": 0.341}}
+    ncu_smem_pipe_frac = {"4a": {"k_density": 0.668, "k_force": 0.729, "k_cells_list": 0.390},
+                          "4b": {"k_density": 0.549, "k_force": 0.656, "k_cells_list": 0.341}}
     for k, v in ncu_smem_pipe_frac.get(args.workload, {}).items():
         if k in per_kernel:
             per_kernel[k]["smem_pipe_frac_ncu"] = v
@@ -375,6 +380,7 @@ def main_ours(args, rank, world, local):
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": workload_name(args.workload, n), "particles_per_gpu": n,
                        "parallelism": "replicas only" if world > 1 else "1 gpu",
+                       "neighbour_path": "list-free (MDPD_FLAG_DIRECT)" if args.direct else "Verlet list",
                        "equilibration_steps": args.equilibrate, "skin": c["params"]["skin"],
                        "l2": "inputs larger than L2" if n * 700 > 126e6 * 2 else "inputs fit L2 (small case)",
                        "rebuilds_in_window": rebuilds, "mean_list_len": round(n_list, 2),
@@ -406,6 +412,8 @@ def main():
     ap.add_argument("--workload", default="4a", choices=["4a", "4b", "0", "1", "2", "3"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--equilibrate", type=int, default=EQUILIBRATE, help="untimed steps after loading")
+    ap.add_argument("--direct", action="store_true", help="list-free path (MDPD_FLAG_DIRECT): no Verlet list")
+    ap.add_argument("--no-graph", action="store_true", help="launch the kernels one by one (MDPD_FLAG_NO_GRAPH; for ncu)")
     ap.add_argument("--skin", type=float, default=None, help="override the Verlet-list skin (default: the config's 0.25)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))

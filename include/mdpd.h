@@ -63,6 +63,9 @@ typedef struct {
 } mdpd_params;
 
 #define MDPD_FLAG_NO_GRAPH 1u /* launch kernels one by one instead of replaying the captured CUDA graph */
+#define MDPD_FLAG_DIRECT 2u   /* list-free path: no Verlet list; every step finds the r < rc neighbours straight from the
+                                 cells (same results; the cells are still re-sorted on the skin/2 displacement trigger).
+                                 Fixed by mdpd_load_particles. */
 
 /* Create a handle on CUDA device `device`; `cuda_stream` is a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream)
  * or NULL for the default stream.  The handle must be destroyed with mdpd_destroy. */

@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_PKG, "libmdpd_b200.so")
 MDPD_OK, MDPD_EINVAL, MDPD_ENOMEM, MDPD_ECUDA = 0, -1, -2, -3
 MDPD_EOVERFLOW, MDPD_ESTATE, MDPD_ENAN, MDPD_EINSOLID = -4, -5, -6, -7
 MDPD_FLAG_NO_GRAPH = 1
+MDPD_FLAG_DIRECT = 2
 
 _ERRNAME = {-1: "MDPD_EINVAL", -2: "MDPD_ENOMEM", -3: "MDPD_ECUDA", -4: "MDPD_EOVERFLOW", -5: "MDPD_ESTATE",
             -6: "MDPD_ENAN", -7: "MDPD_EINSOLID"}

@@ -49,7 +49,6 @@ struct Ctl {
   unsigned has_wall;  // some particle is frozen (set by k_pack)
   unsigned long long steps, rebuilds, bounces, sum_nbr, overflow, nan_events, sum_act, dens_passes, graph_rebuilds, pad2;
   double vir[6];             // k_force<.., VIRIAL>: sum over list entries of r_a F^C_b (xx, yy, zz, xy, xz, yz); each pair twice
-  unsigned long long ph[4];  // -DMDPD_PHASES: clock cycles of k_force's staging / sort / pair loop, summed over CTAs, and the CTA count
 };
 
 struct TileInfo {  // one CTA of the list / density / force passes
@@ -86,6 +85,11 @@ struct DevP {  // passed by value to every kernel
   Ctl* ctl;
   // sizes
   unsigned N, ncell, cap, ntiles, tile_cap, run_stride;
+  unsigned nrun_max;     // run records per tile: 3 (ty + 2)(tz + 2)
+  unsigned hb_off;       // recipe: offset (in uint4) of the tile's table of first staged slots of its halo cells (u16)
+  unsigned cap_act;      // capacity of the per-step in-range (r < rc) lists of the list-free path
+  unsigned rows_verlet, rows_direct;  // bytes per row of k_cells' per-warp row buffers (list build / list-free pass)
+  float dot_margin;      // slack of the approximate (dot-product form) range test of k_cells, in units of r^2
   int ncx, ncy, ncz;
   int mx, my, mz;
   // geometry
@@ -521,11 +525,6 @@ constexpr int HMAX = 216;                      // halo cells of the largest tile
 constexpr int HTAB = 224;                      // table size (HMAX + 1 rounded up)
 static_assert(HMAX + 1 <= HTAB, "halo table");
 constexpr unsigned LCAP = 128;                 // per-particle list capacity
-constexpr int SCH = 4;                         // candidate chunks (of 32) held in registers at a time
-constexpr unsigned MAXCAND = 512;               // candidates (particles of a cell's 27-cell stencil) per window of the list build
-constexpr unsigned MSTRIDE = 17;                // words per particle slot of the hit masks (MAXCAND / 32 + 1: bank spread)
-constexpr unsigned BUILD_HIST = 132;  // LCAP + 1 bins of the list-length histogram of k_build_list, padded to 16 bytes
-constexpr unsigned BUILD_SCRATCH16 = (32 * MSTRIDE * 4 + 2 * MAXCAND * 2) / 2;  // per-warp scratch of the list build, in 16-bit units
 
 struct TileSmem {
   float4* spos;      // [cap + 1] (x_rel, y_rel, z_rel, particle word); slot cap = the far-away sentinel
@@ -667,7 +666,7 @@ __device__ __forceinline__ bool stage_fast(const DevP& p, const TileInfo& T, con
   float4* const shtab = (float4*)sm.hbase;  // [27] shift of every code
   // the records are requested together with the header (whose nruns bounds them): one latency for both
   const uint4* __restrict__ rec = p.runs + (size_t)blockIdx.x * p.run_stride + 1;
-  const unsigned nrec = p.run_stride - 1u;
+  const unsigned nrec = p.nrun_max;
   const unsigned total = hdr.x, nruns = hdr.y, nitems = hdr.z & 0xFFFFu;
   for (unsigned r = threadIdx.x; r < nrec; r += blockDim.x) {
     const uint4 R = rec[r];
@@ -723,361 +722,491 @@ __device__ __forceinline__ bool stage_fast(const DevP& p, const TileInfo& T, con
   return true;
 }
 
-// Written by warp 0 of k_build_list right after stage_tile (hbase = first staged slot of every halo cell, hshift.w =
-// global index - staged slot of the cell's particles).
-__device__ __forceinline__ void write_tile_runs(const DevP& p, const TileInfo& T, const TileSmem& sm, unsigned total,
-                                                unsigned os, unsigned nown) {
-  const int lane = threadIdx.x & 31;
+// ----------------------------------------------------------------------------------------------------------------
+// Tile recipe.  After every sort k_tile_recipe (one CTA per tile) writes what the tile passes need to stage the tile
+// without rediscovering its geometry: the header and run records described above, and the table of the first
+// staged slot of every halo cell (16-bit, nh + 1 entries, at uint4 offset hb_off of the tile's record).  It also
+// keeps the two occupancy maxima (tile + halo: shared-memory capacity; tile alone: CTA size).
+// ----------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) k_tile_recipe(const DevP p, int latch_faults) {
+  if (!p.ctl->rebuild) return;
+  __shared__ unsigned s_hb[HTAB];  // particles of every halo cell, then their exclusive scan (first staged slot)
+  __shared__ unsigned s_g[HTAB];   // first sorted (global) index of every halo cell
+  const TileInfo T = p.tiles[blockIdx.x];
   const int hxn = T.ex + 2, hyn = T.ey + 2, hzn = T.ez + 2;
-  const unsigned nruns = 3u * hyn * hzn;
-  uint4* const out = p.runs + (size_t)blockIdx.x * p.run_stride;
-  unsigned run_items = 0;
-  for (unsigned r0 = 0; r0 < nruns; r0 += 32) {
-    const unsigned r = r0 + lane;
-    unsigned cnt = 0, sb = 0, g = 0, code = 0;
-    if (r < nruns) {
-      const int seg = r % 3, hy = (r / 3) % hyn, hz = r / (3 * hyn);
-      const int hx = seg == 0 ? 0 : (seg == 1 ? 1 : hxn - 1), len = seg == 1 ? T.ex : 1;
-      const int h0 = (hz * hyn + hy) * hxn + hx;
-      sb = sm.hbase[h0];
-      cnt = sm.hbase[h0 + len] - sb;
-      g = sb + f2u(sm.hshift[h0].w);
-      const int cx = T.c0x + hx - 1, cy = T.c0y + hy - 1, cz = T.c0z + hz - 1;
-      code = (cx < 0 ? 1u : (cx >= p.ncx ? 2u : 0u)) + 3u * (cy < 0 ? 1u : (cy >= p.ncy ? 2u : 0u)) +
-             9u * (cz < 0 ? 1u : (cz >= p.ncz ? 2u : 0u));
-    }
-    const unsigned nit = (cnt + 31u) >> 5;
-    unsigned incl = nit;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const unsigned t = __shfl_up_sync(0xffffffffu, incl, o);
-      if (lane >= o) incl += t;
-    }
-    if (r < nruns) out[1 + r] = make_uint4(g, sb | (cnt << 16), code, run_items + incl - nit);
-    run_items += __shfl_sync(0xffffffffu, incl, 31);
-  }
-  if (lane == 0) out[0] = make_uint4(total, nruns, run_items | (nown << 16), os);
-}
-
-// per-tile statistics after the first sort (load time): largest halo population (shared-memory capacity) and largest
-// tile.  One warp per tile, lanes over the halo cells.  During stepping k_build_list keeps the same two maxima.
-__global__ void __launch_bounds__(128) k_tile_stats(const DevP p) {
-  const unsigned t = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  const int lane = threadIdx.x & 31;
-  if (t >= p.ntiles) return;
-  const TileInfo T = p.tiles[t];
-  const int hxn = T.ex + 2, hyn = T.ey + 2, nh = hxn * hyn * (T.ez + 2);
-  unsigned halo = 0;
-  for (int h = lane; h < nh; h += 32) {
+  const int nh = hxn * hyn * hzn;
+  for (int h = threadIdx.x; h < nh; h += blockDim.x) {
     const int hx = h % hxn, hy = (h / hxn) % hyn, hz = h / (hxn * hyn);
     float a;
     const int cx = halo_cell(T.c0x, hx, p.ncx, 0.f, 0.f, a), cy = halo_cell(T.c0y, hy, p.ncy, 0.f, 0.f, a),
               cz = halo_cell(T.c0z, hz, p.ncz, 0.f, 0.f, a);
     const unsigned r = p.cell_rank[((unsigned)cz * p.ncy + cy) * p.ncx + cx];
-    halo += p.cell_start[r + 1] - p.cell_start[r];
+    const unsigned s = p.cell_start[r];
+    s_hb[h] = p.cell_start[r + 1] - s;
+    s_g[h] = s;
   }
-  halo = __reduce_add_sync(0xffffffffu, halo);
-  if (lane == 0) {
-    atomicMax(&p.ctl->max_halo, halo);
-    atomicMax(&p.ctl->max_own, p.cell_start[T.rank0 + T.ncell_own] - p.cell_start[T.rank0]);
-  }
-}
-
-// Own particles are handed to the warps in order of decreasing list length (a counting sort on the length in shared
-// memory, the order written to `out`): group g = sorted particles 32 g .. 32 g + 31, so the lanes of a warp finish
-// together; warp w then takes the groups w, 2W-1-w, 2W+w, 4W-1-w, ... (a long group is followed by a short one), so
-// the warps of the CTA finish together too.  Which thread evaluates which particle does not change any result.
-// The order for the density pass (key: list length) is made once per list build, the order for the force pass (key:
-// in-range count of the step) by the density pass that precedes it.  hist = the hbase table (dead by then).
-// All threads of the CTA must call it.
-template <class LenFn, class RecFn>
-__device__ __forceinline__ void sort_own_by_length(const TileSmem& sm, unsigned nown, uint2* out, LenFn len, RecFn rec) {
-  unsigned* const hist = sm.hbase;  // [LCAP + 1] <= HTAB
   __syncthreads();
-  for (unsigned k = threadIdx.x; k <= LCAP; k += blockDim.x) hist[k] = 0u;
-  __syncthreads();
-  for (unsigned t = threadIdx.x; t < nown; t += blockDim.x) atomicAdd(&hist[LCAP - min(len(t), LCAP)], 1u);  // bin 0 = longest
-  __syncthreads();
-  if (threadIdx.x < 32) {  // exclusive scan of the LCAP + 1 bins by warp 0
-    const int lane = threadIdx.x;
+  const int lane = threadIdx.x & 31;
+  if (threadIdx.x < 32) {  // exclusive scan of the counts by warp 0
     unsigned run = 0;
-    for (unsigned b0 = 0; b0 <= LCAP; b0 += 32) {
-      const unsigned k = b0 + lane;
-      const unsigned c = k <= LCAP ? hist[k] : 0u;
+    for (int b0 = 0; b0 < nh; b0 += 32) {
+      const int h = b0 + lane;
+      const unsigned c = h < nh ? s_hb[h] : 0u;
       unsigned incl = c;
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) {
-        const unsigned v = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= o) incl += v;
+        const unsigned t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
       }
-      if (k <= LCAP) hist[k] = run + incl - c;
+      if (h < nh) s_hb[h] = run + incl - c;
       run += __shfl_sync(0xffffffffu, incl, 31);
     }
+    if (lane == 0) s_hb[nh] = run;
   }
   __syncthreads();
-  for (unsigned t = threadIdx.x; t < nown; t += blockDim.x) out[atomicAdd(&hist[LCAP - min(len(t), LCAP)], 1u)] = rec(t);
+  const unsigned total = s_hb[nh];
+  const bool fits = total <= p.tile_cap;
+  const unsigned own_s = p.cell_start[T.rank0], own_n = p.cell_start[T.rank0 + T.ncell_own] - own_s;
+  uint4* const out = p.runs + (size_t)blockIdx.x * p.run_stride;
+  unsigned short* const hb16 = (unsigned short*)(out + p.hb_off);
+  for (int h = threadIdx.x; h <= nh; h += blockDim.x) hb16[h] = (unsigned short)min(s_hb[h], 0xFFFFu);
+  if (threadIdx.x < 32) {  // run records: per (y, z) halo row the cell at x = -1, the tile-aligned cells, the cell at x = ex
+    const unsigned nruns = 3u * hyn * hzn;
+    unsigned run_items = 0;
+    for (unsigned r0 = 0; r0 < nruns; r0 += 32) {
+      const unsigned r = r0 + lane;
+      unsigned cnt = 0, sb = 0, g = 0, code = 0;
+      if (r < nruns) {
+        const int seg = r % 3, hy = (r / 3) % hyn, hz = r / (3 * hyn);
+        const int hx = seg == 0 ? 0 : (seg == 1 ? 1 : hxn - 1), len = seg == 1 ? T.ex : 1;
+        const int h0 = (hz * hyn + hy) * hxn + hx;
+        sb = s_hb[h0];
+        cnt = s_hb[h0 + len] - sb;
+        g = s_g[h0];
+        const int cx = T.c0x + hx - 1, cy = T.c0y + hy - 1, cz = T.c0z + hz - 1;
+        code = (cx < 0 ? 1u : (cx >= p.ncx ? 2u : 0u)) + 3u * (cy < 0 ? 1u : (cy >= p.ncy ? 2u : 0u)) +
+               9u * (cz < 0 ? 1u : (cz >= p.ncz ? 2u : 0u));
+      }
+      const unsigned nit = (cnt + 31u) >> 5;
+      unsigned incl = nit;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const unsigned t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+      }
+      if (r < nruns) out[1 + r] = make_uint4(g, sb | (cnt << 16), code, run_items + incl - nit);
+      run_items += __shfl_sync(0xffffffffu, incl, 31);
+    }
+    if (lane == 0) {
+      out[0] = fits ? make_uint4(total, nruns, run_items | (own_n << 16), own_s) : make_uint4(0xFFFFFFFFu, 0u, own_n << 16, own_s);
+      atomicMax(&p.ctl->max_halo, total);
+      atomicMax(&p.ctl->max_own, own_n);
+      if (!fits && latch_faults) {  // reported as MDPD_EOVERFLOW; the tile passes skip this tile
+        atomicOr(&p.ctl->err, ERR_TILE);
+        atomicAdd(&p.ctl->overflow, 1ull);
+      }
+    }
+  }
 }
 
-// group of 32 sorted own particles that warp `warp` of W takes in its round r (see above)
+// group of 32 sorted own particles that warp `warp` of W takes in its round r (see the hand-out below)
 __device__ __forceinline__ unsigned group_of_round(unsigned r, unsigned warp, unsigned W) {
   return (r & 1u) ? (r + 1u) * W - 1u - warp : r * W + warp;
 }
 
 // ----------------------------------------------------------------------------------------------------------------
-// a3: Verlet list (full list: every j != i with r < rc + skin at build time).  Two phases per pair of own cells.
+// a3 (and S8f f1): k_cells -- neighbours straight from the cells.  One kernel, two uses:
+//   MODE 0  Verlet list build (full list: every j != i with r < rc + skin at build time), in the rebuild chain;
+//   MODE 1  the list-free path (mdpd_params.flags & MDPD_FLAG_DIRECT): every step, the in-range (r < rc) lists of
+//           the step straight from the 27-cell stencil, the density pass over them, and the hand-out of the force pass.
 //
-// Phase 1, warp per cell ("32 distances per instruction"): the candidates of the cell's 27-cell stencil are nine
-// contiguous runs of the staged array (one per (y, z) row of halo cells); they are flattened and held IN REGISTERS,
-// SCH chunks of 32 at a time (one candidate per lane and chunk), while the warp loops over the cell's own particles:
-// one broadcast load of x_i, one distance per lane, one ballot -- the 32-bit hit mask of (particle, chunk) goes to
-// shared memory.  No per-hit work at all in this phase.
-//
-// Phase 2, thread per particle: the two cells of the pair occupy the two half-warps; every lane walks the set bits
-// of its particle's masks in increasing candidate order (deterministic), looks the staged slot up in the cell's
-// candidate table and pushes it through a 128-bit shift register; every 8 entries one 16-byte chunk is stored
-// straight to the list, layout [chunk][i], the last chunk padded with the sentinel slot.
+// Orientation: LANE = own particle, the candidate is BROADCAST.  A warp takes a group of consecutive own cells of one
+// x-row of the tile holding at most 32 particles (one per lane); the candidates of the whole group are nine contiguous
+// runs of the staged image (the (y, z) rows of the stencil, from one cell left of the group to one cell right of
+// it).  The staged image holds, per slot, (x, y, z, -|x|^2) in tile-CENTRED coordinates, so the range test of candidate
+// c against the lane's particle is the dot-product form
+//     |xi|^2 - cut^2 - 2 xi . xc  <  -|xc|^2        (3 FFMA + 1 compare; one uniform 16-byte shared-memory load),
+// evaluated with a slack `dot_margin` on cut^2 that covers its rounding error (|x| <= ~4 in centred coordinates): the
+// hits are a SUPERSET of the exact r^2 < cut^2 set.  A hit costs one predicated 16-bit store of the candidate's
+// staged slot into the lane's row of a per-warp buffer in shared memory and one predicated pointer increment: no
+// ballots, no mask decoding, no compaction, and entries come out in increasing staged-slot order (deterministic).
+// MODE 0 copies the rows to the list (16-byte chunks, layout [chunk][particle]: consecutive lanes write consecutive
+// particles).  MODE 1 then walks its row per lane with the EXACT fp32 distance (same arithmetic as k_density):
+// density sum over r < rd, entries that fail 1e-12 < r^2 < rc^2 exactly (slack hits, coincident particles R10,
+// frozen-frozen pairs R8) are replaced by the far-away sentinel slot, and the row becomes the step's compact list.
 // ----------------------------------------------------------------------------------------------------------------
-#ifndef BUILD_TPB
-#define BUILD_TPB 384  // most threads per CTA of the list build
-#endif
-__global__ void __launch_bounds__(BUILD_TPB) k_build_list(const DevP p) {
-  if (!p.ctl->rebuild) return;
+constexpr int CELLS_MAXW = 12;       // most warps per CTA
+constexpr unsigned ROW_SLACK = 16;   // a full row is noticed within this many candidates
+constexpr unsigned CELLS_ITEMS = 64; // work items per tile: at most one per own cell
+
+__host__ __device__ inline unsigned cells_row_bytes(unsigned rowcap) {
+  unsigned b = 2u * (rowcap + ROW_SLACK) + 16u;  // + one chunk of sentinel padding
+  if (((b >> 4) & 1u) == 0u) b += 16u;           // odd number of 16-byte groups: 16-byte row reads of consecutive lanes do not collide
+  return b;
+}
+__host__ __device__ inline size_t cells_smem_bytes(unsigned tile_cap, unsigned row_bytes, unsigned nwarps) {
+  return (size_t)(tile_cap + 1) * 16 + HTAB * 16 + HTAB * 4 + HTAB * 2 + (size_t)nwarps * 32 * row_bytes;
+}
+
+__device__ __forceinline__ void sts_u16(unsigned addr, unsigned v) {
+  asm volatile("st.shared.u16 [%0], %1;" ::"r"(addr), "h"((unsigned short)v) : "memory");
+}
+__device__ __forceinline__ uint4 lds4u(unsigned addr) {
+  uint4 v;
+  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+  return v;
+}
+
+// stage_fast's copy (recipe -> items -> cp.async), then one pass in place to centred coordinates and -|x|^2 (bit 0 of
+// which carries the frozen flag when HAS_WALL); also fetches the tile's table of first staged slots.
+template <bool HAS_WALL>
+__device__ __forceinline__ bool stage_cells(const DevP& p, const TileInfo& T, const uint4 hdr, const float4* __restrict__ pos,
+                                            float4* img, uint2* items, float4* shtab, unsigned short* hb) {
+  const uint4* __restrict__ rcp = p.runs + (size_t)blockIdx.x * p.run_stride;
+  const uint4* __restrict__ rec = rcp + 1;
+  const unsigned nrec = p.nrun_max;
+  const unsigned total = hdr.x, nruns = hdr.y, nitems = hdr.z & 0xFFFFu;
+  if (total > p.tile_cap) return false;  // flagged by k_tile_recipe (block-uniform)
+  for (unsigned r = threadIdx.x; r < nrec; r += blockDim.x) {
+    const uint4 R = rec[r];
+    if (r < nruns) {
+      const unsigned cnt = R.y >> 16, sb = R.y & 0xFFFFu;
+      unsigned io = R.w;
+      for (unsigned c = 0; c < cnt; c += 32, ++io)
+        items[io] = make_uint2(R.x + c, (sb + c) | ((min(32u, cnt - c) - 1u) << 16) | (R.z << 21));
+    }
+  }
+  {
+    const unsigned nh1 = (unsigned)((T.ex + 2) * (T.ey + 2) * (T.ez + 2)) + 1u;
+    const uint4* __restrict__ src = rcp + p.hb_off;
+    uint4* const dst = (uint4*)hb;
+    for (unsigned q = threadIdx.x; q < (nh1 + 7u) / 8u; q += blockDim.x) dst[q] = src[q];
+  }
+  if (threadIdx.x < 27) {  // shift of every periodic-image code, minus the tile centre (both on the 2^-6 grid)
+    const unsigned c = threadIdx.x, cx = c % 3u, cy = (c / 3u) % 3u, cz = c / 9u;
+    const float ox = tile_origin(T.c0x, p.edge_x), oy = tile_origin(T.c0y, p.edge_y), oz = tile_origin(T.c0z, p.edge_z);
+    const float hx = floorf(0.5f * (float)T.ex * p.edge_x * 64.0f) * (1.0f / 64.0f),
+                hy = floorf(0.5f * (float)T.ey * p.edge_y * 64.0f) * (1.0f / 64.0f),
+                hz = floorf(0.5f * (float)T.ez * p.edge_z * 64.0f) * (1.0f / 64.0f);
+    shtab[c] = make_float4((cx == 0u ? -ox : (cx == 1u ? -p.Lx : p.Lx - ox)) - hx, (cy == 0u ? -oy : (cy == 1u ? -p.Ly : p.Ly - oy)) - hy,
+                           (cz == 0u ? -oz : (cz == 1u ? -p.Lz : p.Lz - oz)) - hz, 0.f);
+  }
+  __syncthreads();
+  const unsigned warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
+  const unsigned ibase = smem_addr(img);
+  for (unsigned q = warp; q < nitems; q += W) {
+    const uint2 it = items[q];
+    if (lane <= ((it.y >> 16) & 31u)) cp_async16(ibase + (((it.y & 0xFFFFu) + lane) << 4), pos + it.x + lane);
+  }
+  cp_async_wait_all();
+  __syncwarp();
+  for (unsigned q = warp; q < nitems; q += W) {  // a warp touches only what it copied itself
+    const uint2 it = items[q];
+    if (lane <= ((it.y >> 16) & 31u)) {
+      const float4 sh = shtab[it.y >> 21];
+      float4* const xp = img + (it.y & 0xFFFFu) + lane;
+      float4 x = *xp;
+      x.x += sh.x;
+      x.y += sh.y;
+      x.z += sh.z;
+      float q2 = -fmaf(x.z, x.z, fmaf(x.y, x.y, x.x * x.x));
+      if (HAS_WALL) q2 = u2f((f2u(q2) & ~1u) | (f2u(x.w) >> 31));
+      x.w = q2;
+      *xp = x;
+    }
+  }
+  if (threadIdx.x == 0) img[p.tile_cap] = make_float4(1e9f, 1e9f, 1e9f, -3e18f);  // sentinel slot: out of range of everything
+  __syncthreads();
+  return true;
+}
+
+// candidates [s, se) of the staged image against the lane's particle; hits are appended to the lane's row
+template <bool EXCL>
+__device__ __forceinline__ void scan_range(const unsigned ibase, unsigned s, const unsigned se, const float ax, const float ay,
+                                           const float az, float& bi, const unsigned self, unsigned& rp, const unsigned rp_lim,
+                                           bool& over) {
+  auto test = [&](const float4 c, const unsigned slot) {
+    const float v = fmaf(c.x, ax, fmaf(c.y, ay, fmaf(c.z, az, bi)));
+    bool hit = v < c.w;
+    if (EXCL) hit = hit && slot != self;
+    if (hit) {
+      sts_u16(rp, slot);
+      rp += 2u;
+    }
+  };
+  while (s < se) {
+    if (__any_sync(0xffffffffu, rp > rp_lim)) {  // a full row stops collecting: its list is reported as overflowed
+      if (rp > rp_lim) {
+        bi = __int_as_float(0x7f800000);
+        over = true;
+      }
+    }
+    const unsigned e = min(se, s + ROW_SLACK);
+    for (; s + 4u <= e; s += 4u) {
+      const unsigned a = ibase + (s << 4);
+      const float4 c0 = lds4(a), c1 = lds4(a + 16u), c2 = lds4(a + 32u), c3 = lds4(a + 48u);
+      test(c0, s);
+      test(c1, s + 1u);
+      test(c2, s + 2u);
+      test(c3, s + 3u);
+    }
+    for (; s < e; ++s) test(lds4(ibase + (s << 4)), s);
+  }
+}
+
+template <bool HAS_WALL, bool ALL>
+__device__ __forceinline__ void direct_entry(const DevP& p, const unsigned ibase, const float4 xi, const unsigned walli,
+                                             const unsigned j, const unsigned kaddr, const unsigned sent, float& rho,
+                                             unsigned& nin) {
+  const float4 xj = lds4(ibase + (j << 4));  // padding entries hit the far-away sentinel
+  const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
+  const float r2 = dx * dx + dy * dy + dz * dz;
+  const float rr = r2 + 1e-30f;  // r = 0 (coincident particles, R10) must not produce 0 * inf
+  const float w = __saturatef(fmaf(-(rr * rsqrt_fast(rr)), p.inv_rd, 1.0f));
+  rho = fmaf(w, w, rho);
+  bool in = f2u(r2 - 1e-12f) < f2u(p.rc2 - 1e-12f);  // 1e-12 < r2 < rc2, exact (see density_entry)
+  if (HAS_WALL && ALL) in = in && !(walli & f2u(xj.w) & 1u);  // frozen-frozen pairs do not interact (R8)
+  if (!in) sts_u16(kaddr, sent);
+  nin += in ? 1u : 0u;
+}
+
+template <int MODE, bool HAS_WALL, bool ALL>
+__global__ void __launch_bounds__(CELLS_MAXW * 32, 2) k_cells(const DevP p, int always) {
+  if (!always && !p.ctl->rebuild) return;
   extern __shared__ __align__(16) unsigned char smraw[];
-  const TileSmem sm = carve_smem(smraw, p.tile_cap, false);
+  float4* const img = (float4*)smraw;
+  unsigned char* q = smraw + (size_t)(p.tile_cap + 1) * 16;
+  uint2* const sitems = (uint2*)q;                    // staging items; afterwards the work items and the histogram
+  uint4* const witems = (uint4*)q;                    // [CELLS_ITEMS]
+  unsigned* const lhist = (unsigned*)(q + CELLS_ITEMS * 16);  // [LCAP + 1] bins (bin 0 = longest), then: max, sum, faults, next item
+  q += HTAB * 16;
+  float4* const shtab = (float4*)q;
+  q += HTAB * 4;
+  unsigned short* const hb = (unsigned short*)q;
+  q += HTAB * 2;
+  static_assert(CELLS_ITEMS * 16 + (LCAP + 8) * 4 <= HTAB * 16, "k_cells scratch");
   const unsigned cur = p.ctl->cur;
   const TileInfo T = p.tiles[blockIdx.x];
-  {  // the list-length histogram lives behind the warps' scratch; stage_tile's barriers order this before its first use
-    unsigned* const lh = (unsigned*)(sm.queue + (size_t)(blockDim.x >> 5) * BUILD_SCRATCH16);
-    for (unsigned k = threadIdx.x; k < BUILD_HIST; k += blockDim.x) lh[k] = 0u;
-  }
-  const unsigned total = stage_tile<false>(p, T, p.pos[cur], nullptr, sm);
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
-  if (threadIdx.x == 0) {
-    atomicMax(&p.ctl->max_halo, total == 0xFFFFFFFFu ? sm.hbase[(T.ex + 2) * (T.ey + 2) * (T.ez + 2)] : total);
-    atomicMax(&p.ctl->max_own, p.cell_start[T.rank0 + T.ncell_own] - p.cell_start[T.rank0]);
-  }
-  const unsigned own_s = p.cell_start[T.rank0], own_n = p.cell_start[T.rank0 + T.ncell_own] - own_s;
-  if (total == 0xFFFFFFFFu) {  // does not fit: flag it, leave empty lists; the per-step passes skip the tile
-    for (unsigned i = own_s + threadIdx.x; i < own_s + own_n; i += blockDim.x) {
-      p.nnbr[i] = 0u;
-      p.self_loc[i] = 0;
-    }
-    if (threadIdx.x == 0) {
-      p.runs[(size_t)blockIdx.x * p.run_stride] = make_uint4(0xFFFFFFFFu, 0u, own_n << 16, own_s);
-      atomicOr(&p.ctl->err, ERR_TILE);
-      atomicAdd(&p.ctl->overflow, 1ull);
+  const uint4 hdr = p.runs[(size_t)blockIdx.x * p.run_stride];
+  const unsigned os = hdr.w, nown = hdr.z >> 16;
+  const unsigned warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (!stage_cells<HAS_WALL>(p, T, hdr, p.pos[cur], img, sitems, shtab, hb)) {  // does not fit: empty lists, the passes skip the tile
+    for (unsigned t = threadIdx.x; t < nown; t += blockDim.x) {
+      if (MODE == 0) {
+        p.nnbr[os + t] = 0u;
+        p.self_loc[os + t] = 0;
+      } else {
+        p.nact[os + t] = 0;
+      }
     }
     return;
   }
-  if (warp == 0) write_tile_runs(p, T, sm, total, own_s, own_n);  // staging recipe of the per-step passes
+  for (unsigned k = threadIdx.x; k < LCAP + 8u; k += blockDim.x) lhist[k] = 0u;
+  __syncthreads();
   const int hxn = T.ex + 2, hyn = T.ey + 2;
-  // per-warp scratch behind the tables: hit masks [32 particle slots][MSTRIDE] and two candidate tables [MAXCAND]
-  unsigned* const masks = (unsigned*)(sm.queue + (size_t)warp * BUILD_SCRATCH16);
-  unsigned short* const tables = (unsigned short*)(masks + 32 * MSTRIDE);
-  // behind the warps' scratch: histogram of the list lengths, filled as the lengths become known, for the hand-out order
-  // of the density pass (counting sort at the end: one pass over the lengths instead of two)
-  unsigned* const lhist = (unsigned*)(sm.queue + (size_t)nwarps * BUILD_SCRATCH16);  // [LCAP + 1] (+ padding)
+  // work items: per own x-row, maximal groups of consecutive cells holding <= 32 particles (a fuller cell is its own item)
+  unsigned nitems_w = 0;
+  if (warp == 0) {
+    const int nrows = T.ey * T.ez;
+    unsigned gS[4], gN[4], gM[4];
+    unsigned ng = 0, g_row = 0, sb_row = 0;
+    if ((int)lane < nrows) {
+      const int hy = 1 + (int)lane % T.ey, hz = 1 + (int)lane / T.ey;
+      const int h0 = (hz * hyn + hy) * hxn + 1;
+      g_row = p.runs[(size_t)blockIdx.x * p.run_stride + 1 + (unsigned)(hz * hyn + hy) * 3u + 1u].x;
+      sb_row = hb[h0];
+      int a = 0;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        if (a < T.ex) {
+          int b = a;
+          unsigned n = (unsigned)hb[h0 + a + 1] - hb[h0 + a];
+          while (b + 1 < T.ex && n + ((unsigned)hb[h0 + b + 2] - hb[h0 + b + 1]) <= 32u) {
+            ++b;
+            n += (unsigned)hb[h0 + b + 1] - hb[h0 + b];
+          }
+          gS[k] = hb[h0 + a];
+          gN[k] = n;
+          gM[k] = (unsigned)a | ((unsigned)b << 8) | ((unsigned)hy << 16) | ((unsigned)hz << 24);
+          ng = (unsigned)k + 1u;
+          a = b + 1;
+        }
+      }
+    }
+    unsigned incl = ng;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const unsigned t = __shfl_up_sync(0xffffffffu, incl, o);
+      if ((int)lane >= o) incl += t;
+    }
+    nitems_w = __shfl_sync(0xffffffffu, incl, 31);
+    unsigned io = incl - ng;
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+      if ((unsigned)k < ng) witems[io + k] = make_uint4(gS[k], gN[k], g_row + (gS[k] - sb_row), gM[k]);
+    if (lane == 0) lhist[LCAP + 5] = nitems_w;
+  }
+  __syncthreads();
+  const unsigned nitems = lhist[LCAP + 5];
+  const unsigned rowcap = MODE ? p.cap_act : p.cap, row_bytes = MODE ? p.rows_direct : p.rows_verlet;
+  const float cut2 = (MODE ? p.rc2 : p.rlist2) + p.dot_margin;
   const unsigned sent = p.tile_cap;
+  const unsigned ibase = smem_addr(img);
+  const unsigned rbase = smem_addr(q) + (warp * 32u + lane) * row_bytes;  // this lane's row
+  const unsigned rp_lim = rbase + 2u * rowcap;
   unsigned smax = 0, ssum = 0;
   bool sover = false;
-  const int half = lane >> 4, hl = lane & 15;
-  for (unsigned oc0 = 2 * warp; oc0 < T.ncell_own; oc0 += 2 * nwarps) {
-    // the pair's cells: geometry of each (warp-uniform)
-    unsigned c_lb[2], c_n[2], c_gb[2], c_nch[2];
-#pragma unroll
-    for (int hh = 0; hh < 2; ++hh) {
-      const unsigned oc = oc0 + hh;
-      c_lb[hh] = c_n[hh] = c_gb[hh] = c_nch[hh] = 0;
-      if (oc < T.ncell_own) {
-        const int lx = oc % T.ex, ly = (oc / T.ex) % T.ey, lz = oc / (T.ex * T.ey);
-        const int hown = ((lz + 1) * hyn + (ly + 1)) * hxn + lx + 1;
-        c_lb[hh] = sm.hbase[hown];
-        c_n[hh] = sm.hbase[hown + 1] - c_lb[hh];
-        c_gb[hh] = c_lb[hh] + f2u(sm.hshift[hown].w);
+  float4* __restrict__ vel = p.vel[cur];
+  for (;;) {
+    unsigned it = 0;
+    if (lane == 0) it = atomicAdd(&lhist[LCAP + 4], 1u);
+    it = __shfl_sync(0xffffffffu, it, 0);
+    if (it >= nitems) break;
+    const uint4 Wk = witems[it];
+    const unsigned S0 = Wk.x, n = Wk.y, G0 = Wk.z;
+    const int ca = (int)(Wk.w & 255u), cb = (int)((Wk.w >> 8) & 255u), hy = (int)((Wk.w >> 16) & 255u), hz = (int)(Wk.w >> 24);
+    for (unsigned r0 = 0; r0 < n; r0 += 32u) {
+      const unsigned li = r0 + lane;
+      const bool active = li < n;
+      const unsigned self = S0 + li;
+      const float4 xi = img[active ? self : S0];
+      const float ax = -2.0f * xi.x, ay = -2.0f * xi.y, az = -2.0f * xi.z;
+      float bi = active ? fmaf(xi.z, xi.z, fmaf(xi.y, xi.y, xi.x * xi.x)) - cut2 : __int_as_float(0x7f800000);
+      unsigned rp = rbase;
+      bool over = false;
+      const unsigned lo = S0 + r0, hi = min(S0 + n, lo + 32u);  // this round's own particles among the candidates
+#pragma unroll 1
+      for (int qq = 0; qq < 9; ++qq) {
+        const int hrow = ((hz - 1 + qq / 3) * hyn + (hy - 1 + qq % 3)) * hxn + ca;  // halo x of cell ca - 1
+        const unsigned sb = hb[hrow], se = hb[hrow + (cb - ca + 3)];
+        if (qq == 4) {
+          scan_range<false>(ibase, sb, lo, ax, ay, az, bi, self, rp, rp_lim, over);
+          scan_range<true>(ibase, lo, hi, ax, ay, az, bi, self, rp, rp_lim, over);
+          scan_range<false>(ibase, hi, se, ax, ay, az, bi, self, rp, rp_lim, over);
+        } else {
+          scan_range<false>(ibase, sb, se, ax, ay, az, bi, self, rp, rp_lim, over);
+        }
       }
-    }
-    const unsigned rounds = (max(c_n[0], c_n[1]) + 15u) >> 4;  // 16 particle slots per cell and round
-    for (unsigned rd = 0; rd < rounds; ++rd) {
-      const unsigned b0 = rd * 16u;
-      // phase-2 state of the lane's particle; it persists over the candidate windows
-      const bool act = b0 + hl < (half ? c_n[1] : c_n[0]);
-      const unsigned self = (half ? c_lb[1] : c_lb[0]) + b0 + hl;
-      const unsigned gi = (half ? c_gb[1] : c_gb[0]) + b0 + hl;
-      uint4* out = p.nbr + gi;
-      unsigned a0 = 0, a1 = 0, a2 = 0, a3 = 0, n = 0;
-      bool more = true;
-      for (unsigned win = 0; more; win += MAXCAND) {  // windows of MAXCAND candidates (one window unless very dense)
-        more = false;
-        // ---------------- phase 1: hit masks of this round's particles, cell by cell ----------------
-#pragma unroll
-        for (int hh = 0; hh < 2; ++hh) {
-          c_nch[hh] = 0;
-          if (b0 >= c_n[hh]) continue;  // warp-uniform
-          const unsigned nb = min(16u, c_n[hh] - b0);
-          const unsigned oc = oc0 + hh;
-          const int lx = oc % T.ex, ly = (oc / T.ex) % T.ey, lz = oc / (T.ex * T.ey);
-          // the nine candidate runs: lane r < 9 holds run r = (dz, dy); inclusive scan of the run lengths
-          unsigned run_b = 0, run_n = 0;
-          if (lane < 9) {
-            const int hrow = ((lz + lane / 3) * hyn + (ly + lane % 3)) * hxn + lx;
-            run_b = sm.hbase[hrow];
-            run_n = sm.hbase[hrow + 3] - run_b;
-          }
-          unsigned incl = run_n;
-#pragma unroll
-          for (int o = 1; o < 16; o <<= 1) {
-            const unsigned t = __shfl_up_sync(0xffffffffu, incl, o);
-            if (lane >= o) incl += t;
-          }
-          const unsigned ncand = __shfl_sync(0xffffffffu, incl, 8);
-          if (win >= ncand) continue;  // this cell has no candidates left
-          const unsigned wend = min(ncand, win + MAXCAND);
-          if (wend < ncand) more = true;
-          c_nch[hh] = (wend - win + 31u) >> 5;
-          const unsigned run_o = incl - run_n;  // exclusive offset of the lane's run
-          unsigned rend[8];
-#pragma unroll
-          for (int r = 0; r < 8; ++r) rend[r] = __shfl_sync(0xffffffffu, incl, r);
-          unsigned short* const tb = tables + hh * MAXCAND;
-          unsigned* const mrow = masks + (hh * 16) * MSTRIDE;
-          for (unsigned sc = win; sc < wend; sc += 32 * SCH) {
-            float cx[SCH], cy[SCH], cz[SCH];
-#pragma unroll
-            for (int t = 0; t < SCH; ++t) {  // flat candidate index -> staged slot (past the end: the sentinel, never hit)
-              const unsigned f = sc + t * 32 + lane;
-              unsigned r = 0;
-#pragma unroll
-              for (int q = 0; q < 8; ++q) r += (f >= rend[q]) ? 1u : 0u;
-              const unsigned rb = __shfl_sync(0xffffffffu, run_b, r), ro = __shfl_sync(0xffffffffu, run_o, r);
-              const unsigned cs = f < wend ? rb + (f - ro) : sent;
-              if (f - win < MAXCAND) tb[f - win] = (unsigned short)cs;
-              const float4 xj = sm.spos[cs];
-              cx[t] = xj.x;
-              cy[t] = xj.y;
-              cz[t] = xj.z;
-            }
-            const unsigned ch0 = (sc - win) >> 5;
-            for (unsigned il = 0; il < nb; ++il) {
-              const float4 xi = sm.spos[c_lb[hh] + b0 + il];  // warp-uniform: broadcast
-              unsigned* const mr = mrow + il * MSTRIDE + ch0;
-#pragma unroll
-              for (int t = 0; t < SCH; ++t) {
-                const float dx = xi.x - cx[t], dy = xi.y - cy[t], dz = xi.z - cz[t];
-                const float r2 = dx * dx + dy * dy + dz * dz;
-                const unsigned b = __ballot_sync(0xffffffffu, r2 < p.rlist2);
-                if (lane == 0) mr[t] = b;
-              }
-            }
-          }
+      unsigned cnt = (rp - rbase) >> 1;
+      if (cnt > rowcap) over = true;
+      if (over) cnt = 0;  // reported as MDPD_EOVERFLOW; this particle's list is emptied
+      for (unsigned k = cnt; k & 7u; ++k) sts_u16(rbase + 2u * k, sent);  // pad the last chunk with the sentinel
+      __syncwarp();
+      const unsigned gi = G0 + li;
+      const unsigned nch = active ? (cnt + 7u) >> 3 : 0u;
+      if (MODE == 0) {
+        const unsigned wch = __reduce_max_sync(0xffffffffu, nch);
+        for (unsigned c = 0; c < wch; ++c)
+          if (c < nch) p.nbr[(size_t)c * p.N + gi] = lds4u(rbase + 16u * c);
+        if (active) {
+          p.nnbr[gi] = cnt;
+          p.self_loc[gi] = (unsigned short)self;
+          atomicAdd(&lhist[LCAP - min(cnt, LCAP)], 1u);
+          smax = max(smax, cnt);
+          ssum += cnt;
+          sover = sover || over;
+        }
+      } else {
+        const unsigned walli = HAS_WALL ? (f2u(xi.w) & 1u) : 0u;
+        float rho = 0.0f;
+        unsigned nin = 0;
+        for (unsigned c = 0; c < nch; ++c) {
+          const unsigned ka = rbase + 16u * c;
+          const uint4 e = lds4u(ka);
+          direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.x & 0xFFFFu, ka, sent, rho, nin);
+          direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.x >> 16, ka + 2u, sent, rho, nin);
+          direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.y & 0xFFFFu, ka + 4u, sent, rho, nin);
+          direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.y >> 16, ka + 6u, sent, rho, nin);
+          direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.z & 0xFFFFu, ka + 8u, sent, rho, nin);
+          direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.z >> 16, ka + 10u, sent, rho, nin);
+          direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.w & 0xFFFFu, ka + 12u, sent, rho, nin);
+          direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.w >> 16, ka + 14u, sent, rho, nin);
         }
         __syncwarp();
-        // ---------------- phase 2: lane = particle; decode the window's masks into the list ----------------
-        {
-          const unsigned nch = act ? (half ? c_nch[1] : c_nch[0]) : 0u;
-          const unsigned* const mr = masks + lane * MSTRIDE;
-          const unsigned short* const tb = tables + half * MAXCAND;
-          // one loop, two kinds of iteration: fetch the next mask word, or consume the lowest set bit of the current one
-          unsigned t = 0, w = 0;
-          unsigned left = nch;  // mask words not fetched yet
-          while (left | w) {
-            if (w == 0u) {
-              w = mr[t];
-              ++t;
-              --left;
-            } else {
-              const unsigned b = __ffs(w) - 1u;
-              w &= w - 1u;
-              const unsigned slot = tb[(t - 1u) * 32u + b];
-              if (slot != self) {
-                a0 = __funnelshift_r(a0, a1, 16);
-                a1 = __funnelshift_r(a1, a2, 16);
-                a2 = __funnelshift_r(a2, a3, 16);
-                a3 = __funnelshift_r(a3, slot, 16);
-                ++n;
-                if ((n & 7u) == 0u && n <= p.cap) {
-                  *out = make_uint4(a0, a1, a2, a3);
-                  out += p.N;
-                }
-              }
-            }
-          }
+        const unsigned wch = __reduce_max_sync(0xffffffffu, nch);
+        for (unsigned c = 0; c < wch; ++c)
+          if (c < nch) p.act[(size_t)c * p.N + gi] = lds4u(rbase + 16u * c);
+        if (active) {
+          p.nact[gi] = (unsigned short)cnt;
+          vel[gi].w = rho * p.Krho;
+          const unsigned fy = (HAS_WALL && !ALL && walli) ? 0x80000000u : cnt;  // frozen: force not needed (R8)
+          p.dinfo[gi] = make_uint2((gi - os) | (self << 16), fy);             // unsorted; the tail below orders them
+          atomicAdd(&lhist[LCAP - min(fy & 0x7FFFFFFFu, LCAP)], 1u);
+          ssum += nin;
+          sover = sover || over;
         }
-        __syncwarp();
       }
-      if ((n & 7u) && n <= p.cap) {  // last, partial chunk: pad with the sentinel
-        for (unsigned q = n & 7u; q < 8u; ++q) {
-          a0 = __funnelshift_r(a0, a1, 16);
-          a1 = __funnelshift_r(a1, a2, 16);
-          a2 = __funnelshift_r(a2, a3, 16);
-          a3 = __funnelshift_r(a3, sent, 16);
-        }
-        *out = make_uint4(a0, a1, a2, a3);
-      }
-      if (act) {
-        if (n > p.cap) {  // reported as MDPD_EOVERFLOW; this particle's list is emptied
-          sover = true;
-          n = 0;
-        }
-        p.nnbr[gi] = n;
-        p.self_loc[gi] = (unsigned short)self;
-        atomicAdd(&lhist[LCAP - min(n, LCAP)], 1u);  // bin 0 = longest
-        smax = max(smax, n);
-        ssum += n;
-      }
+      __syncwarp();
     }
   }
-  // hand-out order of the density pass: own particles by decreasing list length (uses the now dead hbase table)
-  // statistics of the tile: per warp into shared memory (lhist[LCAP + 1 ..]), one set of global atomics per CTA
+  // statistics of the tile: per warp into shared memory, one set of global atomics per CTA
   smax = __reduce_max_sync(0xffffffffu, smax);
   ssum = __reduce_add_sync(0xffffffffu, ssum);
   const unsigned wover = __any_sync(0xffffffffu, sover);
   if (lane == 0) {
     atomicMax(&lhist[LCAP + 1], smax);
     atomicAdd(&lhist[LCAP + 2], ssum);
-    if (wover) atomicOr(&lhist[LCAP + 1], 0x80000000u);
+    if (wover) atomicOr(&lhist[LCAP + 3], 1u);
   }
-  {  // the histogram is complete: scan it, then scatter the records (lengths and own slots were just written: L1 / L2)
-    __syncthreads();
-    if (threadIdx.x == 0) {
-      Ctl* c = p.ctl;
-      const unsigned mx = lhist[LCAP + 1];
-      atomicMax(&c->max_nbr, mx & 0x7FFFFFFFu);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    Ctl* c = p.ctl;
+    if (MODE == 0) {
+      atomicMax(&c->max_nbr, lhist[LCAP + 1]);
       atomicAdd(&c->sum_nbr, (unsigned long long)lhist[LCAP + 2]);
-      if (mx >> 31) {
-        atomicOr(&c->err, ERR_OVERFLOW);
-        atomicAdd(&c->overflow, 1ull);
-      }
+    } else {
+      atomicAdd(&c->sum_act, (unsigned long long)lhist[LCAP + 2]);
+      if (blockIdx.x == 0) atomicAdd(&c->dens_passes, 1ull);
     }
-    if (threadIdx.x < 32) {  // exclusive scan of the LCAP + 1 bins by warp 0
-      unsigned run = 0;
-      for (unsigned b0 = 0; b0 <= LCAP; b0 += 32) {
-        const unsigned k = b0 + lane;
-        const unsigned c = k <= LCAP ? lhist[k] : 0u;
-        unsigned incl = c;
+    if (lhist[LCAP + 3]) {
+      atomicOr(&c->err, ERR_OVERFLOW);
+      atomicAdd(&c->overflow, 1ull);
+    }
+  }
+  // Hand-out order of the pass that follows (MODE 0: the density pass, by decreasing list length; MODE 1: the force pass,
+  // by decreasing in-range count): counting sort in shared memory, the histogram was filled on the fly.  Group g =
+  // sorted particles 32 g .. 32 g + 31 (the lanes of a warp finish together); warp w takes the groups w, 2W-1-w, 2W+w,
+  // ... (a long group, then a short one: the warps of a CTA finish together).  Which thread evaluates which particle
+  // changes no result.
+  if (threadIdx.x < 32) {  // exclusive scan of the LCAP + 1 bins by warp 0
+    unsigned run = 0;
+    for (unsigned b0 = 0; b0 <= LCAP; b0 += 32) {
+      const unsigned k = b0 + lane;
+      const unsigned c = k <= LCAP ? lhist[k] : 0u;
+      unsigned incl = c;
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-          const unsigned v = __shfl_up_sync(0xffffffffu, incl, o);
-          if (lane >= o) incl += v;
-        }
-        if (k <= LCAP) lhist[k] = run + incl - c;
-        run += __shfl_sync(0xffffffffu, incl, 31);
+      for (int o = 1; o < 32; o <<= 1) {
+        const unsigned v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= (unsigned)o) incl += v;
       }
+      if (k <= LCAP) lhist[k] = run + incl - c;
+      run += __shfl_sync(0xffffffffu, incl, 31);
     }
-    __syncthreads();
-    uint2* __restrict__ dout = p.dinfo + own_s;
-    for (unsigned t = threadIdx.x; t < own_n; t += blockDim.x) {
-      const unsigned n = p.nnbr[own_s + t];
-      dout[atomicAdd(&lhist[LCAP - min(n, LCAP)], 1u)] = make_uint2(t | ((unsigned)p.self_loc[own_s + t] << 16), n);
+  }
+  __syncthreads();
+  if (MODE == 0) {
+    uint2* __restrict__ dout = p.dinfo + os;
+    for (unsigned t = threadIdx.x; t < nown; t += blockDim.x) {
+      const unsigned n = p.nnbr[os + t];
+      dout[atomicAdd(&lhist[LCAP - min(n, LCAP)], 1u)] = make_uint2(t | ((unsigned)p.self_loc[os + t] << 16), n);
+    }
+  } else {
+    uint2* __restrict__ fout = p.finfo + os;
+    for (unsigned t = threadIdx.x; t < nown; t += blockDim.x) {
+      const uint2 d = p.dinfo[os + t];
+      fout[atomicAdd(&lhist[LCAP - min(d.y & 0x7FFFFFFFu, LCAP)], 1u)] = d;
     }
   }
 }
 
-__global__ void k_reset_list_stats(const DevP p) {
-  if (!p.ctl->rebuild) return;
+__global__ void k_reset_list_stats(const DevP p, int always, int tiles) {
+  if (!always && !p.ctl->rebuild) return;
   p.ctl->max_nbr = 0;
   p.ctl->sum_nbr = 0;
-  p.ctl->max_halo = 0;
-  p.ctl->max_own = 0;
+  if (tiles) {
+    p.ctl->max_halo = 0;
+    p.ctl->max_own = 0;
+  }
 }
 
 // ----------------------------------------------------------------------------------------------------------------
@@ -1313,9 +1442,6 @@ __global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
   const TileSmem sm = carve_smem(smraw, p.tile_cap, true);
   const unsigned cur = p.ctl->cur;
   const TileInfo T = p.tiles[blockIdx.x];
-#ifdef MDPD_PHASES
-  const long long ph_t0 = clock64();
-#endif
   const uint4 hdr = p.runs[(size_t)blockIdx.x * p.run_stride];
   const unsigned os = hdr.w, nown = hdr.z >> 16;
   const unsigned warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
@@ -1334,9 +1460,6 @@ __global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
   for (int r = 0; r < PRE; ++r)
     head[r] = (info[r].y & 0x7FFFFFFFu) ? p.act[os + (info[r].x & 0xFFFFu)] : make_uint4(sentw, sentw, sentw, sentw);
   if (!stage_fast<true>(p, T, hdr, p.pos[cur], p.vel[cur], sm)) return;
-#ifdef MDPD_PHASES
-  const long long ph_t1 = clock64();
-#endif
   HashKeys K = make_keys(p.ctl->step, p.seed);
 #pragma unroll
   for (int q = 0; q < 6; ++q) K.k[q] = pin(K.k[q]);
@@ -1401,15 +1524,6 @@ __global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
       if (lane == 0 && v != 0.0) atomicAdd(&p.ctl->vir[q], v);
     }
   }
-#ifdef MDPD_PHASES
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    const long long ph_t3 = clock64();
-    atomicAdd(&p.ctl->ph[0], (unsigned long long)(ph_t1 - ph_t0));
-    atomicAdd(&p.ctl->ph[2], (unsigned long long)(ph_t3 - ph_t1));
-    atomicAdd(&p.ctl->ph[3], 1ull);
-  }
-#endif
 }
 
 // ----------------------------------------------------------------------------------------------------------------
@@ -1493,7 +1607,7 @@ inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 struct Layout {
   size_t pos[2], vel[2], force, xbuild, cell_rank, cell_count, cell_start, scan_bsum, pcell, order, nbr,
       act, nact, nnbr, self_loc, tiles, runs, dperm, fperm, mask, ctl, stage, total;
-  unsigned ncx, ncy, ncz, ncell, cap, scan_blocks;
+  unsigned ncx, ncy, ncz, ncell, cap, cap_act, scan_blocks;
   float rlist;
 };
 
@@ -1526,6 +1640,10 @@ bool make_layout(const mdpd_params& p, uint64_t n, int has_mask, const uint32_t*
   if (p.max_neigh == 0) L.cap = std::min<unsigned>(LCAP, (unsigned)(std::ceil((m_list + 6.0 * std::sqrt(m_list) + 8.0) / 8.0) * 8.0));
   else L.cap = (p.max_neigh + 7u) / 8u * 8u;
   if (L.cap > LCAP) return fail("max_neigh must be <= 128 (the list build assembles a particle's list in shared memory)");
+  {  // capacity of the per-step in-range (r < rc) lists of the list-free path
+    const double m_act = 4.0 / 3.0 * PI * std::pow((double)p.rc, 3) * dens;
+    L.cap_act = std::min<unsigned>(L.cap, (unsigned)(std::ceil((m_act + 6.0 * std::sqrt(m_act) + 8.0) / 8.0) * 8.0));
+  }
   L.scan_blocks = (L.ncell + SCAN_TILE - 1) / SCAN_TILE;
   const size_t N = (size_t)std::max<uint64_t>(n, 1);
   size_t off = 0;
@@ -1551,7 +1669,7 @@ bool make_layout(const mdpd_params& p, uint64_t n, int has_mask, const uint32_t*
   L.nnbr = take(N * 4);
   L.self_loc = take(N * 2);
   L.tiles = take((size_t)L.ncell * sizeof(TileInfo));  // worst case: one cell per tile
-  L.runs = take(((size_t)L.ncell * 28 + 4096) * 16);   // worst case: one cell per tile, 1 + 27 records each
+  L.runs = take(((size_t)L.ncell * 32 + 4096) * 16);   // worst case: one cell per tile: header + 27 records + 4 (slot table)
   L.dperm = take(N * 8);
   L.fperm = take(N * 8);
   L.stage = take(N * 40 + 64);  // load/unload staging: pos, vel, force [n][3] + rho [n] (+ type at load)
@@ -1598,8 +1716,11 @@ struct mdpd_ctx {
   int tile_dim[3] = {4, 4, 4};
   unsigned block = 256;          // threads per CTA of the force pass
   unsigned block_dens = 256;     // threads per CTA of the density pass
-  unsigned block_build = 256;    // threads per CTA of the list build
-  size_t smem_pos = 0, smem_posvel = 0, smem_build = 0;
+  unsigned cells_warps[2] = {4, 4};  // warps per CTA of k_cells (list build / list-free pass)
+  size_t smem_cells[2] = {0, 0};
+  bool direct = false;           // MDPD_FLAG_DIRECT: no Verlet list, neighbours straight from the cells every step
+  unsigned chain_launches = 9;   // kernels of the rebuild chain
+  size_t smem_pos = 0, smem_posvel = 0;
   size_t smem_limit = 0;         // cudaDevAttrMaxSharedMemoryPerBlockOptin
   std::string err;
   Ctl* h_ctl = nullptr;  // pinned
@@ -1631,10 +1752,10 @@ int set_err(mdpd_ctx* h, int code, const char* fmt, ...) {
 
 inline unsigned nblk(uint64_t n, int tpb) { return (unsigned)((n + tpb - 1) / tpb); }
 
-enum ProfSlot { PS_INTEGRATE = 0, PS_CELL_COUNT, PS_SCAN, PS_CELL_FILL, PS_PERMUTE, PS_BUILD_LIST, PS_DENSITY, PS_FORCE,
-                PS_OTHER, PS_COUNT };
-const char* const kProfNames[PS_COUNT] = {"k_integrate", "k_cell_count", "k_scan", "k_cell_fill", "k_permute",
-                                          "k_build_list", "k_density", "k_force", "other"};
+enum ProfSlot { PS_INTEGRATE = 0, PS_CELL_COUNT, PS_SCAN, PS_CELL_FILL, PS_PERMUTE, PS_RECIPE, PS_CELLS_LIST, PS_CELLS_DIRECT,
+                PS_DENSITY, PS_FORCE, PS_OTHER, PS_COUNT };
+const char* const kProfNames[PS_COUNT] = {"k_integrate", "k_cell_count", "k_scan", "k_cell_fill", "k_permute", "k_tile_recipe",
+                                          "k_cells_list", "k_cells_direct", "k_density", "k_force", "other"};
 
 cudaEvent_t prof_event(mdpd_ctx* h) {
   cudaEvent_t e = nullptr;
@@ -1766,26 +1887,40 @@ void build_tile_ranks(const Layout& L, const int tdim[3], std::vector<unsigned>&
   }
 }
 
+// k_cells: mode 0 = Verlet list build, mode 1 = the list-free per-step pass (rho, compact list, hand-out of the force pass)
+int launch_cells(mdpd_ctx* h, int mode, bool all, int always) {
+  const DevP& d = h->d;
+  const unsigned tpb = h->cells_warps[mode] * 32u;
+  const size_t sm = h->smem_cells[mode];
+  if (mode == 0) LAUNCH(h, PS_CELLS_LIST, (k_cells<0, false, false><<<d.ntiles, tpb, sm, h->ls>>>(d, always)));
+  else if (!h->has_wall) LAUNCH(h, PS_CELLS_DIRECT, (k_cells<1, false, false><<<d.ntiles, tpb, sm, h->ls>>>(d, always)));
+  else if (all) LAUNCH(h, PS_CELLS_DIRECT, (k_cells<1, true, true><<<d.ntiles, tpb, sm, h->ls>>>(d, always)));
+  else LAUNCH(h, PS_CELLS_DIRECT, (k_cells<1, true, false><<<d.ntiles, tpb, sm, h->ls>>>(d, always)));
+  return MDPD_OK;
+}
+
+// sort + tile recipe [+ Verlet list]: with_list = false at load time, while the tile shape is probed
 int launch_rebuild_chain(mdpd_ctx* h, bool with_list = true) {
   const DevP& d = h->d;
   // grid-stride kernels on a grid of a few waves: a step whose trigger did not fire pays ~nothing for them
   const unsigned nb = std::min(nblk(h->n, TPB), 148u * 16u);
   cudaStream_t s = h->ls;
-  LAUNCH(h, PS_OTHER, (k_reset_list_stats<<<1, 1, 0, s>>>(d)));
+  LAUNCH(h, PS_OTHER, (k_reset_list_stats<<<1, 1, 0, s>>>(d, 0, 1)));
   LAUNCH(h, PS_CELL_COUNT, (k_cell_count<<<nb, TPB, 0, s>>>(d)));
   LAUNCH(h, PS_SCAN, (k_scan_local<<<h->L.scan_blocks, SCAN_TPB, 0, s>>>(d)));
   LAUNCH(h, PS_SCAN, (k_scan_bsum<<<1, 1024, 0, s>>>(d, h->L.scan_blocks)));
   LAUNCH(h, PS_SCAN, (k_scan_add<<<h->L.scan_blocks, SCAN_TPB, 0, s>>>(d)));
   LAUNCH(h, PS_CELL_FILL, (k_cell_fill<<<nb, TPB, 0, s>>>(d)));
   LAUNCH(h, PS_PERMUTE, (k_permute<<<nb, TPB, 0, s>>>(d)));
-  if (!with_list) LAUNCH(h, PS_OTHER, (k_tile_stats<<<nblk((uint64_t)d.ntiles * 32, 128), 128, 0, s>>>(d)));
-  if (with_list) LAUNCH(h, PS_BUILD_LIST, (k_build_list<<<d.ntiles, h->block_build, h->smem_build, s>>>(d)));
+  LAUNCH(h, PS_RECIPE, (k_tile_recipe<<<d.ntiles, 128, 0, s>>>(d, with_list ? 1 : 0)));
+  if (with_list && !h->direct) launch_cells(h, 0, false, 0);
   return MDPD_OK;
 }
 
 int launch_forces(mdpd_ctx* h, bool all, bool virial = false) {
   const DevP& d = h->d;
-  if (!h->has_wall) LAUNCH(h, PS_DENSITY, (k_density<false, false><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
+  if (h->direct) launch_cells(h, 1, all, 1);
+  else if (!h->has_wall) LAUNCH(h, PS_DENSITY, (k_density<false, false><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
   else if (all) LAUNCH(h, PS_DENSITY, (k_density<true, true><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
   else LAUNCH(h, PS_DENSITY, (k_density<true, false><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
   if (d.s_exp != 1.0f) {  // general exponent of wR: one material, no virial (checked by the callers)
@@ -1919,7 +2054,6 @@ int mdpd_create(mdpd_ctx** out, int device, void* cuda_stream) {
   h->device = device;
   h->stream = (cudaStream_t)cuda_stream;
   h->ls = h->stream;
-  if (const char* e = getenv("MDPD_NO_GRAPH")) h->use_graph = !(e[0] && e[0] != '0');
   if (cudaMallocHost((void**)&h->h_ctl, sizeof(Ctl)) != cudaSuccess ||
       cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
     if (h->h_ctl) cudaFreeHost(h->h_ctl);
@@ -1960,8 +2094,9 @@ int mdpd_set_params(mdpd_ctx* h, const mdpd_params* p) {
   if (h->loaded) {
     const mdpd_params& q = h->prm;
     if (memcmp(q.box, p->box, sizeof q.box) || q.rc != p->rc || q.rd != p->rd || q.skin != p->skin ||
-        q.max_neigh != p->max_neigh || q.mass != p->mass || q.headroom != p->headroom)
-      return set_err(h, MDPD_ESTATE, "box, cut-offs, skin, mass and capacities are frozen after load_particles");
+        q.max_neigh != p->max_neigh || q.mass != p->mass || q.headroom != p->headroom ||
+        ((q.flags ^ p->flags) & MDPD_FLAG_DIRECT))
+      return set_err(h, MDPD_ESTATE, "box, cut-offs, skin, mass, capacities and the neighbour path are frozen after load_particles");
     if (h->pending_B) {  // the outstanding half kick belongs to the old parameters
       CU_TRY(h, cudaSetDevice(h->device));
       finalize_kick(h);
@@ -2063,34 +2198,42 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
     if (type) CU_TRY(h, cudaMemcpyAsync(stype, type, n, cudaMemcpyDefault, h->stream));
     LAUNCH(h, PS_OTHER, (k_pack<<<nblk(n, TPB), TPB, 0, h->stream>>>(h->d, spos, svel, type ? stype : nullptr, 0u)));
   }
+  h->direct = (h->prm.flags & MDPD_FLAG_DIRECT) != 0;
+  h->chain_launches = h->direct ? 8u : 9u;  // reset, count, 3 x scan, fill, permute, recipe [, list]
   // Tile shape: the largest candidate that still gives every SM work and whose most populated tile + halo fits in
-  // shared memory (checked on the device after the sort); MDPD_TILE="tx,ty,tz" / MDPD_BLOCK override for experiments.
+  // shared memory (checked on the device after the sort).
   static const int kCand[][3] = {{4, 4, 4}, {4, 4, 2}, {4, 2, 2}, {2, 2, 2}, {2, 2, 1}, {2, 1, 1}, {1, 1, 1}};
   const int ncand = (int)(sizeof kCand / sizeof kCand[0]);
   int first = 0;
-  int forced[3] = {0, 0, 0};
-  if (const char* e = getenv("MDPD_TILE")) sscanf(e, "%d,%d,%d", &forced[0], &forced[1], &forced[2]);
-  const bool force_tile = forced[0] >= 1 && forced[0] <= 4 && forced[1] >= 1 && forced[1] <= 4 && forced[2] >= 1 && forced[2] <= 4;
-  if (!force_tile) {
+  {
     auto ntiles_of = [&](const int* t) {
       return (size_t)((L.ncx + t[0] - 1) / t[0]) * ((L.ncy + t[1] - 1) / t[1]) * ((L.ncz + t[2] - 1) / t[2]);
     };
     while (first < 3 && ntiles_of(kCand[first]) < 148) ++first;  // small boxes: down to 2 x 2 x 2
   }
   for (int ci = first; ci < ncand; ++ci) {
-    const int* cand = force_tile ? forced : kCand[ci];
+    const int* cand = kCand[ci];
     int tdim[3] = {std::min<int>(cand[0], (int)L.ncx), std::min<int>(cand[1], (int)L.ncy), std::min<int>(cand[2], (int)L.ncz)};
     std::vector<unsigned> rank;
     std::vector<TileInfo> tiles;
     build_tile_ranks(L, tdim, rank, tiles);
     memcpy(h->tile_dim, tdim, sizeof tdim);
     h->d.ntiles = (unsigned)tiles.size();
-    h->d.run_stride = 1u + 3u * (unsigned)((tdim[1] + 2) * (tdim[2] + 2));
-    if ((size_t)h->d.ntiles * h->d.run_stride > (size_t)L.ncell * 28 + 4096)
-      return set_err(h, MDPD_ENOMEM, "tile run table does not fit its reservation");
-    const int vol = tdim[0] * tdim[1] * tdim[2];
+    h->d.nrun_max = 3u * (unsigned)((tdim[1] + 2) * (tdim[2] + 2));
+    h->d.hb_off = 1u + h->d.nrun_max;
+    h->d.run_stride = h->d.hb_off + ((unsigned)((tdim[0] + 2) * (tdim[1] + 2) * (tdim[2] + 2)) + 1u + 7u) / 8u;
+    if ((size_t)h->d.ntiles * h->d.run_stride > (size_t)L.ncell * 32 + 4096)
+      return set_err(h, MDPD_ENOMEM, "tile recipe table does not fit its reservation");
     h->block = TILE_TPB;  // upper bound while the capacity is probed; set from the tile population below
-    h->block_build = vol >= 64 ? BUILD_TPB : (vol >= 32 ? std::min(256, BUILD_TPB) : 128u);
+    {  // slack of k_cells' approximate range test: its rounding error grows with the square of the centred coordinates
+      double x2 = 0.0;
+      for (int k = 0; k < 3; ++k) {
+        const double edge = (double)h->prm.box[k] / (double)(k == 0 ? L.ncx : (k == 1 ? L.ncy : L.ncz));
+        const double x = 0.5 * tdim[k] * edge + edge + 0.5 * (double)h->prm.skin + 1.0 / 32.0;
+        x2 += x * x;
+      }
+      h->d.dot_margin = (float)(6e-6 * x2);
+    }
     const size_t fixed = tile_smem_bytes(0, true, 0);
     // capacity of a tile + halo in staged slots: what the force pass can hold in shared memory, what a 16-bit list entry can
     // address, and what the item list of stage_fast (2 * HTAB items: 3 * 36 runs + one item per 32 slots) can describe
@@ -2109,7 +2252,7 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
     const unsigned max_halo = h->h_ctl->max_halo;
     const double headroom = h->prm.headroom > 0.0f ? std::max(1.0, (double)h->prm.headroom) : 1.15;  // mdpd_params.headroom
     if ((double)max_halo * headroom > (double)cap_limit) {
-      if (force_tile || ci + 1 == ncand)
+      if (ci + 1 == ncand)
         return set_err(h, MDPD_EOVERFLOW, "a tile of %d x %d x %d cells plus halo holds %u particles (x head-room %.2f); shared memory fits %u",
                        tdim[0], tdim[1], tdim[2], max_halo, headroom, cap_limit);
       continue;  // try the next smaller tile shape
@@ -2119,14 +2262,6 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
     const unsigned half_own = ((h->h_ctl->max_own + 1u) / 2u + 31u) / 32u * 32u;
     h->block = std::min<unsigned>(TILE_TPB, std::max(64u, half_own));
     h->block_dens = std::min<unsigned>(DENS_TPB, std::max(64u, half_own));
-    if (const char* e = getenv("MDPD_BLOCK")) {
-      int b = atoi(e);
-      if (b >= 32 && b <= TILE_TPB && b % 32 == 0) h->block = (unsigned)b;
-    }
-    if (const char* e = getenv("MDPD_BLOCK_BUILD")) {
-      int b = atoi(e);
-      if (b >= 32 && b <= BUILD_TPB && b % 32 == 0) h->block_build = (unsigned)b;
-    }
     // head-room for density fluctuations between rebuilds of a long run
     {
       // at least `headroom` (default 15 %) over the fullest tile of the initial state; beyond that, all the shared memory that does not
@@ -2142,10 +2277,24 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
   }
   h->smem_pos = tile_smem_bytes(h->d.tile_cap, false, 0);
   h->smem_posvel = tile_smem_bytes(h->d.tile_cap, true, 0);
-  h->smem_build = tile_smem_bytes(h->d.tile_cap, false, (size_t)BUILD_SCRATCH16 * (h->block_build / 32)) +
-                  4 * (size_t)BUILD_HIST;  // + the list-length histogram
-  if (h->smem_build > h->smem_limit) return set_err(h, MDPD_ENOMEM, "list build needs %zu bytes of shared memory", h->smem_build);
-  CU_TRY(h, cudaFuncSetAttribute(k_build_list, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_build));
+  // k_cells: the staged image plus one row buffer (32 rows) per warp; as many warps as two resident CTAs per SM allow
+  h->d.cap_act = L.cap_act;
+  h->d.rows_verlet = cells_row_bytes(h->d.cap);
+  h->d.rows_direct = cells_row_bytes(h->d.cap_act);
+  for (int mode = 0; mode < 2; ++mode) {
+    const size_t rowb = 32 * (size_t)(mode ? h->d.rows_direct : h->d.rows_verlet);
+    const size_t base = cells_smem_bytes(h->d.tile_cap, 0, 0);
+    const size_t two = (h->smem_limit + 1024) / 2 - 1024;  // per CTA when two are resident
+    size_t nw = two > base ? (two - base) / rowb : 0;
+    if (nw < 4) nw = h->smem_limit > base ? (h->smem_limit - base) / rowb : 0;  // one resident CTA
+    if (nw < 1) return set_err(h, MDPD_ENOMEM, "k_cells: the staged tile and one row buffer do not fit in shared memory");
+    h->cells_warps[mode] = (unsigned)std::min<size_t>(nw, CELLS_MAXW);
+    h->smem_cells[mode] = base + h->cells_warps[mode] * rowb;
+  }
+  CU_TRY(h, (cudaFuncSetAttribute(k_cells<0, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_cells[0])));
+  CU_TRY(h, (cudaFuncSetAttribute(k_cells<1, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_cells[1])));
+  CU_TRY(h, (cudaFuncSetAttribute(k_cells<1, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_cells[1])));
+  CU_TRY(h, (cudaFuncSetAttribute(k_cells<1, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_cells[1])));
   CU_TRY(h, cudaFuncSetAttribute(k_density<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
   CU_TRY(h, cudaFuncSetAttribute(k_density<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
   CU_TRY(h, cudaFuncSetAttribute(k_density<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
@@ -2159,7 +2308,9 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
   CU_TRY(h, (cudaFuncSetAttribute(k_force<true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel)));
   CU_TRY(h, cudaFuncSetAttribute(k_force<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
   if (n) {
-    LAUNCH(h, PS_BUILD_LIST, (k_build_list<<<h->d.ntiles, h->block_build, h->smem_build, h->stream>>>(h->d)));
+    // the recipe again, now against the final capacity (a tile that does not fit is flagged), then the list and the forces
+    LAUNCH(h, PS_RECIPE, (k_tile_recipe<<<h->d.ntiles, 128, 0, h->stream>>>(h->d, 1)));
+    if (!h->direct) launch_cells(h, 0, false, 1);
     launch_forces(h, true);
   }
   h->loaded = true;
@@ -2312,12 +2463,11 @@ int mdpd_get_counters(mdpd_ctx* h, uint64_t out[MDPD_NCOUNTERS]) {
   out[4] = c->sum_nbr;
   out[5] = c->max_halo;
   out[6] = c->overflow + c->nan_events;
-  out[7] = h->launches + 3 * h->graph_steps + 8 * c->graph_rebuilds;  // a graph replay launches 3 kernels (+ 8 on a rebuild)
+  out[7] = h->launches + 3 * h->graph_steps + h->chain_launches * c->graph_rebuilds;  // a graph replay launches 3 kernels (+ the rebuild chain)
   out[8] = c->sum_act;
   out[9] = c->dens_passes;
   out[10] = (uint64_t)h->tile_dim[0] | ((uint64_t)h->tile_dim[1] << 8) | ((uint64_t)h->tile_dim[2] << 16);
   out[11] = h->d.ntiles;
-  for (int k = 0; k < 4; ++k) out[12 + k] = c->ph[k];  // zero unless built with -DMDPD_PHASES
   return rc;
 }
 
@@ -2340,6 +2490,10 @@ int mdpd_get_pairs(mdpd_ctx* h, float rcut, uint64_t* count, uint32_t* pairs, ui
     }
   }
   cudaMemsetAsync(dcnt, 0, 8, h->stream);
+  if (h->direct) {  // the list-free path keeps no Verlet list: build one from the current cells for this call
+    LAUNCH(h, PS_OTHER, (k_reset_list_stats<<<1, 1, 0, h->stream>>>(h->d, 1, 0)));
+    launch_cells(h, 0, false, 1);
+  }
   LAUNCH(h, PS_OTHER, (k_pairs<<<h->d.ntiles, h->block, h->smem_pos, h->stream>>>(h->d, rcut * rcut, dout, cap, dcnt)));
   unsigned long long c = 0;
   cudaMemcpyAsync(&c, dcnt, 8, cudaMemcpyDeviceToHost, h->stream);
