@@ -820,32 +820,44 @@ __device__ __forceinline__ unsigned group_of_round(unsigned r, unsigned warp, un
 //   MODE 1  the list-free path (mdpd_params.flags & MDPD_FLAG_DIRECT): every step, the in-range (r < rc) lists of
 //           the step straight from the 27-cell stencil, the density pass over them, and the hand-out of the force pass.
 //
-// Orientation: LANE = own particle, the candidate is BROADCAST.  A warp takes a group of consecutive own cells of one
-// x-row of the tile holding at most 32 particles (one per lane); the candidates of the whole group are nine contiguous
-// runs of the staged image (the (y, z) rows of the stencil, from one cell left of the group to one cell right of
-// it).  The staged image holds, per slot, (x, y, z, -|x|^2) in tile-CENTRED coordinates, so the range test of candidate
-// c against the lane's particle is the dot-product form
-//     |xi|^2 - cut^2 - 2 xi . xc  <  -|xc|^2        (3 FFMA + 1 compare; one uniform 16-byte shared-memory load),
+// Orientation: LANE = CANDIDATE, the own particle is broadcast.  A warp takes a pair of x-adjacent own cells, one cell
+// at a time.  The candidates of a cell (the particles of its 27-cell stencil: nine contiguous runs of the staged image,
+// one per (y, z) row of halo cells) are flattened and held IN REGISTERS, 32 per chunk, up to CHMAX chunks at a time:
+// per candidate (x, y, z, |x|^2) in tile-CENTRED coordinates and its staged slot.  The warp then loops over the cell's
+// own particles: one uniform 16-byte shared-memory load of x_i (amortised over all chunks), and per chunk the range test
+// in dot-product form
+//     |xc|^2 - 2 xi . xc  <  cut^2 - |xi|^2          (3 FFMA + 1 compare per 32 candidates),
 // evaluated with a slack `dot_margin` on cut^2 that covers its rounding error (|x| <= ~4 in centred coordinates): the
-// hits are a SUPERSET of the exact r^2 < cut^2 set.  A hit costs one predicated 16-bit store of the candidate's
-// staged slot into the lane's row of a per-warp buffer in shared memory and one predicated pointer increment: no
-// ballots, no mask decoding, no compaction, and entries come out in increasing staged-slot order (deterministic).
+// hits are a SUPERSET of the exact r^2 < cut^2 set.  The hits of a chunk go straight into the particle's row of a
+// per-warp row buffer in shared memory: ballot, rank of the lane among the hits (popc of the ballot below the lane),
+// one predicated 16-bit store of the candidate's slot.  No hit masks, no decoding pass; entries come out in increasing
+// candidate (= staged-slot) order: deterministic.  (A first version with LANE = own particle and the candidate
+// broadcast had an even simpler loop but is bound by the 512 bytes every warp-wide 16-byte load returns to the
+// registers: 13.1 ms against 11.4 ms of round 1's kernel on config 4a; profiles/r2_cells.md.)
+// When the rows of the pair are complete, lane = row:
 // MODE 0 copies the rows to the list (16-byte chunks, layout [chunk][particle]: consecutive lanes write consecutive
-// particles).  MODE 1 then walks its row per lane with the EXACT fp32 distance (same arithmetic as k_density):
-// density sum over r < rd, entries that fail 1e-12 < r^2 < rc^2 exactly (slack hits, coincident particles R10,
-// frozen-frozen pairs R8) are replaced by the far-away sentinel slot, and the row becomes the step's compact list.
+// particles).  MODE 1 walks its row with the EXACT fp32 distance (same arithmetic as k_density): density sum over
+// r < rd; entries that fail 1e-12 < r^2 < rc^2 exactly (slack hits, coincident particles R10, frozen-frozen pairs R8)
+// are replaced by the far-away sentinel slot, and the row becomes the step's compact list.
 // ----------------------------------------------------------------------------------------------------------------
-constexpr int CELLS_MAXW = 12;       // most warps per CTA
-constexpr unsigned ROW_SLACK = 16;   // a full row is noticed within this many candidates
-constexpr unsigned CELLS_ITEMS = 64; // work items per tile: at most one per own cell
+#ifndef CELLS_W0
+#define CELLS_W0 8
+#endif
+constexpr int CELLS_MAXW0 = CELLS_W0;  // most warps per CTA of the list build (two resident CTAs: 65536 / (64 W) registers per thread)
+constexpr int CELLS_MAXW = 8;          // ... of the list-free pass
+constexpr int CHMAX = 12;             // candidate chunks (of 32) held in registers at a time: one window
+constexpr unsigned ROW_SLACK = 40;    // row capacity beyond the list capacity: the saturated count (cap + 1) plus one chunk's worth of hits
+constexpr unsigned CELLS_ITEMS = 64;  // work items per tile: at most one per own cell
 
 __host__ __device__ inline unsigned cells_row_bytes(unsigned rowcap) {
   unsigned b = 2u * (rowcap + ROW_SLACK) + 16u;  // + one chunk of sentinel padding
   if (((b >> 4) & 1u) == 0u) b += 16u;           // odd number of 16-byte groups: 16-byte row reads of consecutive lanes do not collide
   return b;
 }
-__host__ __device__ inline size_t cells_smem_bytes(unsigned tile_cap, unsigned row_bytes, unsigned nwarps) {
-  return (size_t)(tile_cap + 1) * 16 + HTAB * 16 + HTAB * 4 + HTAB * 2 + (size_t)nwarps * 32 * row_bytes;
+constexpr unsigned CELLS_ROW0_BYTES = 32 * CHMAX * 2 + 16;  // list build: one row per warp, a whole window of hits
+// per_warp: bytes of row buffer per warp (list build: CELLS_ROW0_BYTES; list-free pass: 32 rows + their entry counts)
+__host__ __device__ inline size_t cells_smem_bytes(unsigned tile_cap, size_t per_warp, unsigned nwarps) {
+  return (size_t)(tile_cap + 1) * 16 + HTAB * 16 + HTAB * 4 + HTAB * 2 + (size_t)nwarps * per_warp;
 }
 
 __device__ __forceinline__ void sts_u16(unsigned addr, unsigned v) {
@@ -857,7 +869,7 @@ __device__ __forceinline__ uint4 lds4u(unsigned addr) {
   return v;
 }
 
-// stage_fast's copy (recipe -> items -> cp.async), then one pass in place to centred coordinates and -|x|^2 (bit 0 of
+// stage_fast's copy (recipe -> items -> cp.async), then one pass in place to centred coordinates and |x|^2 (bit 0 of
 // which carries the frozen flag when HAS_WALL); also fetches the tile's table of first staged slots.
 template <bool HAS_WALL>
 __device__ __forceinline__ bool stage_cells(const DevP& p, const TileInfo& T, const uint4 hdr, const float4* __restrict__ pos,
@@ -909,48 +921,103 @@ __device__ __forceinline__ bool stage_cells(const DevP& p, const TileInfo& T, co
       x.x += sh.x;
       x.y += sh.y;
       x.z += sh.z;
-      float q2 = -fmaf(x.z, x.z, fmaf(x.y, x.y, x.x * x.x));
+      float q2 = fmaf(x.z, x.z, fmaf(x.y, x.y, x.x * x.x));
       if (HAS_WALL) q2 = u2f((f2u(q2) & ~1u) | (f2u(x.w) >> 31));
       x.w = q2;
       *xp = x;
     }
   }
-  if (threadIdx.x == 0) img[p.tile_cap] = make_float4(1e9f, 1e9f, 1e9f, -3e18f);  // sentinel slot: out of range of everything
+  if (threadIdx.x == 0) img[p.tile_cap] = make_float4(1e9f, 1e9f, 1e9f, 3e18f);  // sentinel slot: out of range of everything
   __syncthreads();
   return true;
 }
 
-// candidates [s, se) of the staged image against the lane's particle; hits are appended to the lane's row
-template <bool EXCL>
-__device__ __forceinline__ void scan_range(const unsigned ibase, unsigned s, const unsigned se, const float ax, const float ay,
-                                           const float az, float& bi, const unsigned self, unsigned& rp, const unsigned rp_lim,
-                                           bool& over) {
-  auto test = [&](const float4 c, const unsigned slot) {
-    const float v = fmaf(c.x, ax, fmaf(c.y, ay, fmaf(c.z, az, bi)));
-    bool hit = v < c.w;
-    if (EXCL) hit = hit && slot != self;
-    if (hit) {
-      sts_u16(rp, slot);
-      rp += 2u;
+struct CandRegs {  // one window of candidates: chunk t, this lane
+  float x[CHMAX], y[CHMAX], z[CHMAX], q[CHMAX];
+  unsigned s[CHMAX];  // staged slot (the sentinel past the end)
+};
+
+// own particles [il0, il1) of the cell whose first staged slot is S_cell, against the NCH chunks of the window; particle
+// il appends its hits to row row0 + (il - il0) of the warp's row buffer.  All lanes must call it.  (List-free pass.)
+template <int NCH>
+__device__ __forceinline__ void cell_tests(const CandRegs& C, const float4* img, const unsigned S_cell, const unsigned il0,
+                                           const unsigned il1, const unsigned row0, const unsigned rbase_w,
+                                           const unsigned row_bytes, unsigned short* rowcnt, const float cut2,
+                                           const unsigned rowcap, const unsigned ltmask, const unsigned lane) {
+  float4 xi = img[S_cell + il0];
+  for (unsigned il = il0; il < il1; ++il) {
+    const float ax = -2.0f * xi.x, ay = -2.0f * xi.y, az = -2.0f * xi.z;
+    const float thr = cut2 - fmaf(xi.z, xi.z, fmaf(xi.y, xi.y, xi.x * xi.x));
+    const unsigned self = S_cell + il;
+    const unsigned row = row0 + (il - il0);
+    const unsigned ra = rbase_w + row * row_bytes;
+    // running write address of the row; it saturates at rowcap + 1 entries: a list that stays within rowcap is never
+    // clamped, a longer one reads back as rowcap + 1 (an overflow), and no store leaves the row (rowcap + 40 entries)
+    const unsigned lim = ra + 2u * rowcap + 2u;
+    unsigned na = ra + 2u * rowcnt[row];
+    xi = img[S_cell + min(il + 1u, il1 - 1u)];  // next particle's position in flight
+#pragma unroll
+    for (int t = 0; t < NCH; ++t) {
+      const float v = fmaf(C.x[t], ax, fmaf(C.y[t], ay, fmaf(C.z[t], az, C.q[t])));
+      const bool hit = v < thr && C.s[t] != self;
+      const unsigned b = __ballot_sync(0xffffffffu, hit);
+      if (hit) sts_u16(na + 2u * __popc(b & ltmask), C.s[t]);
+      na = min(na + 2u * __popc(b), lim);
     }
-  };
-  while (s < se) {
-    if (__any_sync(0xffffffffu, rp > rp_lim)) {  // a full row stops collecting: its list is reported as overflowed
-      if (rp > rp_lim) {
-        bi = __int_as_float(0x7f800000);
-        over = true;
+    if (lane == 0) rowcnt[row] = (unsigned short)((na - ra) >> 1);
+  }
+}
+
+// List build: the same tests, but a particle's row is complete when its chunk loop ends, so it is copied to the list
+// right away (lane c copies the 16-byte chunk c) and the warp needs ONE row, sized for a whole window of hits: no
+// clamping, and the shared memory it frees buys resident warps.  `ra` = shared address of the warp's row (16-byte
+// aligned), gi0 = sorted index of particle il0.  FIRST / LAST: this window is the first / last of the cell's stencil
+// (both true unless the stencil holds more than 32 CHMAX particles; then the caller loops particle by particle over
+// the windows and `n0` carries the row's fill from window to window).  Statistics are kept by lane 0.
+template <int NCH, bool FIRST, bool LAST>
+__device__ __forceinline__ void cell_tests_flush(const DevP& p, const CandRegs& C, const float4* img, const unsigned S_cell,
+                                                 const unsigned il0, const unsigned il1, const unsigned gi0, const unsigned ra,
+                                                 const float cut2, const unsigned ltmask, const unsigned lane,
+                                                 unsigned* lhist, unsigned& smax, unsigned& ssum, bool& sover, unsigned& n0) {
+  const unsigned sent2 = p.tile_cap | (p.tile_cap << 16);
+  const unsigned fill = (p.cap + 8u + 7u) >> 3;  // chunks that can reach the list, plus one of padding
+  float4 xi = img[S_cell + il0];
+  for (unsigned il = il0; il < il1; ++il) {
+    const float ax = -2.0f * xi.x, ay = -2.0f * xi.y, az = -2.0f * xi.z;
+    const float thr = cut2 - fmaf(xi.z, xi.z, fmaf(xi.y, xi.y, xi.x * xi.x));
+    const unsigned self = S_cell + il;
+    xi = img[S_cell + min(il + 1u, il1 - 1u)];  // next particle's position in flight
+    if (FIRST) {  // fresh row: sentinel everywhere a flushed chunk can look (the hits overwrite it)
+      if (lane < fill) asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(ra + 16u * lane), "r"(sent2) : "memory");
+      __syncwarp();
+    }
+    unsigned na = ra + 2u * (FIRST ? 0u : n0);
+#pragma unroll
+    for (int t = 0; t < NCH; ++t) {
+      const float v = fmaf(C.x[t], ax, fmaf(C.y[t], ay, fmaf(C.z[t], az, C.q[t])));
+      const bool hit = v < thr && C.s[t] != self;
+      const unsigned b = __ballot_sync(0xffffffffu, hit);
+      if (hit) sts_u16(na + 2u * __popc(b & ltmask), C.s[t]);
+      na += 2u * __popc(b);
+    }
+    __syncwarp();
+    unsigned n = (na - ra) >> 1;
+    n0 = n;
+    if (LAST) {
+      const bool over = n > p.cap;
+      if (over) n = 0;  // reported as MDPD_EOVERFLOW; this particle's list is emptied
+      const unsigned gi = gi0 + (il - il0);
+      if (lane < ((n + 7u) >> 3)) p.nbr[(size_t)lane * p.N + gi] = lds4u(ra + 16u * lane);
+      if (lane == 0) {
+        p.nnbr[gi] = n;
+        p.self_loc[gi] = (unsigned short)self;
+        atomicAdd(&lhist[LCAP - min(n, LCAP)], 1u);
+        smax = max(smax, n);
+        ssum += n;
+        sover = sover || over;
       }
+      __syncwarp();
     }
-    const unsigned e = min(se, s + ROW_SLACK);
-    for (; s + 4u <= e; s += 4u) {
-      const unsigned a = ibase + (s << 4);
-      const float4 c0 = lds4(a), c1 = lds4(a + 16u), c2 = lds4(a + 32u), c3 = lds4(a + 48u);
-      test(c0, s);
-      test(c1, s + 1u);
-      test(c2, s + 2u);
-      test(c3, s + 3u);
-    }
-    for (; s < e; ++s) test(lds4(ibase + (s << 4)), s);
   }
 }
 
@@ -971,25 +1038,23 @@ __device__ __forceinline__ void direct_entry(const DevP& p, const unsigned ibase
 }
 
 template <int MODE, bool HAS_WALL, bool ALL>
-__global__ void __launch_bounds__(CELLS_MAXW * 32, 2) k_cells(const DevP p, int always) {
+__global__ void __launch_bounds__((MODE ? CELLS_MAXW : CELLS_MAXW0) * 32, 2) k_cells(const DevP p, int always) {
   if (!always && !p.ctl->rebuild) return;
   extern __shared__ __align__(16) unsigned char smraw[];
   float4* const img = (float4*)smraw;
   unsigned char* q = smraw + (size_t)(p.tile_cap + 1) * 16;
-  uint2* const sitems = (uint2*)q;                    // staging items; afterwards the work items and the histogram
-  uint4* const witems = (uint4*)q;                    // [CELLS_ITEMS]
-  unsigned* const lhist = (unsigned*)(q + CELLS_ITEMS * 16);  // [LCAP + 1] bins (bin 0 = longest), then: max, sum, faults, next item
+  uint2* const sitems = (uint2*)q;                    // staging items; afterwards the histogram
+  unsigned* const lhist = (unsigned*)q;               // [LCAP + 1] bins (bin 0 = longest), then: max, sum, faults, next item
   q += HTAB * 16;
   float4* const shtab = (float4*)q;
   q += HTAB * 4;
   unsigned short* const hb = (unsigned short*)q;
   q += HTAB * 2;
-  static_assert(CELLS_ITEMS * 16 + (LCAP + 8) * 4 <= HTAB * 16, "k_cells scratch");
   const unsigned cur = p.ctl->cur;
   const TileInfo T = p.tiles[blockIdx.x];
   const uint4 hdr = p.runs[(size_t)blockIdx.x * p.run_stride];
   const unsigned os = hdr.w, nown = hdr.z >> 16;
-  const unsigned warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const unsigned warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
   if (!stage_cells<HAS_WALL>(p, T, hdr, p.pos[cur], img, sitems, shtab, hb)) {  // does not fit: empty lists, the passes skip the tile
     for (unsigned t = threadIdx.x; t < nown; t += blockDim.x) {
       if (MODE == 0) {
@@ -1004,140 +1069,174 @@ __global__ void __launch_bounds__(CELLS_MAXW * 32, 2) k_cells(const DevP p, int 
   for (unsigned k = threadIdx.x; k < LCAP + 8u; k += blockDim.x) lhist[k] = 0u;
   __syncthreads();
   const int hxn = T.ex + 2, hyn = T.ey + 2;
-  // work items: per own x-row, maximal groups of consecutive cells holding <= 32 particles (a fuller cell is its own item)
-  unsigned nitems_w = 0;
-  if (warp == 0) {
-    const int nrows = T.ey * T.ez;
-    unsigned gS[4], gN[4], gM[4];
-    unsigned ng = 0, g_row = 0, sb_row = 0;
-    if ((int)lane < nrows) {
-      const int hy = 1 + (int)lane % T.ey, hz = 1 + (int)lane / T.ey;
-      const int h0 = (hz * hyn + hy) * hxn + 1;
-      g_row = p.runs[(size_t)blockIdx.x * p.run_stride + 1 + (unsigned)(hz * hyn + hy) * 3u + 1u].x;
-      sb_row = hb[h0];
-      int a = 0;
-#pragma unroll
-      for (int k = 0; k < 4; ++k) {
-        if (a < T.ex) {
-          int b = a;
-          unsigned n = (unsigned)hb[h0 + a + 1] - hb[h0 + a];
-          while (b + 1 < T.ex && n + ((unsigned)hb[h0 + b + 2] - hb[h0 + b + 1]) <= 32u) {
-            ++b;
-            n += (unsigned)hb[h0 + b + 1] - hb[h0 + b];
-          }
-          gS[k] = hb[h0 + a];
-          gN[k] = n;
-          gM[k] = (unsigned)a | ((unsigned)b << 8) | ((unsigned)hy << 16) | ((unsigned)hz << 24);
-          ng = (unsigned)k + 1u;
-          a = b + 1;
-        }
-      }
-    }
-    unsigned incl = ng;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const unsigned t = __shfl_up_sync(0xffffffffu, incl, o);
-      if ((int)lane >= o) incl += t;
-    }
-    nitems_w = __shfl_sync(0xffffffffu, incl, 31);
-    unsigned io = incl - ng;
-#pragma unroll
-    for (int k = 0; k < 4; ++k)
-      if ((unsigned)k < ng) witems[io + k] = make_uint4(gS[k], gN[k], g_row + (gS[k] - sb_row), gM[k]);
-    if (lane == 0) lhist[LCAP + 5] = nitems_w;
-  }
-  __syncthreads();
-  const unsigned nitems = lhist[LCAP + 5];
-  const unsigned rowcap = MODE ? p.cap_act : p.cap, row_bytes = MODE ? p.rows_direct : p.rows_verlet;
+  const unsigned rowcap = p.cap_act, row_bytes = p.rows_direct;  // MODE 1: 32 rows per warp
   const float cut2 = (MODE ? p.rc2 : p.rlist2) + p.dot_margin;
   const unsigned sent = p.tile_cap;
   const unsigned ibase = smem_addr(img);
-  const unsigned rbase = smem_addr(q) + (warp * 32u + lane) * row_bytes;  // this lane's row
-  const unsigned rp_lim = rbase + 2u * rowcap;
+  // MODE 0: one row per warp (a window's worth of hits); MODE 1: 32 rows per warp and their entry counts
+  unsigned short* const rowcnt = (unsigned short*)(q + (size_t)W * 32 * row_bytes) + warp * 32;
+  const unsigned rbase_w = smem_addr(q) + warp * (MODE ? 32u * row_bytes : CELLS_ROW0_BYTES);
+  const unsigned rbase = rbase_w + lane * row_bytes;  // MODE 1: the row this lane flushes
+  const unsigned ltmask = (1u << lane) - 1u;
+  const uint4* __restrict__ rec = p.runs + (size_t)blockIdx.x * p.run_stride + 1;
   unsigned smax = 0, ssum = 0;
   bool sover = false;
   float4* __restrict__ vel = p.vel[cur];
+  // MODE 1, rows in use: lane = row; which particle the row belongs to
+  unsigned rows_used = 0, my_gi = 0, my_self = 0;
+
+  auto flush = [&]() {
+    __syncwarp();
+    const bool active = lane < rows_used;
+    unsigned cnt = active ? rowcnt[lane] : 0u;
+    const bool over = cnt > rowcap;
+    if (over) cnt = 0;  // reported as MDPD_EOVERFLOW; this particle's list is emptied
+    if (active)
+      for (unsigned k = cnt; k & 7u; ++k) sts_u16(rbase + 2u * k, sent);  // pad the last chunk with the sentinel
+    __syncwarp();
+    const unsigned nch = (cnt + 7u) >> 3;
+    const unsigned wch = __reduce_max_sync(0xffffffffu, nch);
+    const float4 xi = img[active ? my_self : sent];
+    const unsigned walli = HAS_WALL ? (f2u(xi.w) & 1u) : 0u;
+    float rho = 0.0f;
+    unsigned nin = 0;
+    for (unsigned c = 0; c < nch; ++c) {
+      const unsigned ka = rbase + 16u * c;
+      const uint4 e = lds4u(ka);
+      direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.x & 0xFFFFu, ka, sent, rho, nin);
+      direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.x >> 16, ka + 2u, sent, rho, nin);
+      direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.y & 0xFFFFu, ka + 4u, sent, rho, nin);
+      direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.y >> 16, ka + 6u, sent, rho, nin);
+      direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.z & 0xFFFFu, ka + 8u, sent, rho, nin);
+      direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.z >> 16, ka + 10u, sent, rho, nin);
+      direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.w & 0xFFFFu, ka + 12u, sent, rho, nin);
+      direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.w >> 16, ka + 14u, sent, rho, nin);
+    }
+    __syncwarp();
+    for (unsigned c = 0; c < wch; ++c)
+      if (c < nch) p.act[(size_t)c * p.N + my_gi] = lds4u(rbase + 16u * c);
+    if (active) {
+      p.nact[my_gi] = (unsigned short)cnt;
+      vel[my_gi].w = rho * p.Krho;
+      const unsigned fy = (HAS_WALL && !ALL && walli) ? 0x80000000u : cnt;  // frozen: force not needed (R8)
+      p.dinfo[my_gi] = make_uint2((my_gi - os) | (my_self << 16), fy);     // unsorted; the tail below orders them
+      atomicAdd(&lhist[LCAP - min(fy & 0x7FFFFFFFu, LCAP)], 1u);
+      ssum += nin;
+      sover = sover || over;
+    }
+    __syncwarp();
+    rows_used = 0;
+  };
+
+  // work items: pairs of x-adjacent own cells, handed out through a counter in shared memory
+  const unsigned xpairs = ((unsigned)T.ex + 1u) >> 1, nitems = xpairs * (unsigned)(T.ey * T.ez);
   for (;;) {
     unsigned it = 0;
     if (lane == 0) it = atomicAdd(&lhist[LCAP + 4], 1u);
     it = __shfl_sync(0xffffffffu, it, 0);
     if (it >= nitems) break;
-    const uint4 Wk = witems[it];
-    const unsigned S0 = Wk.x, n = Wk.y, G0 = Wk.z;
-    const int ca = (int)(Wk.w & 255u), cb = (int)((Wk.w >> 8) & 255u), hy = (int)((Wk.w >> 16) & 255u), hz = (int)(Wk.w >> 24);
-    for (unsigned r0 = 0; r0 < n; r0 += 32u) {
-      const unsigned li = r0 + lane;
-      const bool active = li < n;
-      const unsigned self = S0 + li;
-      const float4 xi = img[active ? self : S0];
-      const float ax = -2.0f * xi.x, ay = -2.0f * xi.y, az = -2.0f * xi.z;
-      float bi = active ? fmaf(xi.z, xi.z, fmaf(xi.y, xi.y, xi.x * xi.x)) - cut2 : __int_as_float(0x7f800000);
-      unsigned rp = rbase;
-      bool over = false;
-      const unsigned lo = S0 + r0, hi = min(S0 + n, lo + 32u);  // this round's own particles among the candidates
-#pragma unroll 1
-      for (int qq = 0; qq < 9; ++qq) {
-        const int hrow = ((hz - 1 + qq / 3) * hyn + (hy - 1 + qq % 3)) * hxn + ca;  // halo x of cell ca - 1
-        const unsigned sb = hb[hrow], se = hb[hrow + (cb - ca + 3)];
-        if (qq == 4) {
-          scan_range<false>(ibase, sb, lo, ax, ay, az, bi, self, rp, rp_lim, over);
-          scan_range<true>(ibase, lo, hi, ax, ay, az, bi, self, rp, rp_lim, over);
-          scan_range<false>(ibase, hi, se, ax, ay, az, bi, self, rp, rp_lim, over);
-        } else {
-          scan_range<false>(ibase, sb, se, ax, ay, az, bi, self, rp, rp_lim, over);
-        }
+    const int xp = (int)(it % xpairs), rowi = (int)(it / xpairs);
+    const int hy = 1 + rowi % T.ey, hz = 1 + rowi / T.ey;
+    const int h0 = (hz * hyn + hy) * hxn + 1;  // halo index of the row's first own cell
+    const unsigned g_row = rec[(unsigned)(hz * hyn + hy) * 3u + 1u].x, sb_row = hb[h0];
+    for (int cx = 2 * xp; cx < min(2 * xp + 2, T.ex); ++cx) {
+      const unsigned S_cell = hb[h0 + cx], n = (unsigned)hb[h0 + cx + 1] - S_cell, G_cell = g_row + (S_cell - sb_row);
+      if (n == 0) continue;
+      // the nine candidate runs: lane r < 9 holds run r = (dz, dy); inclusive scan of the run lengths
+      unsigned run_b = 0, run_n = 0;
+      if (lane < 9) {
+        const int hrow = ((hz - 1 + (int)lane / 3) * hyn + (hy - 1 + (int)lane % 3)) * hxn + cx;  // halo x of cell cx - 1
+        run_b = hb[hrow];
+        run_n = (unsigned)hb[hrow + 3] - run_b;
       }
-      unsigned cnt = (rp - rbase) >> 1;
-      if (cnt > rowcap) over = true;
-      if (over) cnt = 0;  // reported as MDPD_EOVERFLOW; this particle's list is emptied
-      for (unsigned k = cnt; k & 7u; ++k) sts_u16(rbase + 2u * k, sent);  // pad the last chunk with the sentinel
-      __syncwarp();
-      const unsigned gi = G0 + li;
-      const unsigned nch = active ? (cnt + 7u) >> 3 : 0u;
+      unsigned incl = run_n;
+#pragma unroll
+      for (int o = 1; o < 16; o <<= 1) {
+        const unsigned t = __shfl_up_sync(0xffffffffu, incl, o);
+        if ((int)lane >= o) incl += t;
+      }
+      const unsigned ncand = __shfl_sync(0xffffffffu, incl, 8);
+      const unsigned run_o = incl - run_n;  // exclusive offset of the lane's run
+      unsigned rend[8];
+#pragma unroll
+      for (int r = 0; r < 8; ++r) rend[r] = __shfl_sync(0xffffffffu, incl, r);
+      CandRegs C;
+      // one window of candidates into registers: flat candidate index -> staged slot (past the end: the sentinel, never hit)
+      auto load_window = [&](const unsigned win, const unsigned nch) {
+#pragma unroll
+        for (int t = 0; t < CHMAX; ++t) {
+          if ((unsigned)t < nch) {  // warp-uniform
+            const unsigned f = win + 32u * t + lane;
+            unsigned r = 0;
+#pragma unroll
+            for (int qq = 0; qq < 8; ++qq) r += (f >= rend[qq]) ? 1u : 0u;
+            const unsigned rb = __shfl_sync(0xffffffffu, run_b, r), ro = __shfl_sync(0xffffffffu, run_o, r);
+            const unsigned cs = f < ncand ? rb + (f - ro) : sent;
+            const float4 xc = img[cs];
+            C.x[t] = xc.x;
+            C.y[t] = xc.y;
+            C.z[t] = xc.z;
+            C.q[t] = xc.w;
+            C.s[t] = cs;
+          }
+        }
+      };
       if (MODE == 0) {
-        const unsigned wch = __reduce_max_sync(0xffffffffu, nch);
-        for (unsigned c = 0; c < wch; ++c)
-          if (c < nch) p.nbr[(size_t)c * p.N + gi] = lds4u(rbase + 16u * c);
-        if (active) {
-          p.nnbr[gi] = cnt;
-          p.self_loc[gi] = (unsigned short)self;
-          atomicAdd(&lhist[LCAP - min(cnt, LCAP)], 1u);
-          smax = max(smax, cnt);
-          ssum += cnt;
-          sover = sover || over;
+        unsigned n0 = 0;
+        if (ncand <= 32u * CHMAX) {  // the whole stencil fits one window: particle after particle, each flushed at once
+          const unsigned nch = (ncand + 31u) >> 5;
+          load_window(0u, nch);
+#define CELLS_CASE(K)                                                                                                           \
+  case K:                                                                                                                         \
+    cell_tests_flush<K, true, true>(p, C, img, S_cell, 0u, n, G_cell, rbase_w, cut2, ltmask, lane, lhist, smax, ssum, sover, n0); \
+    break;
+          switch (nch) {
+            CELLS_CASE(1) CELLS_CASE(2) CELLS_CASE(3) CELLS_CASE(4) CELLS_CASE(5) CELLS_CASE(6)
+            CELLS_CASE(7) CELLS_CASE(8) CELLS_CASE(9) CELLS_CASE(10) CELLS_CASE(11) CELLS_CASE(12)
+            default: break;
+          }
+#undef CELLS_CASE
+        } else {  // very dense: particle by particle over the windows, the row carried from window to window
+          for (unsigned il = 0; il < n; ++il) {
+            for (unsigned win = 0; win < ncand; win += 32u * CHMAX) {
+              const bool last = win + 32u * CHMAX >= ncand;
+              load_window(win, CHMAX);
+              if (win == 0u) cell_tests_flush<CHMAX, true, false>(p, C, img, S_cell, il, il + 1u, G_cell + il, rbase_w, cut2, ltmask, lane, lhist, smax, ssum, sover, n0);
+              else if (!last) cell_tests_flush<CHMAX, false, false>(p, C, img, S_cell, il, il + 1u, G_cell + il, rbase_w, cut2, ltmask, lane, lhist, smax, ssum, sover, n0);
+              else cell_tests_flush<CHMAX, false, true>(p, C, img, S_cell, il, il + 1u, G_cell + il, rbase_w, cut2, ltmask, lane, lhist, smax, ssum, sover, n0);
+            }
+          }
         }
       } else {
-        const unsigned walli = HAS_WALL ? (f2u(xi.w) & 1u) : 0u;
-        float rho = 0.0f;
-        unsigned nin = 0;
-        for (unsigned c = 0; c < nch; ++c) {
-          const unsigned ka = rbase + 16u * c;
-          const uint4 e = lds4u(ka);
-          direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.x & 0xFFFFu, ka, sent, rho, nin);
-          direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.x >> 16, ka + 2u, sent, rho, nin);
-          direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.y & 0xFFFFu, ka + 4u, sent, rho, nin);
-          direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.y >> 16, ka + 6u, sent, rho, nin);
-          direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.z & 0xFFFFu, ka + 8u, sent, rho, nin);
-          direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.z >> 16, ka + 10u, sent, rho, nin);
-          direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.w & 0xFFFFu, ka + 12u, sent, rho, nin);
-          direct_entry<HAS_WALL, ALL>(p, ibase, xi, walli, e.w >> 16, ka + 14u, sent, rho, nin);
-        }
-        __syncwarp();
-        const unsigned wch = __reduce_max_sync(0xffffffffu, nch);
-        for (unsigned c = 0; c < wch; ++c)
-          if (c < nch) p.act[(size_t)c * p.N + gi] = lds4u(rbase + 16u * c);
-        if (active) {
-          p.nact[gi] = (unsigned short)cnt;
-          vel[gi].w = rho * p.Krho;
-          const unsigned fy = (HAS_WALL && !ALL && walli) ? 0x80000000u : cnt;  // frozen: force not needed (R8)
-          p.dinfo[gi] = make_uint2((gi - os) | (self << 16), fy);             // unsorted; the tail below orders them
-          atomicAdd(&lhist[LCAP - min(fy & 0x7FFFFFFFu, LCAP)], 1u);
-          ssum += nin;
-          sover = sover || over;
+        for (unsigned r0 = 0; r0 < n;) {
+          if (rows_used == 32u || (r0 == 0 && rows_used + n > 32u && n <= 32u)) flush();  // keep a cell's rows together when they fit
+          const unsigned take = min(n - r0, 32u - rows_used);
+          if (lane >= rows_used && lane < rows_used + take) {
+            my_gi = G_cell + r0 + (lane - rows_used);
+            my_self = S_cell + r0 + (lane - rows_used);
+            rowcnt[lane] = 0;
+          }
+          __syncwarp();
+          for (unsigned win = 0; win < ncand; win += 32u * CHMAX) {  // one window unless the stencil holds more than 384 particles
+            const unsigned nch = (min(ncand, win + 32u * CHMAX) - win + 31u) >> 5;
+            load_window(win, nch);
+#define CELLS_CASE(K)                                                                                                           \
+  case K:                                                                                                                         \
+    cell_tests<K>(C, img, S_cell, r0, r0 + take, rows_used, rbase_w, row_bytes, rowcnt, cut2, rowcap, ltmask, lane);              \
+    break;
+            switch (nch) {
+              CELLS_CASE(1) CELLS_CASE(2) CELLS_CASE(3) CELLS_CASE(4) CELLS_CASE(5) CELLS_CASE(6)
+              CELLS_CASE(7) CELLS_CASE(8) CELLS_CASE(9) CELLS_CASE(10) CELLS_CASE(11) CELLS_CASE(12)
+              default: break;
+            }
+#undef CELLS_CASE
+          }
+          rows_used += take;
+          r0 += take;
         }
       }
-      __syncwarp();
     }
+    if (MODE == 1) flush();
   }
   // statistics of the tile: per warp into shared memory, one set of global atomics per CTA
   smax = __reduce_max_sync(0xffffffffu, smax);
@@ -2282,13 +2381,13 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
   h->d.rows_verlet = cells_row_bytes(h->d.cap);
   h->d.rows_direct = cells_row_bytes(h->d.cap_act);
   for (int mode = 0; mode < 2; ++mode) {
-    const size_t rowb = 32 * (size_t)(mode ? h->d.rows_direct : h->d.rows_verlet);
+    const size_t rowb = mode ? 32 * (size_t)h->d.rows_direct + 64 : (size_t)CELLS_ROW0_BYTES;
     const size_t base = cells_smem_bytes(h->d.tile_cap, 0, 0);
     const size_t two = (h->smem_limit + 1024) / 2 - 1024;  // per CTA when two are resident
     size_t nw = two > base ? (two - base) / rowb : 0;
     if (nw < 4) nw = h->smem_limit > base ? (h->smem_limit - base) / rowb : 0;  // one resident CTA
     if (nw < 1) return set_err(h, MDPD_ENOMEM, "k_cells: the staged tile and one row buffer do not fit in shared memory");
-    h->cells_warps[mode] = (unsigned)std::min<size_t>(nw, CELLS_MAXW);
+    h->cells_warps[mode] = (unsigned)std::min<size_t>(nw, mode ? CELLS_MAXW : CELLS_MAXW0);
     h->smem_cells[mode] = base + h->cells_warps[mode] * rowb;
   }
   CU_TRY(h, (cudaFuncSetAttribute(k_cells<0, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_cells[0])));
