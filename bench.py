@@ -217,7 +217,7 @@ def main_ours(args, rank, world, local):
     c = wl.make_config(args.workload if args.workload in ("4a", "4b") else int(args.workload))
     if args.skin is not None:
         c["params"]["skin"] = float(args.skin)
-    c["params"]["flags"] = (2 if args.direct else 0) | (1 if args.no_graph else 0)
+    c["params"]["flags"] = (2 if args.direct else 0) | (1 if args.no_graph else 0) | (4 if args.tma else 0) | (8 if args.cpasync else 0)
     n = len(c["pos"])
     md = None if c.get("mask") is None else c["mask"].shape[::-1]
     # pinned host buffers (inputs of the e2e leg, outputs of get_state)
@@ -413,6 +413,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--equilibrate", type=int, default=EQUILIBRATE, help="untimed steps after loading")
     ap.add_argument("--direct", action="store_true", help="list-free path (MDPD_FLAG_DIRECT): no Verlet list")
+    ap.add_argument("--tma", action="store_true", help="both tile passes stage with cp.async.bulk (MDPD_FLAG_TMA_STAGING)")
+    ap.add_argument("--cpasync", action="store_true", help="both tile passes stage with cp.async (MDPD_FLAG_CPASYNC_STAGING)")
     ap.add_argument("--no-graph", action="store_true", help="launch the kernels one by one (MDPD_FLAG_NO_GRAPH; for ncu)")
     ap.add_argument("--skin", type=float, default=None, help="override the Verlet-list skin (default: the config's 0.25)")
     args = ap.parse_args()

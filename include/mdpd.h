@@ -66,6 +66,10 @@ typedef struct {
 #define MDPD_FLAG_DIRECT 2u   /* list-free path: no Verlet list; every step finds the r < rc neighbours straight from the
                                  cells (same results; the cells are still re-sorted on the skin/2 displacement trigger).
                                  Fixed by mdpd_load_particles. */
+#define MDPD_FLAG_TMA_STAGING 4u     /* BOTH tile passes stage their tile with cp.async.bulk (1-D TMA bulk copies, one per */
+#define MDPD_FLAG_CPASYNC_STAGING 8u /* contiguous run, mbarrier completion) / with per-particle cp.async copies.  Default
+                                        (neither flag): bulk copies in the density pass, cp.async in the force pass, as
+                                        measured in profiles/r2_staging.md.  Same results either way.  Fixed by load. */
 
 /* Create a handle on CUDA device `device`; `cuda_stream` is a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream)
  * or NULL for the default stream.  The handle must be destroyed with mdpd_destroy. */

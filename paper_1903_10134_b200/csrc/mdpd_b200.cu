@@ -90,6 +90,7 @@ struct DevP {  // passed by value to every kernel
   unsigned cap_act;      // capacity of the per-step in-range (r < rc) lists of the list-free path
   unsigned rows_verlet, rows_direct;  // bytes per row of k_cells' per-warp row buffers (list build / list-free pass)
   float dot_margin;      // slack of the approximate (dot-product form) range test of k_cells, in units of r^2
+  unsigned tma_staging;  // bit 0 / bit 1: the density / force pass stages its tile with bulk copies (stage_bulk), else cp.async (stage_fast)
   int ncx, ncy, ncz;
   int mx, my, mz;
   // geometry
@@ -259,8 +260,8 @@ __global__ void k_count_in_solid(DevP p, unsigned* count) {
   x.x = wrap1(x.x, p.Lx);
   x.y = wrap1(x.y, p.Ly);
   x.z = wrap1(x.z, p.Lz);
-  int ix = min((int)(x.x * p.inv_voxel), p.mx - 1), iy = min((int)(x.y * p.inv_voxel), p.my - 1),
-      iz = min((int)(x.z * p.inv_voxel), p.mz - 1);
+  int ix = max(min((int)(x.x * p.inv_voxel), p.mx - 1), 0), iy = max(min((int)(x.y * p.inv_voxel), p.my - 1), 0),
+      iz = max(min((int)(x.z * p.inv_voxel), p.mz - 1), 0);
   if (p.mask[((size_t)iz * p.my + iy) * p.mx + ix]) atomicAdd(count, 1u);
 }
 
@@ -291,12 +292,15 @@ __global__ void __launch_bounds__(TPB) k_integrate(const DevP p, int do_B, int d
         v.y += p.hdt_m * f.y;
         v.z += p.hdt_m * f.z;
         const float nx = x.x + p.dt * v.x, ny = x.y + p.dt * v.y, nz = x.z + p.dt * v.z;
-        bool solid = false;
+        bool solid = false, fin = true;
         if (HAS_MASK) {
           const float wx = wrap1(nx, p.Lx), wy = wrap1(ny, p.Ly), wz = wrap1(nz, p.Lz);
-          int ix = min((int)(wx * p.inv_voxel), p.mx - 1), iy = min((int)(wy * p.inv_voxel), p.my - 1),
-              iz = min((int)(wz * p.inv_voxel), p.mz - 1);
-          if (!(nx == nx && ny == ny && nz == nz)) ix = iy = iz = 0;
+          int ix = max(min((int)(wx * p.inv_voxel), p.mx - 1), 0), iy = max(min((int)(wy * p.inv_voxel), p.my - 1), 0),
+              iz = max(min((int)(wz * p.inv_voxel), p.mz - 1), 0);
+          // a trial position that is not finite, or that one period does not bring back into the box (a runaway
+          // particle), is a fault (MDPD_ENAN), not a mask lookup
+          fin = fabsf(nx - 0.5f * p.Lx) <= 1.5f * p.Lx && fabsf(ny - 0.5f * p.Ly) <= 1.5f * p.Ly && fabsf(nz - 0.5f * p.Lz) <= 1.5f * p.Lz;
+          if (!fin) ix = iy = iz = 0;
           solid = p.mask[((size_t)iz * p.my + iy) * p.mx + ix] != 0;
         }
         if (solid) {  // bounce-back (R7): position kept, velocity reversed
@@ -312,7 +316,7 @@ __global__ void __launch_bounds__(TPB) k_integrate(const DevP p, int do_B, int d
         const float4 xb = p.xbuild[i];
         const float dx = x.x - xb.x, dy = x.y - xb.y, dz = x.z - xb.z;  // unwrapped since the last build
         const float d2 = dx * dx + dy * dy + dz * dz;
-        if (!(d2 < 1e30f)) bad += 1;
+        if (!(d2 < 1e30f) || !fin) bad += 1;
         else d2max = fmaxf(d2max, d2);
         p.pos[cur][i] = x;
       }
@@ -722,6 +726,84 @@ __device__ __forceinline__ bool stage_fast(const DevP& p, const TileInfo& T, con
   return true;
 }
 
+// stage_bulk: the same staged image by the bulk-copy engine (TMA, 1-D form).  A run of the recipe is contiguous both in
+// the sorted arrays and in the staged image, 16-byte aligned on both sides: thread r issues ONE cp.async.bulk
+// (global -> shared, completion counted in bytes on an mbarrier) per run and array, thread 0 arms the mbarrier with the
+// tile's byte count, everybody waits on its phase.  No per-particle copy instructions, no item list.  The periodic
+// shift of a boundary tile is added afterwards, warp per run.  (mdpd_params.flags & MDPD_FLAG_TMA_STAGING; measured
+// against stage_fast in profiles/r2_staging.md.)
+template <bool WITH_VEL>
+__device__ __forceinline__ bool stage_bulk(const DevP& p, const TileInfo& T, const uint4 hdr,
+                                           const float4* __restrict__ pos, const float4* __restrict__ vel,
+                                           const TileSmem& sm) {
+  __shared__ __align__(8) unsigned long long mbar;
+  uint4* const srec = (uint4*)sm.hshift;    // [nruns] <= 108 <= HTAB
+  float4* const shtab = (float4*)sm.hbase;  // [27] shift of every code
+  const uint4* __restrict__ rec = p.runs + (size_t)blockIdx.x * p.run_stride + 1;
+  const unsigned total = hdr.x, nruns = hdr.y;
+  if (total > p.tile_cap) return false;  // flagged by k_tile_recipe (block-uniform)
+  const unsigned mb = smem_addr(&mbar);
+  if (threadIdx.x == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mb) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  if (threadIdx.x < 27) {
+    const unsigned c = threadIdx.x, cx = c % 3u, cy = (c / 3u) % 3u, cz = c / 9u;
+    const float ox = tile_origin(T.c0x, p.edge_x), oy = tile_origin(T.c0y, p.edge_y), oz = tile_origin(T.c0z, p.edge_z);
+    shtab[c] = make_float4(cx == 0u ? -ox : (cx == 1u ? -p.Lx : p.Lx - ox), cy == 0u ? -oy : (cy == 1u ? -p.Ly : p.Ly - oy),
+                           cz == 0u ? -oz : (cz == 1u ? -p.Lz : p.Lz - oz), 0.f);
+  }
+  __syncthreads();
+  const unsigned pbase = smem_addr(sm.spos), vbase = smem_addr(sm.svel);
+  for (unsigned r = threadIdx.x; r < nruns; r += blockDim.x) {
+    const uint4 R = rec[r];
+    srec[r] = R;
+    const unsigned cnt = R.y >> 16, sb = R.y & 0xFFFFu;
+    if (cnt) {
+      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(pbase + (sb << 4)),
+                   "l"(pos + R.x), "r"(cnt << 4), "r"(mb)
+                   : "memory");
+      if (WITH_VEL)
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(vbase + (sb << 4)),
+                     "l"(vel + R.x), "r"(cnt << 4), "r"(mb)
+                     : "memory");
+    }
+  }
+  if (threadIdx.x == 0)
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mb), "r"((total << 4) * (WITH_VEL ? 2u : 1u)) : "memory");
+  {
+    unsigned done = 0;
+    while (!done)
+      asm volatile(
+          "{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }" : "=r"(done) : "r"(mb) : "memory");
+  }
+  const bool interior = T.c0x > 0 && T.c0x + T.ex < p.ncx && T.c0y > 0 && T.c0y + T.ey < p.ncy && T.c0z > 0 && T.c0z + T.ez < p.ncz;
+  if (!interior) {  // to tile-relative coordinates, in place, warp per run
+    __syncthreads();  // the run records
+    const unsigned warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
+    for (unsigned r = warp; r < nruns; r += W) {
+      const uint4 R = srec[r];
+      const unsigned cnt = R.y >> 16, sb = R.y & 0xFFFFu;
+      const float4 sh = shtab[R.z];
+      for (unsigned c = lane; c < cnt; c += 32) {
+        float4* const xp = sm.spos + sb + c;
+        float4 x = *xp;
+        x.x += sh.x;
+        x.y += sh.y;
+        x.z += sh.z;
+        *xp = x;
+      }
+    }
+  }
+  if (threadIdx.x == 0) {  // sentinel slot: list padding points here; it is out of range of everything
+    sm.spos[p.tile_cap] = make_float4(1e9f, 1e9f, 1e9f, 0.f);
+    if (WITH_VEL) sm.svel[p.tile_cap] = make_float4(0.f, 0.f, 0.f, 0.f);
+  }
+  __syncthreads();
+  return true;
+}
+
 // ----------------------------------------------------------------------------------------------------------------
 // Tile recipe.  After every sort k_tile_recipe (one CTA per tile) writes what the tile passes need to stage the tile
 // without rediscovering its geometry: the header and run records described above, and the table of the first
@@ -974,7 +1056,9 @@ __device__ __forceinline__ void cell_tests(const CandRegs& C, const float4* img,
 // aligned), gi0 = sorted index of particle il0.  FIRST / LAST: this window is the first / last of the cell's stencil
 // (both true unless the stencil holds more than 32 CHMAX particles; then the caller loops particle by particle over
 // the windows and `n0` carries the row's fill from window to window).  Statistics are kept by lane 0.
-template <int NCH, bool FIRST, bool LAST>
+// SELF0: the cell's own particles are the first candidates of the window (flat index = index in the cell) and the
+// cell holds at most 32: the particle itself is lane il of chunk 0, nowhere else.
+template <int NCH, bool FIRST, bool LAST, bool SELF0>
 __device__ __forceinline__ void cell_tests_flush(const DevP& p, const CandRegs& C, const float4* img, const unsigned S_cell,
                                                  const unsigned il0, const unsigned il1, const unsigned gi0, const unsigned ra,
                                                  const float cut2, const unsigned ltmask, const unsigned lane,
@@ -982,6 +1066,7 @@ __device__ __forceinline__ void cell_tests_flush(const DevP& p, const CandRegs& 
   const unsigned sent2 = p.tile_cap | (p.tile_cap << 16);
   const unsigned fill = (p.cap + 8u + 7u) >> 3;  // chunks that can reach the list, plus one of padding
   float4 xi = img[S_cell + il0];
+  unsigned myn = 0;  // lane k: list length of particle il0 + k (il1 - il0 <= 32)
   for (unsigned il = il0; il < il1; ++il) {
     const float ax = -2.0f * xi.x, ay = -2.0f * xi.y, az = -2.0f * xi.z;
     const float thr = cut2 - fmaf(xi.z, xi.z, fmaf(xi.y, xi.y, xi.x * xi.x));
@@ -995,7 +1080,12 @@ __device__ __forceinline__ void cell_tests_flush(const DevP& p, const CandRegs& 
 #pragma unroll
     for (int t = 0; t < NCH; ++t) {
       const float v = fmaf(C.x[t], ax, fmaf(C.y[t], ay, fmaf(C.z[t], az, C.q[t])));
-      const bool hit = v < thr && C.s[t] != self;
+      bool hit = v < thr;
+      if (SELF0) {
+        if (t == 0) hit = hit && lane != il;
+      } else {
+        hit = hit && C.s[t] != self;
+      }
       const unsigned b = __ballot_sync(0xffffffffu, hit);
       if (hit) sts_u16(na + 2u * __popc(b & ltmask), C.s[t]);
       na += 2u * __popc(b);
@@ -1004,20 +1094,21 @@ __device__ __forceinline__ void cell_tests_flush(const DevP& p, const CandRegs& 
     unsigned n = (na - ra) >> 1;
     n0 = n;
     if (LAST) {
-      const bool over = n > p.cap;
-      if (over) n = 0;  // reported as MDPD_EOVERFLOW; this particle's list is emptied
-      const unsigned gi = gi0 + (il - il0);
-      if (lane < ((n + 7u) >> 3)) p.nbr[(size_t)lane * p.N + gi] = lds4u(ra + 16u * lane);
-      if (lane == 0) {
-        p.nnbr[gi] = n;
-        p.self_loc[gi] = (unsigned short)self;
-        atomicAdd(&lhist[LCAP - min(n, LCAP)], 1u);
-        smax = max(smax, n);
-        ssum += n;
-        sover = sover || over;
-      }
+      if (n > p.cap) n = 0xFFFFu;  // overflow marker
+      if (lane < (((n > p.cap ? 0u : n) + 7u) >> 3)) p.nbr[(size_t)lane * p.N + gi0 + (il - il0)] = lds4u(ra + 16u * lane);
+      if (lane == il - il0) myn = n;
       __syncwarp();
     }
+  }
+  if (LAST && lane < il1 - il0) {  // lane = particle: lengths, own slots, histogram of the hand-out sort, statistics
+    const bool over = myn > p.cap;
+    if (over) myn = 0;  // reported as MDPD_EOVERFLOW; this particle's list is emptied
+    p.nnbr[gi0 + lane] = myn;
+    p.self_loc[gi0 + lane] = (unsigned short)(S_cell + il0 + lane);
+    atomicAdd(&lhist[LCAP - min(myn, LCAP)], 1u);
+    smax = max(smax, myn);
+    ssum += myn;
+    sover = sover || over;
   }
 }
 
@@ -1142,12 +1233,18 @@ __global__ void __launch_bounds__((MODE ? CELLS_MAXW : CELLS_MAXW0) * 32, 2) k_c
     for (int cx = 2 * xp; cx < min(2 * xp + 2, T.ex); ++cx) {
       const unsigned S_cell = hb[h0 + cx], n = (unsigned)hb[h0 + cx + 1] - S_cell, G_cell = g_row + (S_cell - sb_row);
       if (n == 0) continue;
-      // the nine candidate runs: lane r < 9 holds run r = (dz, dy); inclusive scan of the run lengths
+      // the candidate runs, lane r < 11 holds run r: the cell itself first (so that a particle finds itself at lane il of
+      // chunk 0), then the (dz, dy) rows of the stencil, three cells each, the centre row as its left and right cell;
+      // inclusive scan of the run lengths
       unsigned run_b = 0, run_n = 0;
-      if (lane < 9) {
-        const int hrow = ((hz - 1 + (int)lane / 3) * hyn + (hy - 1 + (int)lane % 3)) * hxn + cx;  // halo x of cell cx - 1
+      if (lane < 11) {
+        const int q9 = lane == 0 ? 4 : (lane <= 4 ? (int)lane - 1 : (lane <= 6 ? 4 : (int)lane - 2));  // the row of run `lane`
+        const int hrow = ((hz - 1 + q9 / 3) * hyn + (hy - 1 + q9 % 3)) * hxn + cx;  // halo x of cell cx - 1
         run_b = hb[hrow];
         run_n = (unsigned)hb[hrow + 3] - run_b;
+        if (lane == 0) { run_b = S_cell; run_n = n; }
+        if (lane == 5) run_n = S_cell - run_b;
+        if (lane == 6) { run_n = run_b + run_n - (S_cell + n); run_b = S_cell + n; }
       }
       unsigned incl = run_n;
 #pragma unroll
@@ -1155,11 +1252,11 @@ __global__ void __launch_bounds__((MODE ? CELLS_MAXW : CELLS_MAXW0) * 32, 2) k_c
         const unsigned t = __shfl_up_sync(0xffffffffu, incl, o);
         if ((int)lane >= o) incl += t;
       }
-      const unsigned ncand = __shfl_sync(0xffffffffu, incl, 8);
+      const unsigned ncand = __shfl_sync(0xffffffffu, incl, 10);
       const unsigned run_o = incl - run_n;  // exclusive offset of the lane's run
-      unsigned rend[8];
+      unsigned rend[10];
 #pragma unroll
-      for (int r = 0; r < 8; ++r) rend[r] = __shfl_sync(0xffffffffu, incl, r);
+      for (int r = 0; r < 10; ++r) rend[r] = __shfl_sync(0xffffffffu, incl, r);
       CandRegs C;
       // one window of candidates into registers: flat candidate index -> staged slot (past the end: the sentinel, never hit)
       auto load_window = [&](const unsigned win, const unsigned nch) {
@@ -1169,7 +1266,7 @@ __global__ void __launch_bounds__((MODE ? CELLS_MAXW : CELLS_MAXW0) * 32, 2) k_c
             const unsigned f = win + 32u * t + lane;
             unsigned r = 0;
 #pragma unroll
-            for (int qq = 0; qq < 8; ++qq) r += (f >= rend[qq]) ? 1u : 0u;
+            for (int qq = 0; qq < 10; ++qq) r += (f >= rend[qq]) ? 1u : 0u;
             const unsigned rb = __shfl_sync(0xffffffffu, run_b, r), ro = __shfl_sync(0xffffffffu, run_o, r);
             const unsigned cs = f < ncand ? rb + (f - ro) : sent;
             const float4 xc = img[cs];
@@ -1186,24 +1283,32 @@ __global__ void __launch_bounds__((MODE ? CELLS_MAXW : CELLS_MAXW0) * 32, 2) k_c
         if (ncand <= 32u * CHMAX) {  // the whole stencil fits one window: particle after particle, each flushed at once
           const unsigned nch = (ncand + 31u) >> 5;
           load_window(0u, nch);
-#define CELLS_CASE(K)                                                                                                           \
-  case K:                                                                                                                         \
-    cell_tests_flush<K, true, true>(p, C, img, S_cell, 0u, n, G_cell, rbase_w, cut2, ltmask, lane, lhist, smax, ssum, sover, n0); \
+          for (unsigned r0 = 0; r0 < n; r0 += 32u) {
+            const unsigned r1 = min(n, r0 + 32u);
+#define CELLS_CASE(K)                                                                                                              \
+  case K:                                                                                                                            \
+    if (n <= 32u)                                                                                                                    \
+      cell_tests_flush<K, true, true, true>(p, C, img, S_cell, r0, r1, G_cell + r0, rbase_w, cut2, ltmask, lane, lhist, smax, ssum,  \
+                                            sover, n0);                                                                              \
+    else                                                                                                                             \
+      cell_tests_flush<K, true, true, false>(p, C, img, S_cell, r0, r1, G_cell + r0, rbase_w, cut2, ltmask, lane, lhist, smax, ssum, \
+                                             sover, n0);                                                                             \
     break;
-          switch (nch) {
-            CELLS_CASE(1) CELLS_CASE(2) CELLS_CASE(3) CELLS_CASE(4) CELLS_CASE(5) CELLS_CASE(6)
-            CELLS_CASE(7) CELLS_CASE(8) CELLS_CASE(9) CELLS_CASE(10) CELLS_CASE(11) CELLS_CASE(12)
-            default: break;
-          }
+            switch (nch) {
+              CELLS_CASE(1) CELLS_CASE(2) CELLS_CASE(3) CELLS_CASE(4) CELLS_CASE(5) CELLS_CASE(6)
+              CELLS_CASE(7) CELLS_CASE(8) CELLS_CASE(9) CELLS_CASE(10) CELLS_CASE(11) CELLS_CASE(12)
+              default: break;
+            }
 #undef CELLS_CASE
+          }
         } else {  // very dense: particle by particle over the windows, the row carried from window to window
           for (unsigned il = 0; il < n; ++il) {
             for (unsigned win = 0; win < ncand; win += 32u * CHMAX) {
               const bool last = win + 32u * CHMAX >= ncand;
               load_window(win, CHMAX);
-              if (win == 0u) cell_tests_flush<CHMAX, true, false>(p, C, img, S_cell, il, il + 1u, G_cell + il, rbase_w, cut2, ltmask, lane, lhist, smax, ssum, sover, n0);
-              else if (!last) cell_tests_flush<CHMAX, false, false>(p, C, img, S_cell, il, il + 1u, G_cell + il, rbase_w, cut2, ltmask, lane, lhist, smax, ssum, sover, n0);
-              else cell_tests_flush<CHMAX, false, true>(p, C, img, S_cell, il, il + 1u, G_cell + il, rbase_w, cut2, ltmask, lane, lhist, smax, ssum, sover, n0);
+              if (win == 0u) cell_tests_flush<CHMAX, true, false, false>(p, C, img, S_cell, il, il + 1u, G_cell + il, rbase_w, cut2, ltmask, lane, lhist, smax, ssum, sover, n0);
+              else if (!last) cell_tests_flush<CHMAX, false, false, false>(p, C, img, S_cell, il, il + 1u, G_cell + il, rbase_w, cut2, ltmask, lane, lhist, smax, ssum, sover, n0);
+              else cell_tests_flush<CHMAX, false, true, false>(p, C, img, S_cell, il, il + 1u, G_cell + il, rbase_w, cut2, ltmask, lane, lhist, smax, ssum, sover, n0);
             }
           }
         }
@@ -1366,7 +1471,8 @@ __global__ void __launch_bounds__(DENS_TPB, DENS_MINB) k_density(const DevP p) {
   }
 #pragma unroll
   for (int r = 0; r < PRE; ++r) head[r] = info[r].y ? p.nbr[os + (info[r].x & 0xFFFFu)] : make_uint4(0, 0, 0, 0);
-  if (!stage_fast<false>(p, T, hdr, p.pos[cur], nullptr, sm)) return;  // flagged by k_build_list
+  if (!((p.tma_staging & 1u) ? stage_bulk<false>(p, T, hdr, p.pos[cur], nullptr, sm) : stage_fast<false>(p, T, hdr, p.pos[cur], nullptr, sm)))
+    return;  // flagged by k_tile_recipe
   float4* __restrict__ vel = p.vel[cur];
   const unsigned sent = p.tile_cap;
   const unsigned pbase = smem_addr(sm.spos);
@@ -1558,7 +1664,8 @@ __global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
 #pragma unroll
   for (int r = 0; r < PRE; ++r)
     head[r] = (info[r].y & 0x7FFFFFFFu) ? p.act[os + (info[r].x & 0xFFFFu)] : make_uint4(sentw, sentw, sentw, sentw);
-  if (!stage_fast<true>(p, T, hdr, p.pos[cur], p.vel[cur], sm)) return;
+  if (!((p.tma_staging & 2u) ? stage_bulk<true>(p, T, hdr, p.pos[cur], p.vel[cur], sm) : stage_fast<true>(p, T, hdr, p.pos[cur], p.vel[cur], sm)))
+    return;
   HashKeys K = make_keys(p.ctl->step, p.seed);
 #pragma unroll
   for (int q = 0; q < 6; ++q) K.k[q] = pin(K.k[q]);
@@ -1577,8 +1684,11 @@ __global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
       rec = p.finfo[os + t];
       nxt = (rec.y & 0x7FFFFFFFu) ? p.act[os + (rec.x & 0xFFFFu)] : make_uint4(sentw, sentw, sentw, sentw);
     }
-    if (rec.y >> 31) continue;  // frozen particles are never integrated (R8): their force is not needed
     const unsigned i = os + (rec.x & 0xFFFFu);
+    if (rec.y >> 31) {  // frozen particles are never integrated (R8): their force is not needed; reported as zero
+      p.force[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+      continue;
+    }
     const unsigned li = rec.x >> 16;
     const float4 xi = sm.spos[li];
     const unsigned wi = f2u(xi.w);
@@ -2194,7 +2304,7 @@ int mdpd_set_params(mdpd_ctx* h, const mdpd_params* p) {
     const mdpd_params& q = h->prm;
     if (memcmp(q.box, p->box, sizeof q.box) || q.rc != p->rc || q.rd != p->rd || q.skin != p->skin ||
         q.max_neigh != p->max_neigh || q.mass != p->mass || q.headroom != p->headroom ||
-        ((q.flags ^ p->flags) & MDPD_FLAG_DIRECT))
+        ((q.flags ^ p->flags) & (MDPD_FLAG_DIRECT | MDPD_FLAG_TMA_STAGING | MDPD_FLAG_CPASYNC_STAGING)))
       return set_err(h, MDPD_ESTATE, "box, cut-offs, skin, mass, capacities and the neighbour path are frozen after load_particles");
     if (h->pending_B) {  // the outstanding half kick belongs to the old parameters
       CU_TRY(h, cudaSetDevice(h->device));
@@ -2298,6 +2408,8 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
     LAUNCH(h, PS_OTHER, (k_pack<<<nblk(n, TPB), TPB, 0, h->stream>>>(h->d, spos, svel, type ? stype : nullptr, 0u)));
   }
   h->direct = (h->prm.flags & MDPD_FLAG_DIRECT) != 0;
+  // chosen by measurement (profiles/r2_staging.md): bulk copies win in the density pass, per-particle cp.async in the force pass
+  h->d.tma_staging = (h->prm.flags & MDPD_FLAG_TMA_STAGING) ? 3u : ((h->prm.flags & MDPD_FLAG_CPASYNC_STAGING) ? 0u : 1u);
   h->chain_launches = h->direct ? 8u : 9u;  // reset, count, 3 x scan, fill, permute, recipe [, list]
   // Tile shape: the largest candidate that still gives every SM work and whose most populated tile + halo fits in
   // shared memory (checked on the device after the sort).

@@ -39,10 +39,13 @@ def make_case(seed):
     return dict(params=p, pos=pos, vel=vel, type=typ)
 
 
+@pytest.mark.parametrize("direct", [False, True])
 @pytest.mark.parametrize("seed", range(12))
-def test_random_case(gpu, seed):
+def test_random_case(gpu, seed, direct):
     from oracle.mdpd_ref import RefSim
     c = make_case(seed)
+    if direct:
+        c["params"]["flags"] = 2   # MDPD_FLAG_DIRECT: the list-free path
     s = gpu.Simulation(c["params"])
     s.load_particles(c["pos"], c["vel"], c["type"])
     r = RefSim(c["params"])

@@ -39,8 +39,11 @@ def ref_sim(c, step=0, brute=False):
     return s
 
 
-def gpu_sim(pk, c, step=0):
-    s = pk.Simulation(c["params"])
+def gpu_sim(pk, c, step=0, direct=False):
+    prm = dict(c["params"])
+    if direct:
+        prm["flags"] = 2        # MDPD_FLAG_DIRECT: the list-free path
+    s = pk.Simulation(prm)
     md = None if c.get("mask") is None else c["mask"].shape[::-1]
     s.load_particles(c["pos"], c["vel"], c["type"], mask_dims=md)
     if c.get("mask") is not None:
@@ -102,12 +105,13 @@ def test_pair_sets_quantised_inputs_identical(gpu, box, n, seed):
     g.close()
 
 
+@pytest.mark.parametrize("direct", [False, True])
 @pytest.mark.parametrize("cfg", [0, 1])
-def test_pair_sets_random_fp32_inputs(gpu, cfg):
+def test_pair_sets_random_fp32_inputs(gpu, cfg, direct):
     """random fp32 positions; the oracle gets the same values upcast.  Sets identical except pairs
     within 4 ulp of a cut-off (|r^2/rcut^2 - 1| < 4 * 2^-23), which are listed and must be few."""
     c = wl.make_config(cfg)
-    g, r = gpu_sim(gpu, c), ref_sim(c)
+    g, r = gpu_sim(gpu, c, direct=direct), ref_sim(c)
     x = c["pos"].astype(np.float64)
     box = np.asarray(c["params"]["box"])
     for rcut in (0.75, 1.0, 1.25):
@@ -125,12 +129,13 @@ def test_pair_sets_random_fp32_inputs(gpu, cfg):
 
 
 # --------------------------------------------------------------------------- (2) density and force, same state
+@pytest.mark.parametrize("direct", [False, True])
 @pytest.mark.parametrize("cfg,step", [(0, 0), (0, 17), (1, 3), (2, 5)])
-def test_density_force_parity_configs(gpu, cfg, step):
+def test_density_force_parity_configs(gpu, cfg, step, direct):
     """rho and F (Eq. 1 + dissipative + hashed random, P:L186 body force) on BASELINE configs
     0, 1, 2 from identical fp32-valued positions / velocities: max error <= 1e-4 RMS."""
     c = wl.make_config(cfg)
-    g, r = gpu_sim(gpu, c, step), ref_sim(c, step)
+    g, r = gpu_sim(gpu, c, step, direct=direct), ref_sim(c, step)
     sg, sr = g.get_state(), r.get_state()
     assert_rho_force_parity(sg, sr, what=f"cfg{cfg}")
     # frozen particles: v = 0 (R8); wall-wall forces skipped, so a wall particle deep in the wall feels only fluid
@@ -140,10 +145,11 @@ def test_density_force_parity_configs(gpu, cfg, step):
     g.close()
 
 
-def test_density_force_parity_pore_network_small(gpu):
+@pytest.mark.parametrize("direct", [False, True])
+def test_density_force_parity_pore_network_small(gpu, direct):
     """Config 3's recipe at 32^3 voxels (box 16^3, ~8.6 k fluid + wall shell): mask, frozen shell, body force."""
     c = wl.make_pore_network(nvox=32, corr=3.0, seed=wl.BASE_SEED + 3)
-    g, r = gpu_sim(gpu, c, 2), ref_sim(c, 2)
+    g, r = gpu_sim(gpu, c, 2, direct=direct), ref_sim(c, 2)
     assert_rho_force_parity(g.get_state(), r.get_state(), what="pore32")
     g.close()
 
