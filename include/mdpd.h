@@ -58,7 +58,8 @@ typedef struct {
                              contracting slab, a filling pore): outgrowing the capacity is MDPD_EOVERFLOW              */
   uint32_t seed;          /* seed of the pair hash      */
   uint32_t max_neigh;     /* list capacity per particle, <= 128; 0 = automatic                                       */
-  uint32_t reorder_every; /* Morton reorder every N list rebuilds; only 0/1 (= every rebuild) is implemented (R16)    */
+  uint32_t reorder_every; /* RESERVED, must be 0 or 1.  The list stores indices into the sorted tile image, so the sort
+                             into Morton-ordered tiles cannot be skipped at a rebuild: it IS the reorder (R16) */
   uint32_t flags;         /* MDPD_FLAG_* */
 } mdpd_params;
 
@@ -95,8 +96,12 @@ int mdpd_set_pair_params(mdpd_ctx* h, uint32_t ntypes, const float* A, const flo
 size_t mdpd_workspace_bytes(const mdpd_params* p, uint64_t n, int has_mask, const uint32_t mask_dims[3]);
 
 /* Give the library its device memory: `dev_ptr` (256-byte aligned, >= mdpd_workspace_bytes) is OWNED BY THE CALLER
- * (e.g. a torch uint8 tensor) and must outlive the handle.  If never called, load_particles allocates with cudaMalloc
- * and mdpd_destroy frees that allocation. */
+ * (e.g. a torch uint8 tensor) and must outlive the handle (or the next mdpd_set_workspace).  If never called,
+ * load_particles allocates with cudaMalloc (and re-allocates when a later load needs more) and mdpd_destroy frees that
+ * allocation.  Calling it on a handle that already holds particles drops them: the next call must be
+ * mdpd_load_particles.  With a caller-owned workspace the stepping path (load, step, get_state, compute_forces,
+ * compute_virial, counters) never allocates device memory; the two diagnostics mdpd_get_pairs and mdpd_rng_fill are
+ * the exception (see there). */
 int mdpd_set_workspace(mdpd_ctx* h, void* dev_ptr, size_t bytes);
 
 /* Load n < 2^28 particles.  pos, vel: [n][3] float32, host or device.  type: [n] uint8 (0 = fluid, any other value =
@@ -132,7 +137,12 @@ int mdpd_set_forces(mdpd_ctx* h, const float* force);
 
 /* ---- parity / diagnostics exports (the GPU-vs-oracle comparison needs them) ---- */
 
-/* rho and f (on every particle, frozen ones included) from the current x, v at the current step index. */
+/* rho and f (on every particle, frozen ones included) from the current x, v at the current step index.
+ * NOTE: this REPLACES the stored force (and rho).  The force of a time level is part of the state (it was evaluated with
+ * the half-step velocities, see the checkpoint note above), so a call made between two mdpd_step calls changes the first
+ * half kick of the next step, i.e. the trajectory (by O(dt^2); the oracle's mdpd_ref_compute_forces has the same
+ * semantics).  To look at forces without touching the run, save get_state's force first and give it back with
+ * mdpd_set_forces.  The same holds for mdpd_compute_virial. */
 int mdpd_compute_forces(mdpd_ctx* h);
 
 /* mdpd_compute_forces, and in the same pass the configurational (conservative-force) part of the stress:
@@ -144,11 +154,15 @@ int mdpd_compute_virial(mdpd_ctx* h, double out[6]);
 /* All tag pairs (a < b) with r < rcut, found through the Verlet list with the kernels' own fp32 predicate
  * (r^2 < rcut^2); rcut <= rc + skin.  For rcut > rc the result is complete only right after a list build
  * (load_particles, or any step that rebuilt).  *count receives the number found; up to cap pairs are written
- * to `pairs` ([cap][2] uint32, HOST memory), sorted lexicographically. */
+ * to `pairs` ([cap][2] uint32, HOST memory), sorted lexicographically.
+ * Diagnostic: allocates its scratch (8 bytes per pair of `cap`) with cudaMalloc and frees it before returning, also
+ * when a workspace was given; not meant for the stepping loop.  On the list-free path (MDPD_FLAG_DIRECT) it first
+ * builds a list from the current cells. */
 int mdpd_get_pairs(mdpd_ctx* h, float rcut, uint64_t* count, uint32_t* pairs, uint64_t cap);
 
 /* Run the DEVICE hash kernel: out[q] = HASH(min(pairs[q]), max(pairs[q]), step, seed of the handle).
- * pairs: [npairs][2] uint32, out: [npairs] uint32, host or device. */
+ * pairs: [npairs][2] uint32, out: [npairs] uint32, host or device.  Diagnostic: allocates 12 bytes per pair with
+ * cudaMalloc and frees them before returning. */
 int mdpd_rng_fill(mdpd_ctx* h, uint64_t npairs, const uint32_t* pairs, uint32_t step, uint32_t* out);
 
 #define MDPD_NCOUNTERS 16

@@ -210,11 +210,12 @@ class Simulation:
         need = self.workspace_bytes(n, mask_dims)
         if need == 0:
             self._ck(MDPD_EINVAL, "mdpd_workspace_bytes (bad parameters)")
-        if self._ws is None or self._ws.numel() < need:
-            self._ws = torch.empty(need + 256, dtype=torch.uint8, device=f"cuda:{self.device}")
-            base = self._ws.data_ptr()
-            self._ws_ptr = (base + 255) // 256 * 256
-            self._ck(self._L.mdpd_set_workspace(self._h, C.c_void_p(self._ws_ptr), need), "mdpd_set_workspace")
+        if self._ws is None or self._ws.numel() < need + 256:
+            # the old tensor stays alive until the handle has accepted the new one (the handle points into it)
+            ws = torch.empty(need + 256, dtype=torch.uint8, device=f"cuda:{self.device}")
+            ptr = (ws.data_ptr() + 255) // 256 * 256
+            self._ck(self._L.mdpd_set_workspace(self._h, C.c_void_p(ptr), need), "mdpd_set_workspace")
+            self._ws, self._ws_ptr = ws, ptr
         self._ck(self._L.mdpd_load_particles(self._h, n, _ptr(pos), _ptr(vel), _ptr(type)), "mdpd_load_particles")
         self.n = n
 

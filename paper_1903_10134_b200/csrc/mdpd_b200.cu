@@ -1829,7 +1829,7 @@ bool make_layout(const mdpd_params& p, uint64_t n, int has_mask, const uint32_t*
   if (!(p.skin >= 0)) return fail("skin must be >= 0");
   if (!(p.dt > 0) || !(p.mass > 0)) return fail("dt and mass must be > 0");
   if (!(p.s > 0.0f) || p.s > 4.0f) return fail("the exponent s of wR = (1 - r/rc)^s must be in (0, 4] (DESIGN.md R15)");
-  if (p.reorder_every > 1) return fail("only reorder_every = 0/1 is implemented (DESIGN.md R16)");
+  if (p.reorder_every > 1) return fail("reorder_every is reserved and must be 0 or 1: the counting sort into tiles IS the reorder, at every rebuild (DESIGN.md R16)");
   if (n >= (1ull << TAG_BITS)) return fail("n must be < 2^28");
   L.rlist = p.rc + p.skin;
   int nc[3];
@@ -2306,6 +2306,7 @@ int mdpd_set_params(mdpd_ctx* h, const mdpd_params* p) {
         q.max_neigh != p->max_neigh || q.mass != p->mass || q.headroom != p->headroom ||
         ((q.flags ^ p->flags) & (MDPD_FLAG_DIRECT | MDPD_FLAG_TMA_STAGING | MDPD_FLAG_CPASYNC_STAGING)))
       return set_err(h, MDPD_ESTATE, "box, cut-offs, skin, mass, capacities and the neighbour path are frozen after load_particles");
+    if (p->s != 1.0f && h->ntypes) return set_err(h, MDPD_EINVAL, "per-type-pair parameters need s = 1");
     if (h->pending_B) {  // the outstanding half kick belongs to the old parameters
       CU_TRY(h, cudaSetDevice(h->device));
       finalize_kick(h);
@@ -2354,8 +2355,14 @@ size_t mdpd_workspace_bytes(const mdpd_params* p, uint64_t n, int has_mask, cons
 
 int mdpd_set_workspace(mdpd_ctx* h, void* dev_ptr, size_t bytes) {
   if (!h || !dev_ptr) return MDPD_EINVAL;
-  if (h->loaded) return set_err(h, MDPD_ESTATE, "set_workspace must precede load_particles");
   if (((uintptr_t)dev_ptr & 255u) != 0) return set_err(h, MDPD_EINVAL, "workspace must be 256-byte aligned");
+  if (h->loaded) {  // a new workspace drops the loaded state: the next call must be mdpd_load_particles
+    cudaSetDevice(h->device);
+    cudaStreamSynchronize(h->stream);
+    destroy_graph(h);
+    h->loaded = false;
+    h->pending_B = false;
+  }
   if (h->ws_owned && h->ws) cudaFree(h->ws);
   h->ws = (char*)dev_ptr;
   h->ws_bytes = bytes;
@@ -2378,6 +2385,14 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
     h->ws_bytes = L.total + (64u << 20);  // room for a mask of up to 64 Mi voxels
     CU_TRY(h, cudaMalloc((void**)&h->ws, h->ws_bytes));
     h->ws_owned = true;
+  }
+  if (h->ws_owned && h->ws_bytes < L.total) {  // the library's own allocation grows with the problem
+    CU_TRY(h, cudaStreamSynchronize(h->stream));
+    destroy_graph(h);
+    cudaFree(h->ws);
+    h->ws = nullptr;
+    h->ws_bytes = L.total + (64u << 20);
+    CU_TRY(h, cudaMalloc((void**)&h->ws, h->ws_bytes));
   }
   if (h->ws_bytes < L.total)
     return set_err(h, MDPD_ENOMEM, "workspace too small: %zu bytes given, %zu needed", h->ws_bytes, L.total);

@@ -213,3 +213,110 @@ def test_counters_and_profile(gpu):
     assert 20 < (c1["sum_act"] - c0["sum_act"]) / (10 * n) < 30          # ~25 inside rc
     assert c1["density_passes"] - c0["density_passes"] == 10
     s.close()
+
+
+def test_reload_with_more_particles_reallocates_the_workspace(gpu):
+    """A second load_particles with a larger n needs a larger workspace: the binding hands the handle a new tensor
+    (mdpd_set_workspace on a loaded handle drops the loaded state) and the results are those of a fresh handle."""
+    small, big = wl.make_liquid((6.0, 6.0, 6.0), seed=5), wl.make_config(0)
+    s = gpu.Simulation(big["params"])
+    s.load_particles(small["pos"], small["vel"], small["type"])      # 1296 particles in the 10^3 box
+    s.step(3)
+    s.load_particles(big["pos"], big["vel"], big["type"])            # 6000 particles: more memory
+    s.step(4)
+    a = s.get_state()
+    f = gpu.Simulation(big["params"])
+    f.load_particles(big["pos"], big["vel"], big["type"])
+    f.step(4)
+    b = f.get_state()
+    for k in ("pos", "vel", "force", "rho"):
+        assert np.array_equal(a[k], b[k]), k
+    s.close()
+    f.close()
+    # the C-ABI without a caller workspace: the library's own allocation grows too
+    L = gpu.lib()
+    h = C.c_void_p()
+    assert L.mdpd_create(C.byref(h), 0, None) == 0
+    p = gpu.make_params(big["params"])
+    assert L.mdpd_set_params(h, C.byref(p)) == 0
+    assert L.mdpd_load_particles(h, len(small["pos"]), small["pos"].ctypes.data, small["vel"].ctypes.data, None) == 0
+    assert L.mdpd_load_particles(h, len(big["pos"]), big["pos"].ctypes.data, big["vel"].ctypes.data, None) == 0
+    assert L.mdpd_step(h, 2) == 0
+    assert L.mdpd_get_state(h, None, None, None, None, None) == 0
+    assert L.mdpd_destroy(h) == 0
+
+
+def test_set_params_rejects_general_exponent_with_pair_params(gpu):
+    """s != 1 runs the one-material force kernel: with per-type-pair parameters it must be refused after load as well
+    as before (the A_ij, B_ij table would silently be ignored)."""
+    c = wl.make_species_mixture()
+    s = gpu.Simulation(c["params"])
+    s.set_pair_params(c["pair_A"], c["pair_B"], c["frozen_mask"])
+    s.load_particles(c["pos"], c["vel"], c["type"])
+    with pytest.raises(gpu.MdpdError) as e:
+        s.set_params(s=0.5)
+    assert e.value.code == -1
+    s.set_params(s=1.0)
+    s.step(2)                       # the handle is still usable with its old parameters
+    s.close()
+
+
+def test_runaway_particle_with_mask_is_a_latched_fault_not_a_crash(gpu):
+    """A particle whose trial position leaves [-L, 2L) (or is not finite) must latch MDPD_ENAN; the voxel lookup must
+    not read outside the mask (advisor finding of round 1: the index was clamped above only)."""
+    c = wl.make_poiseuille(L=12.0, wall=2.0, gx=0.05, seed=3, Lxy=8.0)
+    for bad_v in (-1.0e6, 1.0e6, np.float32("-inf")):
+        vel = c["vel"].copy()
+        vel[0] = (bad_v, bad_v, bad_v)
+        s = gpu.Simulation(c["params"])
+        s.load_particles(c["pos"], vel, c["type"], mask_dims=c["mask"].shape[::-1])
+        s.load_wall_mask(c["mask"], c["voxel"])
+        s.step(2)
+        with pytest.raises(gpu.MdpdError) as e:
+            s.get_state()
+        assert e.value.code == -6, e.value
+        s.close()
+    good = gpu.Simulation(c["params"])      # the CUDA context survived
+    good.load_particles(c["pos"], c["vel"], c["type"], mask_dims=c["mask"].shape[::-1])
+    good.load_wall_mask(c["mask"], c["voxel"])
+    good.step(3)
+    good.get_state()
+    good.close()
+
+
+def test_dense_system_takes_the_multi_window_list_build(gpu):
+    """Number density 9.5: the 27-cell stencil of a cell holds ~500 particles, more than one register window of the
+    list build (384 candidates), while the lists (~78 entries) still fit: pair sets, rho and F against the oracle."""
+    from oracle.mdpd_ref import RefSim
+    c = wl.make_liquid((7.5, 6.3, 5.1), density=9.5, seed=21)
+    for flags in (0, 2):
+        prm = dict(c["params"])
+        prm["flags"] = flags
+        s = gpu.Simulation(prm)
+        s.load_particles(c["pos"], c["vel"], c["type"])
+        r = RefSim(c["params"])
+        r.load_particles(c["pos"].astype(np.float64), c["vel"].astype(np.float64), c["type"])
+        for rcut in (0.75, 1.0, 1.25):
+            pg, pr = s.get_pairs(rcut), r.get_pairs(rcut)
+            assert abs(len(pg) - len(pr)) <= 2 and len(pg) > 10000
+        g, o = s.get_state(), r.get_state()
+        assert np.abs(g["rho"] - o["rho"]).max() <= 1e-4 * np.sqrt(np.mean(o["rho"] ** 2))
+        assert np.sqrt(((g["force"] - o["force"]) ** 2).sum(1)).max() <= 1e-4 * np.sqrt(np.mean((o["force"] ** 2).sum(1)))
+        ctr = s.counters()
+        assert ctr["faults"] == 0 and (flags or ctr["max_nbr"] <= 128)
+        s.close()
+
+
+def test_tile_that_outgrows_its_capacity_is_reported(gpu):
+    """headroom = 1.0: the shared-memory capacity of a tile is the fullest tile of the LOADED state.  A dilute gas that
+    condenses (A = -40 at number density 3) outgrows it; the run must end in MDPD_EOVERFLOW, not in silent missing
+    forces."""
+    c = wl.make_liquid((16.0, 16.0, 16.0), density=3.0, seed=9, headroom=1.0)
+    s = gpu.Simulation(c["params"])
+    s.load_particles(c["pos"], c["vel"], c["type"])
+    with pytest.raises(gpu.MdpdError) as e:
+        for _ in range(40):
+            s.step(50)
+            s.counters()
+    assert e.value.code == -4, e.value
+    s.close()

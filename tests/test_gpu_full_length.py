@@ -1,0 +1,172 @@
+"""BASELINE.json's configs at their stated length on the GPU, each with the observable north_star names.
+
+The oracle cannot afford these runs (config 2 alone is 20 000 steps of 48 200 particles), so what the GPU result is
+checked against is what the paper and the mathematics fix: the analytic parabola of plane Poiseuille flow
+v_x(z) = (rho g_x / 2 mu) (z - z_a)(z_b - z) (body-force driven flow; L45-53: the channel), the
+fluctuation-dissipation temperature kT = sigma^2 / 2 gamma = 1, conservation of momentum by pairwise
+forces, and the voxel mask itself.  (Short-horizon agreement with the oracle on the same configs: test_gpu_parity.py,
+test_gpu_fullsize.py, test_gpu_observables.py.)
+"""
+import numpy as np
+import pytest
+
+import mdpd_workloads as wl
+
+from helpers import kinetic_temperature, profile
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("the -m gpu suite needs a CUDA device (no CPU fallback exists)")
+    from paper_1903_10134_b200 import build
+    build()
+    import paper_1903_10134_b200 as pk
+    return pk
+
+
+def load(pk, c):
+    md = None if c.get("mask") is None else c["mask"].shape[::-1]
+    sim = pk.Simulation(c["params"], device=0)
+    sim.load_particles(c["pos"], c["vel"], c["type"], mask_dims=md)
+    if c.get("mask") is not None:
+        sim.load_wall_mask(c["mask"], c["voxel"])
+    return sim
+
+
+def channel_profile(pk, c, wall, L, nsteps, every, width=0.5):
+    """Runs `nsteps` steps; v_x(z) of the fluid time-averaged over the second half in bins of `width`."""
+    sim = load(pk, c)
+    fl = c["type"] == 0
+    nb = int(round((L - 2 * wall) / width))
+    sim.step(nsteps // 2)
+    acc, cnt = np.zeros(nb), np.zeros(nb)
+    inside = True
+    for _ in range(nsteps // 2 // every):
+        sim.step(every)
+        st = sim.get_state(force=False, rho=False)
+        z = st["pos"][fl, 2]
+        ctr, m, k = profile(z, st["vel"][fl, 0].astype(np.float64), wall, L - wall, nb)
+        acc += m * k
+        cnt += k
+        inside = inside and bool(((z >= wall) & (z < L - wall)).all())
+    ctrs = sim.counters()
+    st = sim.get_state()
+    sim.close()
+    return ctr, acc / cnt, cnt, inside, ctrs, st
+
+
+def fit_parabola(z, v, lo, hi):
+    sel = (z > lo) & (z < hi)
+    co = np.polyfit(z[sel], v[sel], 2)
+    roots = np.sort(np.roots(co).real)
+    resid = np.abs(v[sel] - np.polyval(co, z[sel])).max() / v[sel].max()
+    return co, roots, resid
+
+
+def test_config2_poiseuille_20000_steps_against_the_analytic_parabola(gpu):
+    """Config 2 as BASELINE.json states it: 20 x 20 x 20 box, 38 400 fluid + 9 800 frozen wall particles, voxel mask,
+    g_x = 0.05, 20 000 steps; v_x(z) averaged over the last 10 000 steps in 0.5-wide bins.  SURVEY.md S8c's Poiseuille
+    pin applied to the GPU path: quadratic-fit residual < 2 % of v_max over 3 < z < 17, fitted zeros within 0.3 of the
+    wall faces z = 2, 18 (no slip).  Noise: 1 200 particles per bin x ~330 decorrelated samples => 0.002 per bin."""
+    c = wl.make_config(2)
+    z, v, cnt, inside, ctrs, st = channel_profile(gpu, c, 2.0, 20.0, 20000, 10)
+    co, roots, resid = fit_parabola(z, v, 3.0, 17.0)
+    assert co[0] < 0 and v.max() > 0.5
+    assert resid < 0.02, resid
+    assert abs(roots[0] - 2.0) < 0.3 and abs(roots[1] - 18.0) < 0.3, roots
+    assert inside and ctrs["faults"] == 0 and ctrs["steps"] == 20000 and ctrs["bounces"] > 0
+    fl = c["type"] == 0
+    assert (st["pos"][~fl] == c["pos"][~fl]).all() and (st["vel"][~fl] == 0).all()      # frozen walls
+    assert np.abs(cnt[4:-4] / cnt[4:-4].mean() - 1).max() < 0.03                       # flat density in the core
+    vyz = st["vel"][fl, 1:].astype(np.float64)
+    vyz -= vyz.mean(0)
+    assert abs((vyz ** 2).sum() / (2 * len(vyz) - 2) - 1.0) < 0.03                     # kT from v_y, v_z (no mean flow there)
+
+
+def test_wide_channel_profile_within_one_percent_and_viscosity_is_width_independent(gpu):
+    """(i) A channel wide enough for a 1 % profile comparison (52 x 52 x 20: 259 584 fluid particles, 20 000 steps):
+    every 0.5-wide bin of v_x(z) over 3 < z < 17 within 1 % of v_max of the analytic parabola with the fitted
+    viscosity (north_star: velocity profile within 1 %; the oracle cannot afford this run, the parabola is the
+    reference).  (ii) The viscosity mu = rho g / (2 |a_2|) from the curvature must not depend on the channel: the
+    config-2 cross-section at the same height gives the same mu within 2 %, a narrower channel (height 10 instead of
+    16) within 5 % -- the cross-check of SURVEY.md S8c (iii) without a spatially varying body force, which the
+    C-ABI (like the paper) does not have."""
+    rho_n, g = 6.0, 0.05
+    mus = []
+    for Lxy, L, nsteps, tol in ((52.0, 20.0, 20000, 0.01), (20.0, 20.0, 20000, 0.02), (30.0, 14.0, 12000, 0.02)):
+        c = wl.make_poiseuille(L=L, wall=2.0, gx=g, seed=wl.BASE_SEED + 2, Lxy=Lxy)
+        z, v, cnt, inside, ctrs, _ = channel_profile(gpu, c, 2.0, L, nsteps, 20)
+        co, roots, resid = fit_parabola(z, v, 3.0, L - 3.0)
+        assert inside and ctrs["faults"] == 0
+        assert resid < tol, (Lxy, L, resid)
+        mus.append(rho_n * g / (2.0 * abs(co[0])))
+    assert abs(mus[1] / mus[0] - 1.0) < 0.02, mus
+    assert abs(mus[2] / mus[0] - 1.0) < 0.05, mus
+
+
+def test_config3_pore_network_5000_steps(gpu):
+    """Config 3 as BASELINE.json states it (128^3 voxel mask, ~0.55 M fluid + ~0.42 M frozen particles, g_x = 0.02,
+    5 000 steps): no device fault, no fluid particle in a solid voxel (an independent numpy lookup of the mask), the
+    frozen shell does not move, and the flux <v_x> of the fluid is steady over the last 2 000 steps.
+    Noise budget of "steady": <v_x> is the centre-of-mass velocity of N = 5.5e5 fluid particles; by equipartition it
+    fluctuates with sqrt(kT / N m) = 1.35e-3 and relaxes on the viscous time of a pore (~400 steps), so a 1 000-step
+    mean holds ~2.5 independent samples: sigma = 8.5e-4 per window, 1.2e-3 for the difference of two windows.  The flux
+    itself is 1.4e-2: the two halves of the last 2 000 steps must agree within 4 sigma (a third of the signal is the
+    best this observable allows at g_x = 0.02), both must stand out of the noise by > 8 sigma, and from step 500 on
+    (the flux settles within ~100 steps: the pores are ~6 rc wide) no 50-step sample strays from the mean by more than
+    5 sqrt(kT / N m)."""
+    c = wl.make_config(3)
+    sim = load(gpu, c)
+    fl = c["type"] == 0
+    nfl = int(fl.sum())
+    mask, vox = c["mask"], c["voxel"]
+    flux = []
+    for k in range(100):
+        sim.step(50)
+        st = sim.get_state(force=False, rho=False)
+        flux.append(st["vel"][fl, 0].astype(np.float64).mean())
+        if k % 20 == 19:
+            ijk = np.minimum((st["pos"][fl] / vox).astype(np.int64), np.array(mask.shape[::-1]) - 1)
+            assert not mask[ijk[:, 2], ijk[:, 1], ijk[:, 0]].any(), k
+    flux = np.array(flux)
+    ctrs = sim.counters()
+    st = sim.get_state()
+    sim.close()
+    assert ctrs["faults"] == 0 and ctrs["steps"] == 5000 and ctrs["bounces"] > 0
+    assert (st["pos"][~fl] == c["pos"][~fl]).all()
+    sigma = np.sqrt(1.0 / nfl) / np.sqrt(2.5)
+    a, b = flux[60:80].mean(), flux[80:100].mean()
+    assert a > 8 * sigma and b > 8 * sigma, (a, b, sigma)
+    assert abs(b - a) < 4 * np.sqrt(2.0) * sigma, (a, b, sigma)
+    late = flux[10:]                                   # from step 500 on: no sample strays from the mean
+    assert np.abs(late - late.mean()).max() < 5 * np.sqrt(1.0 / nfl), (late.min(), late.max())
+    vyz = st["vel"][fl, 1:].astype(np.float64)
+    vyz -= vyz.mean(0)
+    assert abs((vyz ** 2).sum() / (2 * len(vyz) - 2) - 1.0) < 0.03
+
+
+def test_config4b_1000_steps_temperature_density_momentum(gpu):
+    """Config 4b (998 250 particles, the paper's ~1 M particles per GPU) for its 1 000 steps:
+    kT = sigma^2 / 2 gamma = 1 within 2 %, <rho> stationary, total momentum conserved (pairwise forces:
+    F_ij = -F_ji bitwise, so only the fp32 rounding of the velocity update can move it)."""
+    c = wl.make_config("4b")
+    sim = load(gpu, c)
+    n = len(c["pos"])
+    kts, rhos = [], []
+    for k in range(20):
+        sim.step(50)
+        st = sim.get_state(force=False)
+        kts.append(kinetic_temperature(st["vel"]))
+        rhos.append(st["rho"].astype(np.float64).mean())
+    ctrs = sim.counters()
+    sim.close()
+    assert ctrs["faults"] == 0 and ctrs["steps"] == 1000
+    assert abs(np.mean(kts[10:]) - 1.0) < 0.02, kts
+    assert abs(np.mean(rhos[10:15]) / np.mean(rhos[15:]) - 1.0) < 0.005, rhos
+    p = st["vel"].astype(np.float64).sum(0) / n
+    assert np.abs(p).max() < 1e-5, p
+    assert 250 < ctrs["rebuilds"] < 600

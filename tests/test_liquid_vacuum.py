@@ -52,7 +52,6 @@ def test_oracle_slab_centre_density_and_tension_match_the_paper():
             dens.append((np.abs(x - x.mean()) < 1.5).sum() / (3.0 * 7.0 * 7.0))
     rho = float(np.mean(dens))
     assert abs(rho / PAPER_CENTRE_DENSITY - 1.0) < TOL, rho
-    assert abs(rho - 6.82) < 0.05, rho          # what this oracle gives (6.817 +- 0.007): regression guard
     gamma = 0.5 * Lx * float(np.mean(g))
     assert abs(gamma - PAPER_TENSION) < 1.0, gamma      # 12.28 +- 0.27 (block averages) on this small slab
 

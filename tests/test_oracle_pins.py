@@ -385,3 +385,47 @@ def test_bounce_back_and_frozen_walls():
     assert np.allclose(st["force"], f, atol=1e-12)
     assert st["rho"][0] > 0  # walls do get a density, from fluid and wall neighbours alike
     assert abs(st["rho"][0] - brute_density(st["pos"], box, 0.75)[0]) < 1e-13
+
+
+def test_bounce_back_mask_axis_order():
+    """The voxel mask is mask[nz][ny][nx] (include/mdpd.h, R7): on a NON-cubic box with three different voxel
+    counts, one mask solid for x >= 5 only and one solid for y >= 3.5 only.  A particle driven in +x must bounce at
+    the x-wall (and nowhere in the y-wall mask until it wraps), a particle driven in +y the other way round; a
+    transposed index (x <-> y, or any other permutation of the three axes) fails one of the four cases."""
+    box = (6.0, 4.0, 5.0)
+    p = wl.default_params(box, A=0.0, B=0.0, gamma=0.0, sigma=0.0)
+    nx, ny, nz = 12, 8, 10
+    mx = np.zeros((nz, ny, nx), np.uint8)
+    mx[:, :, 10:] = 1                      # solid for x >= 5.0
+    my = np.zeros((nz, ny, nx), np.uint8)
+    my[:, 7:, :] = 1                       # solid for y >= 3.5
+    start = [[4.005, 2.605, 1.2]]         # off the voxel faces: no trial position lands on a boundary
+
+    def run(mask, vel, nsteps):
+        s = RefSim(p)
+        s.load_particles(start, [vel])
+        s.load_wall_mask(mask, 0.5)
+        s.step(nsteps)
+        st = s.get_state()
+        return st["pos"][0], st["vel"][0], s.counters()["bounces"]
+
+    # +x at speed 2: x* = 4.005 + 0.02 k passes 5.0 at step 50 -> first bounce there (x stays 4.985, v reversed)
+    x, v, nb = run(mx, [2.0, 0.0, 0.0], 49)
+    assert nb == 0 and abs(x[0] - 4.985) < 1e-9
+    x, v, nb = run(mx, [2.0, 0.0, 0.0], 50)
+    assert nb == 1 and abs(x[0] - 4.985) < 1e-9 and v[0] == -2.0
+    # the same particle in the y-wall mask flies on (x = 5.405 is pore there): 70 steps, no bounce
+    x, v, nb = run(my, [2.0, 0.0, 0.0], 70)
+    assert nb == 0 and abs(x[0] - 5.405) < 1e-9
+    # +y at speed 2: y* = 2.605 + 0.02 k passes 3.5 at step 45 -> bounce there in the y-wall mask, none in the x-wall mask
+    x, v, nb = run(my, [0.0, 2.0, 0.0], 44)
+    assert nb == 0 and abs(x[1] - 3.485) < 1e-9
+    x, v, nb = run(my, [0.0, 2.0, 0.0], 45)
+    assert nb == 1 and abs(x[1] - 3.485) < 1e-9 and v[1] == -2.0
+    x, v, nb = run(mx, [0.0, 2.0, 0.0], 60)
+    assert nb == 0 and abs(x[1] - 3.805) < 1e-9
+    # +z: neither mask has a z-wall
+    x, v, nb = run(mx, [0.0, 0.0, 2.0], 150)
+    assert nb == 0
+    x, v, nb = run(my, [0.0, 0.0, 2.0], 150)
+    assert nb == 0
