@@ -117,6 +117,19 @@ def oracle_sample_edge(budget_particle_steps):
     return int(min(40, max(6, edge)))
 
 
+def host_cpu():
+    """CPU model and core count of this box, for the oracle timings."""
+    model = "unknown"
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.lower().startswith("model name"):
+                model = line.split(":", 1)[1].strip()
+                break
+    except OSError:
+        pass
+    return {"cpu_model": model, "nproc": os.cpu_count(), "threads_used": 1}
+
+
 def run_oracle_sample(workload, nsteps, edge, warm=0):
     """Times `nsteps` timesteps of the fp64 oracle on a bounded sample of the workload.  Returns (rate, n, seconds)."""
     import mdpd_workloads as wl
@@ -153,8 +166,8 @@ def main_reference(args, rank, world):
             "ms_per_step": 1e3 * dt / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic", "impl": "reference",
             "config": {"workload": workload_name(args.workload, "sampled"), "sample": sample},
-            "cpu_baseline": {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
-                             "sample": f"{sample}; {K} steps per run, one timestep per step"},
+            "cpu_baseline": dict({"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                  "sample": f"{sample}; {K} steps per run, one timestep per step"}, **host_cpu()),
             "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -333,20 +346,42 @@ def main_ours(args, rank, world, local):
     roof["step"] = {"alu_gops": round(win_ops / (tot * 1e-3) / 1e9, 1), "alu_frac": round(win_ops / (tot * 1e-3) / 1e9 / alu_peak, 4),
                     "ops_per_particle_step": round(win_ops / (n * K), 1)}
     roof["ms_per_launch"] = d.get("ms_per_launch")
-    # DRAM bytes per launch of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum) from the committed
-    # ncu --set full capture of this workload, scaled per particle: profiles/r1k_fast_staging_4x4x4.md (config 4a / 4b)
-    ncu_dram_bytes_per_particle = {"4a": {"k_cells_list": 149.6, "k_density": 268.1, "k_force": 126.2, "k_integrate": 94.8},
-                                   "4b": {"k_cells_list": 88.0, "k_density": 232.7, "k_force": 113.0, "k_integrate": 64.5}}
-    # l1tex__data_pipe_lsu_wavefronts_mem_shared (% of peak) of the same captures: the unit that actually limits the two
-    # per-step passes (16-byte gathers from the staged tile); static, from profiles/, not measured live
-    ncu_smem_pipe_frac = {"4a": {"k_density": 0.668, "k_force": 0.729, "k_cells_list": 0.390},
-                          "4b": {"k_density": 0.549, "k_force": 0.656, "k_cells_list": 0.341}}
-    for k, v in ncu_smem_pipe_frac.get(args.workload, {}).items():
-        if k in per_kernel:
-            per_kernel[k]["smem_pipe_frac_ncu"] = v
-    tpp = ncu_dram_bytes_per_particle.get(args.workload, {}).get(dom)
-    roof["traffic"] = None if tpp is None else tpp * n
-    roof["traffic_source"] = None if tpp is None else "ncu --set full capture in profiles/r1k_fast_staging_4x4x4.md"
+    # The bar north_star sets: the density + force passes together against their roofline (ALU: the FFMA issue rate
+    # measured above; HBM: the measured copy bandwidth), from the summed algorithmic work and the summed launch times.
+    dens_k = "k_cells_direct" if args.direct else "k_density"
+    if dens_k in per_kernel and "k_force" in per_kernel:
+        t_df = (per_kernel[dens_k]["ms_per_launch"] + per_kernel["k_force"]["ms_per_launch"]) * 1e-3
+        o_df = algorithmic_ops(dens_k, n, n_list, n_act, n_cand) + algorithmic_ops("k_force", n, n_list, n_act)
+        b_df = algorithmic_bytes(dens_k, n, n_list, n_act) + algorithmic_bytes("k_force", n, n_list, n_act)
+        roof["density_plus_force"] = {"ms": round(t_df * 1e3, 4), "alu_frac": round(o_df / t_df / 1e9 / alu_peak, 4),
+                                      "hbm_frac": round(b_df / t_df / 1e9 / peak_gbs, 4), "target": 0.60}
+    # "as implemented" evaluates every pair from both ends (full list: no atomics, bitwise F_ij = -F_ji, deterministic
+    # sums); the method's minimum is each pair once: half the pair work of every pass
+    roof["method_minimum_frac"] = None if roof.get("frac") is None else round(0.5 * roof["frac"], 4)
+    roof["step"]["alu_frac_method_minimum"] = round(0.5 * roof["step"]["alu_frac"], 4)
+    # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) and the shared-memory data-pipe utilisation come
+    # from the committed ncu --set full capture of this workload, profiles/ncu_r2_<workload>.json, which records the
+    # SHA-256 of the kernel source it was taken from: a capture of another build is reported as stale, not as a number.
+    roof["traffic"], roof["traffic_source"] = None, None
+    try:
+        import hashlib
+        cap = json.load(open(os.path.join(ROOT, "profiles", f"ncu_r2_{args.workload}.json")))
+        src = os.path.join(ROOT, "paper_1903_10134_b200", "csrc", "mdpd_b200.cu")
+        sha = hashlib.sha256(open(src, "rb").read()).hexdigest()
+        if sha != cap.get("kernel_source_sha256"):
+            roof["traffic_source"] = (f"stale: profiles/ncu_r2_{args.workload}.json was captured at commit {cap.get('commit')} "
+                                      "from another version of csrc/mdpd_b200.cu")
+        else:
+            kc = cap.get("kernels", {})
+            for k, v in kc.items():
+                if k in per_kernel:
+                    per_kernel[k]["dram_bytes_per_launch_ncu"] = v.get("dram_bytes_per_launch")
+                    per_kernel[k]["smem_pipe_frac_ncu"] = v.get("smem_pipe_frac")
+            if dom in kc and not args.direct:
+                roof["traffic"] = kc[dom].get("dram_bytes_per_launch")
+            roof["traffic_source"] = f"profiles/ncu_r2_{args.workload}.json (ncu --set full, commit {cap.get('commit')})"
+    except FileNotFoundError:
+        roof["traffic_source"] = f"no capture committed for workload {args.workload}"
     roof["hbm_peak_gbs"] = peak_gbs
     roof["per_kernel"] = per_kernel
 
@@ -393,8 +428,8 @@ def main_ours(args, rank, world, local):
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         edge = oracle_sample_edge(20.0 * 4.0e5 / 20)          # ~20 s: 20 steps of a ~4e5-particle box
         rate, ns, dt, sample = run_oracle_sample(args.workload, 20, edge)
-        line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
-                                "sample": f"{sample}; 20 timesteps in {dt:.1f} s (serial C, fp64)"}
+        line["cpu_baseline"] = dict({"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                     "sample": f"{sample}; 20 timesteps in {dt:.1f} s (serial C, fp64, one thread)"}, **host_cpu())
     sim.close()
     if rank == 0:
         print(json.dumps(line), flush=True)

@@ -27,16 +27,16 @@ def needs_build() -> bool:
     return any(os.path.getmtime(f) > t for f in SRC + HDR + [os.path.abspath(__file__)])
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, defines=()) -> str:
+    """defines: extra -D options, e.g. ("-DMDPD_CHECKS",) for the build with the kernels' own bounds checks."""
     if force or needs_build():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         tmp = LIB + f".tmp{os.getpid()}"
-        extra = os.environ.get("MDPD_NVCC_EXTRA", "").split()   # e.g. "-DTILE_TPB=448" for tuning experiments
-        cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SRC
+        cmd = [nvcc] + NVCC_FLAGS + list(defines) + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SRC
         subprocess.check_call(cmd)
         os.replace(tmp, LIB)
     return LIB
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, defines=[a for a in sys.argv[1:] if a.startswith("-D")]))

@@ -27,6 +27,18 @@ constexpr unsigned ERR_OVERFLOW = 1u;
 constexpr unsigned ERR_NAN = 2u;
 constexpr unsigned ERR_TILE = 4u;  // a tile + halo does not fit the shared-memory capacity
 constexpr unsigned ERR_TYPE = 8u;  // a particle's species index is not below the number of species
+constexpr unsigned ERR_CHECK = 16u;  // -DMDPD_CHECKS: an internal bounds check failed (reported as MDPD_ECUDA)
+// Bounds checks of the kernels' own index arithmetic (every index into the staged image, the row buffers, the lists and
+// the particle arrays), compiled in with -DMDPD_CHECKS (python -m paper_1903_10134_b200.build --force -DMDPD_CHECKS) and
+// run over the whole GPU test suite: this pool has compute-sanitizer closed, see profiles/sanitizer_r2.md.
+#ifdef MDPD_CHECKS
+#define MDPD_CHECK(p, cond)                              \
+  do {                                                   \
+    if (!(cond)) atomicOr(&(p).ctl->err, ERR_CHECK);     \
+  } while (0)
+#else
+#define MDPD_CHECK(p, cond) ((void)0)
+#endif
 // particle word (pos.w): tag (load-order index) | species << 28 | frozen << 31
 constexpr unsigned TAG_BITS = 28, TAG_MASK = (1u << TAG_BITS) - 1u, MAXTYPES = 8;
 constexpr int TPB = 128;           // threads per block of the per-particle kernels
@@ -476,6 +488,7 @@ __global__ void __launch_bounds__(TPB) k_cell_fill(const DevP p) {
   for (unsigned i = blockIdx.x * blockDim.x + threadIdx.x; i < p.N; i += gridDim.x * blockDim.x) {
     unsigned c = p.pcell[i];
     unsigned slot = atomicSub(&p.cell_count[c], 1u) - 1u;  // the histogram counts back down to zero: self-cleaning
+    MDPD_CHECK(p, c < p.ncell && p.cell_start[c] + slot < p.N);
     p.order[p.cell_start[c] + slot] = i;
   }
 }
@@ -500,6 +513,7 @@ __global__ void __launch_bounds__(TPB) k_permute(const DevP p) {
     rank += (ot < tag) ? 1u : 0u;
   }
   const unsigned dst = cs + rank;
+  MDPD_CHECK(p, dst < p.N && i < p.N && ce <= p.N && c < p.ncell);
   p.pos[cur][dst] = x;
   p.vel[cur][dst] = p.vel[src][i];
   p.xbuild[dst] = x;
@@ -677,11 +691,12 @@ __device__ __forceinline__ bool stage_fast(const DevP& p, const TileInfo& T, con
     if (r < nruns && total <= p.tile_cap) {
       const unsigned cnt = R.y >> 16, sb = R.y & 0xFFFFu;
       unsigned io = R.w;
+      MDPD_CHECK(p, sb + cnt <= p.tile_cap && R.x + cnt <= p.N && R.z < 27u && R.w + ((cnt + 31u) >> 5) <= 2u * HTAB);
       for (unsigned c = 0; c < cnt; c += 32, ++io)
         items[io] = make_uint2(R.x + c, (sb + c) | ((min(32u, cnt - c) - 1u) << 16) | (R.z << 21));
     }
   }
-  if (total > p.tile_cap) return false;  // flagged by k_build_list (block-uniform)
+  if (total > p.tile_cap) return false;  // flagged by k_tile_recipe (block-uniform)
   if (threadIdx.x < 27) {
     const unsigned c = threadIdx.x, cx = c % 3u, cy = (c / 3u) % 3u, cz = c / 9u;
     const float ox = tile_origin(T.c0x, p.edge_x), oy = tile_origin(T.c0y, p.edge_y), oz = tile_origin(T.c0z, p.edge_z);
@@ -760,6 +775,7 @@ __device__ __forceinline__ bool stage_bulk(const DevP& p, const TileInfo& T, con
     const uint4 R = rec[r];
     srec[r] = R;
     const unsigned cnt = R.y >> 16, sb = R.y & 0xFFFFu;
+    MDPD_CHECK(p, sb + cnt <= p.tile_cap && R.x + cnt <= p.N && R.z < 27u && r < (unsigned)HTAB);
     if (cnt) {
       asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(pbase + (sb << 4)),
                    "l"(pos + R.x), "r"(cnt << 4), "r"(mb)
@@ -966,6 +982,7 @@ __device__ __forceinline__ bool stage_cells(const DevP& p, const TileInfo& T, co
     if (r < nruns) {
       const unsigned cnt = R.y >> 16, sb = R.y & 0xFFFFu;
       unsigned io = R.w;
+      MDPD_CHECK(p, sb + cnt <= p.tile_cap && R.x + cnt <= p.N && R.z < 27u && R.w + ((cnt + 31u) >> 5) <= 2u * HTAB);
       for (unsigned c = 0; c < cnt; c += 32, ++io)
         items[io] = make_uint2(R.x + c, (sb + c) | ((min(32u, cnt - c) - 1u) << 16) | (R.z << 21));
     }
@@ -1022,7 +1039,7 @@ struct CandRegs {  // one window of candidates: chunk t, this lane
 // own particles [il0, il1) of the cell whose first staged slot is S_cell, against the NCH chunks of the window; particle
 // il appends its hits to row row0 + (il - il0) of the warp's row buffer.  All lanes must call it.  (List-free pass.)
 template <int NCH>
-__device__ __forceinline__ void cell_tests(const CandRegs& C, const float4* img, const unsigned S_cell, const unsigned il0,
+__device__ __forceinline__ void cell_tests(const DevP& p, const CandRegs& C, const float4* img, const unsigned S_cell, const unsigned il0,
                                            const unsigned il1, const unsigned row0, const unsigned rbase_w,
                                            const unsigned row_bytes, unsigned short* rowcnt, const float cut2,
                                            const unsigned rowcap, const unsigned ltmask, const unsigned lane) {
@@ -1043,6 +1060,7 @@ __device__ __forceinline__ void cell_tests(const CandRegs& C, const float4* img,
       const float v = fmaf(C.x[t], ax, fmaf(C.y[t], ay, fmaf(C.z[t], az, C.q[t])));
       const bool hit = v < thr && C.s[t] != self;
       const unsigned b = __ballot_sync(0xffffffffu, hit);
+      MDPD_CHECK(p, na + 2u * __popc(b) <= ra + row_bytes - 16u && row < 32u);
       if (hit) sts_u16(na + 2u * __popc(b & ltmask), C.s[t]);
       na = min(na + 2u * __popc(b), lim);
     }
@@ -1087,12 +1105,14 @@ __device__ __forceinline__ void cell_tests_flush(const DevP& p, const CandRegs& 
         hit = hit && C.s[t] != self;
       }
       const unsigned b = __ballot_sync(0xffffffffu, hit);
+      MDPD_CHECK(p, na + 2u * __popc(b) <= ra + CELLS_ROW0_BYTES);
       if (hit) sts_u16(na + 2u * __popc(b & ltmask), C.s[t]);
       na += 2u * __popc(b);
     }
     __syncwarp();
     unsigned n = (na - ra) >> 1;
     n0 = n;
+    MDPD_CHECK(p, gi0 + (il - il0) < p.N && S_cell + il < p.tile_cap);
     if (LAST) {
       if (n > p.cap) n = 0xFFFFu;  // overflow marker
       if (lane < (((n > p.cap ? 0u : n) + 7u) >> 3)) p.nbr[(size_t)lane * p.N + gi0 + (il - il0)] = lds4u(ra + 16u * lane);
@@ -1116,6 +1136,7 @@ template <bool HAS_WALL, bool ALL>
 __device__ __forceinline__ void direct_entry(const DevP& p, const unsigned ibase, const float4 xi, const unsigned walli,
                                              const unsigned j, const unsigned kaddr, const unsigned sent, float& rho,
                                              unsigned& nin) {
+  MDPD_CHECK(p, j <= p.tile_cap);
   const float4 xj = lds4(ibase + (j << 4));  // padding entries hit the far-away sentinel
   const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
   const float r2 = dx * dx + dy * dy + dz * dz;
@@ -1269,6 +1290,7 @@ __global__ void __launch_bounds__((MODE ? CELLS_MAXW : CELLS_MAXW0) * 32, 2) k_c
             for (int qq = 0; qq < 10; ++qq) r += (f >= rend[qq]) ? 1u : 0u;
             const unsigned rb = __shfl_sync(0xffffffffu, run_b, r), ro = __shfl_sync(0xffffffffu, run_o, r);
             const unsigned cs = f < ncand ? rb + (f - ro) : sent;
+            MDPD_CHECK(p, cs <= p.tile_cap && r <= 10u);
             const float4 xc = img[cs];
             C.x[t] = xc.x;
             C.y[t] = xc.y;
@@ -1327,7 +1349,7 @@ __global__ void __launch_bounds__((MODE ? CELLS_MAXW : CELLS_MAXW0) * 32, 2) k_c
             load_window(win, nch);
 #define CELLS_CASE(K)                                                                                                           \
   case K:                                                                                                                         \
-    cell_tests<K>(C, img, S_cell, r0, r0 + take, rows_used, rbase_w, row_bytes, rowcnt, cut2, rowcap, ltmask, lane);              \
+    cell_tests<K>(p, C, img, S_cell, r0, r0 + take, rows_used, rbase_w, row_bytes, rowcnt, cut2, rowcap, ltmask, lane);              \
     break;
             switch (nch) {
               CELLS_CASE(1) CELLS_CASE(2) CELLS_CASE(3) CELLS_CASE(4) CELLS_CASE(5) CELLS_CASE(6)
@@ -1425,6 +1447,7 @@ template <bool HAS_WALL>
 __device__ __forceinline__ void density_entry(const DevP& p, const unsigned pbase, const float4 xi, const unsigned walli,
                                               const unsigned j, float& rho, unsigned& a0, unsigned& a1, unsigned& a2,
                                               unsigned& a3, unsigned& na, uint4*& ao) {
+  MDPD_CHECK(p, j <= p.tile_cap);
   const float4 xj = lds4(pbase + (j << 4));  // padding entries hit the far-away sentinel
   const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
   const float r2 = dx * dx + dy * dy + dz * dz;
@@ -1497,6 +1520,7 @@ __global__ void __launch_bounds__(DENS_TPB, DENS_MINB) k_density(const DevP p) {
       nxt = rec.y ? p.nbr[os + (rec.x & 0xFFFFu)] : make_uint4(0, 0, 0, 0);
     }
     const unsigned i = os + (rec.x & 0xFFFFu);
+    MDPD_CHECK(p, i < p.N && (rec.x & 0xFFFFu) < nown && (rec.x >> 16) < p.tile_cap && rec.y <= p.cap);
     const float4 xi = sm.spos[rec.x >> 16];
     const unsigned walli = f2u(xi.w) >> 31;
     const unsigned nn = rec.y;
@@ -1599,6 +1623,7 @@ template <bool MULTI, bool VIRIAL, bool SPOW>
 __device__ __forceinline__ void force_entry(const DevP& p, const unsigned pbase, const unsigned vbase, const float4 xi,
                                             const float4 vi, const unsigned tagi, const unsigned j, const HashKeys& K,
                                             const float2* ab, ForceAcc& acc, float* vir) {
+  MDPD_CHECK(p, j <= p.tile_cap);
   const float4 xj = lds4(pbase + (j << 4));
   const float4 vj = lds4(vbase + (j << 4));
   const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
@@ -1690,6 +1715,7 @@ __global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
       continue;
     }
     const unsigned li = rec.x >> 16;
+    MDPD_CHECK(p, i < p.N && (rec.x & 0xFFFFu) < nown && li < p.tile_cap && rec.y <= p.cap);
     const float4 xi = sm.spos[li];
     const unsigned wi = f2u(xi.w);
     const unsigned tagi = wi & TAG_MASK;
@@ -2226,6 +2252,7 @@ int sync_and_check(mdpd_ctx* h) {
   CU_TRY(h, cudaMemcpyAsync(h->h_ctl, h->d.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, h->stream));
   CU_TRY(h, cudaStreamSynchronize(h->stream));
   CU_TRY(h, cudaGetLastError());
+  if (h->h_ctl->err & ERR_CHECK) return set_err(h, MDPD_ECUDA, "an internal bounds check (-DMDPD_CHECKS) failed");
   if (h->h_ctl->err & ERR_TYPE)
     return set_err(h, MDPD_EINVAL, "a particle's type is not below the number of species given to mdpd_set_pair_params");
   if (h->h_ctl->err & ERR_NAN)
