@@ -533,6 +533,9 @@ __global__ void __launch_bounds__(TPB) k_permute(const DevP p) {
 #ifndef DENS_TPB
 #define DENS_TPB 384  // most threads per CTA of the density pass
 #endif
+#ifndef DENS_TPB2
+#define DENS_TPB2 416  // ... of its instantiation for fuller tiles
+#endif
 #ifndef DENS_MINB
 #define DENS_MINB 3
 #endif
@@ -1474,8 +1477,12 @@ __device__ __forceinline__ void density_entry(const DevP& p, const unsigned pbas
 
 constexpr int PRE = 2;  // rounds whose hand-out record and first list chunk are requested before the tile is staged
 
-template <bool HAS_WALL, bool ALL>
-__global__ void __launch_bounds__(DENS_TPB, DENS_MINB) k_density(const DevP p) {
+// TPB: most threads per CTA.  A tile is handed out in two rounds of one particle per thread; 384 threads (three resident
+// CTAs at 56 registers) cover 768 own particles, tiles that hold more (cell edge above 1.255 at number density 6) get
+// the 416-thread instantiation (48 registers, a few spills) instead of a third, almost empty round: 3.38 -> 3.14 ms per
+// launch on config 4a at skin 0.27 (profiles/r2_final.md).
+template <bool HAS_WALL, bool ALL, int TPB>
+__global__ void __launch_bounds__(TPB, DENS_MINB) k_density(const DevP p) {
   extern __shared__ __align__(16) unsigned char smraw[];
   const TileSmem sm = carve_smem(smraw, p.tile_cap, false);
   const unsigned cur = p.ctl->cur;
@@ -1951,6 +1958,7 @@ struct mdpd_ctx {
   int tile_dim[3] = {4, 4, 4};
   unsigned block = 256;          // threads per CTA of the force pass
   unsigned block_dens = 256;     // threads per CTA of the density pass
+  unsigned blocks_from = 0;      // the tile occupancy (max_own) the two block sizes were chosen for
   unsigned cells_warps[2] = {4, 4};  // warps per CTA of k_cells (list build / list-free pass)
   size_t smem_cells[2] = {0, 0};
   bool direct = false;           // MDPD_FLAG_DIRECT: no Verlet list, neighbours straight from the cells every step
@@ -2122,6 +2130,22 @@ void build_tile_ranks(const Layout& L, const int tdim[3], std::vector<unsigned>&
   }
 }
 
+// Threads per CTA of the density / force passes: the own particles of a tile are handed out in two rounds of one
+// particle per thread (every warp gets a long and a short group, see k_cells' tail), so a CTA wants half the fullest
+// tile's population.  The density pass has two instantiations (384 threads at 56 registers, 416 at 48): the wider one
+// only when the fullest tile exceeds what 384 threads cover by more than 5 % (a third, almost empty round in a few tiles
+// costs less than the spills).  Re-evaluated by mdpd_step from the occupancy the last synchronising call saw.
+bool choose_blocks(mdpd_ctx* h, unsigned max_own) {
+  const unsigned half_own = ((max_own + 1u) / 2u + 31u) / 32u * 32u;
+  const unsigned b = std::min<unsigned>(TILE_TPB, std::max(64u, half_own));
+  const unsigned bd = (double)max_own > 2.0 * DENS_TPB * 1.05 ? DENS_TPB2 : std::min<unsigned>(DENS_TPB, std::max(64u, half_own));
+  const bool changed = b != h->block || bd != h->block_dens;
+  h->block = b;
+  h->block_dens = bd;
+  h->blocks_from = max_own;
+  return changed;
+}
+
 // k_cells: mode 0 = Verlet list build, mode 1 = the list-free per-step pass (rho, compact list, hand-out of the force pass)
 int launch_cells(mdpd_ctx* h, int mode, bool all, int always) {
   const DevP& d = h->d;
@@ -2155,9 +2179,15 @@ int launch_rebuild_chain(mdpd_ctx* h, bool with_list = true) {
 int launch_forces(mdpd_ctx* h, bool all, bool virial = false) {
   const DevP& d = h->d;
   if (h->direct) launch_cells(h, 1, all, 1);
-  else if (!h->has_wall) LAUNCH(h, PS_DENSITY, (k_density<false, false><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
-  else if (all) LAUNCH(h, PS_DENSITY, (k_density<true, true><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
-  else LAUNCH(h, PS_DENSITY, (k_density<true, false><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
+  else if (h->block_dens > DENS_TPB) {
+    if (!h->has_wall) LAUNCH(h, PS_DENSITY, (k_density<false, false, DENS_TPB2><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
+    else if (all) LAUNCH(h, PS_DENSITY, (k_density<true, true, DENS_TPB2><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
+    else LAUNCH(h, PS_DENSITY, (k_density<true, false, DENS_TPB2><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
+  } else {
+    if (!h->has_wall) LAUNCH(h, PS_DENSITY, (k_density<false, false, DENS_TPB><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
+    else if (all) LAUNCH(h, PS_DENSITY, (k_density<true, true, DENS_TPB><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
+    else LAUNCH(h, PS_DENSITY, (k_density<true, false, DENS_TPB><<<d.ntiles, h->block_dens, h->smem_pos, h->ls>>>(d)));
+  }
   if (d.s_exp != 1.0f) {  // general exponent of wR: one material, no virial (checked by the callers)
     if (all) LAUNCH(h, PS_FORCE, (k_force<true, false, false, true><<<d.ntiles, h->block, h->smem_posvel, h->ls>>>(d)));
     else LAUNCH(h, PS_FORCE, (k_force<false, false, false, true><<<d.ntiles, h->block, h->smem_posvel, h->ls>>>(d)));
@@ -2510,11 +2540,7 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
                        tdim[0], tdim[1], tdim[2], max_halo, headroom, cap_limit);
       continue;  // try the next smaller tile shape
     }
-    // density / force passes: one thread per own particle of the fullest tile (a tile with more loops)
-    // two rounds on the fullest tile: every warp gets a long and a short group of own particles (see sort_own_by_length)
-    const unsigned half_own = ((h->h_ctl->max_own + 1u) / 2u + 31u) / 32u * 32u;
-    h->block = std::min<unsigned>(TILE_TPB, std::max(64u, half_own));
-    h->block_dens = std::min<unsigned>(DENS_TPB, std::max(64u, half_own));
+    choose_blocks(h, h->h_ctl->max_own);
     // head-room for density fluctuations between rebuilds of a long run
     {
       // at least `headroom` (default 15 %) over the fullest tile of the initial state; beyond that, all the shared memory that does not
@@ -2548,9 +2574,12 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
   CU_TRY(h, (cudaFuncSetAttribute(k_cells<1, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_cells[1])));
   CU_TRY(h, (cudaFuncSetAttribute(k_cells<1, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_cells[1])));
   CU_TRY(h, (cudaFuncSetAttribute(k_cells<1, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_cells[1])));
-  CU_TRY(h, cudaFuncSetAttribute(k_density<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
-  CU_TRY(h, cudaFuncSetAttribute(k_density<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
-  CU_TRY(h, cudaFuncSetAttribute(k_density<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
+  CU_TRY(h, (cudaFuncSetAttribute(k_density<true, true, DENS_TPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos)));
+  CU_TRY(h, (cudaFuncSetAttribute(k_density<true, false, DENS_TPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos)));
+  CU_TRY(h, (cudaFuncSetAttribute(k_density<false, false, DENS_TPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos)));
+  CU_TRY(h, (cudaFuncSetAttribute(k_density<true, true, DENS_TPB2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos)));
+  CU_TRY(h, (cudaFuncSetAttribute(k_density<true, false, DENS_TPB2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos)));
+  CU_TRY(h, (cudaFuncSetAttribute(k_density<false, false, DENS_TPB2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos)));
   CU_TRY(h, cudaFuncSetAttribute(k_pairs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
   CU_TRY(h, cudaFuncSetAttribute(k_force<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
   CU_TRY(h, cudaFuncSetAttribute(k_force<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
@@ -2609,6 +2638,7 @@ int mdpd_step(mdpd_ctx* h, uint32_t nsteps) {
   h->host_step += nsteps;
   if (h->n == 0) return MDPD_OK;
   CU_TRY(h, cudaSetDevice(h->device));
+  if (h->h_ctl->max_own && h->h_ctl->max_own != h->blocks_from && choose_blocks(h, h->h_ctl->max_own)) h->graph_dirty = true;
   const bool graphs = h->use_graph && !h->prof_on && !(h->prm.flags & MDPD_FLAG_NO_GRAPH);
   if (graphs && h->graph_dirty && (nsteps > 1 || h->pending_B)) {
     int rc = build_graph(h);
