@@ -102,6 +102,7 @@ struct DevP {  // passed by value to every kernel
   unsigned cap_act;      // capacity of the per-step in-range (r < rc) lists of the list-free path
   unsigned rows_verlet, rows_direct;  // bytes per row of k_cells' per-warp row buffers (list build / list-free pass)
   float dot_margin;      // slack of the approximate (dot-product form) range test of k_cells, in units of r^2
+  unsigned sms;          // multiprocessors of the device: a tile pass prefetches (L2) for the tile that starts one CTA lifetime later
   unsigned tma_staging;  // bit 0 / bit 1: the density / force pass stages its tile with bulk copies (stage_bulk), else cp.async (stage_fast)
   int ncx, ncy, ncz;
   int mx, my, mz;
@@ -130,6 +131,11 @@ __device__ __forceinline__ float rsqrt_fast(float x) {  // one MUFU.RSQ (2 ulp);
   asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
+__device__ __forceinline__ float sqrt_fast(float x) {  // one MUFU.SQRT; sqrt(0) = 0
+  float y;
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
 __device__ __forceinline__ float u2f(unsigned u) { return __uint_as_float(u); }
 
 // Shared-memory gathers of the hot loops go through 32-bit shared addresses (one LEA per neighbour and array).
@@ -139,6 +145,7 @@ __device__ __forceinline__ float4 lds4(unsigned addr) {
   asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
   return v;
 }
+__device__ __forceinline__ void prefetch_l2(const void* ptr) { asm volatile("prefetch.global.L2 [%0];" ::"l"(ptr)); }
 __device__ __forceinline__ unsigned pin(unsigned v) {  // keeps a loop-invariant value in its register (no rematerialisation)
   asm volatile("" : "+r"(v));
   return v;
@@ -680,17 +687,18 @@ __device__ __forceinline__ void cp_async16(unsigned dst_smem, const void* src) {
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 template <bool WITH_VEL>
-__device__ __forceinline__ bool stage_fast(const DevP& p, const TileInfo& T, const uint4 hdr,
+__device__ __forceinline__ bool stage_fast(const DevP& p, const TileInfo& T, const uint4 hdr, const uint4 R0,
                                            const float4* __restrict__ pos, const float4* __restrict__ vel,
                                            const TileSmem& sm) {
   uint2* const items = (uint2*)sm.hshift;   // [nitems] <= 3 * 36 + tile_cap / 32 <= 2 * HTAB
   float4* const shtab = (float4*)sm.hbase;  // [27] shift of every code
-  // the records are requested together with the header (whose nruns bounds them): one latency for both
+  // R0 = record threadIdx.x, requested by the caller together with the header (whose nruns bounds the records): one
+  // latency for both
   const uint4* __restrict__ rec = p.runs + (size_t)blockIdx.x * p.run_stride + 1;
   const unsigned nrec = p.nrun_max;
   const unsigned total = hdr.x, nruns = hdr.y, nitems = hdr.z & 0xFFFFu;
   for (unsigned r = threadIdx.x; r < nrec; r += blockDim.x) {
-    const uint4 R = rec[r];
+    const uint4 R = r == threadIdx.x ? R0 : rec[r];
     if (r < nruns && total <= p.tile_cap) {
       const unsigned cnt = R.y >> 16, sb = R.y & 0xFFFFu;
       unsigned io = R.w;
@@ -751,7 +759,7 @@ __device__ __forceinline__ bool stage_fast(const DevP& p, const TileInfo& T, con
 // shift of a boundary tile is added afterwards, warp per run.  (mdpd_params.flags & MDPD_FLAG_TMA_STAGING; measured
 // against stage_fast in profiles/r2_staging.md.)
 template <bool WITH_VEL>
-__device__ __forceinline__ bool stage_bulk(const DevP& p, const TileInfo& T, const uint4 hdr,
+__device__ __forceinline__ bool stage_bulk(const DevP& p, const TileInfo& T, const uint4 hdr, const uint4 R0,
                                            const float4* __restrict__ pos, const float4* __restrict__ vel,
                                            const TileSmem& sm) {
   __shared__ __align__(8) unsigned long long mbar;
@@ -775,7 +783,7 @@ __device__ __forceinline__ bool stage_bulk(const DevP& p, const TileInfo& T, con
   __syncthreads();
   const unsigned pbase = smem_addr(sm.spos), vbase = smem_addr(sm.svel);
   for (unsigned r = threadIdx.x; r < nruns; r += blockDim.x) {
-    const uint4 R = rec[r];
+    const uint4 R = r == threadIdx.x ? R0 : rec[r];  // R0: requested by the caller together with the header
     srec[r] = R;
     const unsigned cnt = R.y >> 16, sb = R.y & 0xFFFFu;
     MDPD_CHECK(p, sb + cnt <= p.tile_cap && R.x + cnt <= p.N && R.z < 27u && r < (unsigned)HTAB);
@@ -908,6 +916,25 @@ __global__ void __launch_bounds__(128) k_tile_recipe(const DevP p, int latch_fau
       }
     }
   }
+}
+
+// Record threadIdx.x of this tile's staging recipe (requested together with the header), and L2 prefetches of the recipe
+// of the tile that starts one CTA lifetime later (CTAs start in blockIdx order; `ahead` = resident CTAs of the grid).
+__device__ __forceinline__ uint4 first_record(const DevP& p, const unsigned ahead) {
+  const uint4* __restrict__ rec = p.runs + (size_t)blockIdx.x * p.run_stride + 1;
+  const uint4 R0 = threadIdx.x < p.nrun_max ? rec[threadIdx.x] : make_uint4(0u, 0u, 0u, 0u);
+  const unsigned nb = blockIdx.x + ahead;
+  if (nb < gridDim.x && threadIdx.x * 8u < p.run_stride) prefetch_l2(p.runs + (size_t)nb * p.run_stride + threadIdx.x * 8u);
+  return R0;
+}
+// ... and of its hand-out records and first list chunks (`hdrn` = that tile's header, requested at the start of the CTA,
+// used when the own tile has been staged: nobody waits for it)
+__device__ __forceinline__ void prefetch_handout(const DevP& p, const unsigned ahead, const uint4 hdrn, const uint2* __restrict__ info,
+                                                 const uint4* __restrict__ lst) {
+  if (blockIdx.x + ahead >= gridDim.x) return;
+  const unsigned osn = hdrn.w, nownn = hdrn.z >> 16;
+  if (threadIdx.x * 16u < nownn) prefetch_l2(info + osn + threadIdx.x * 16u);  // 128-byte lines: 16 records, 8 chunks
+  for (unsigned t = threadIdx.x * 8u; t < nownn; t += blockDim.x * 8u) prefetch_l2(lst + osn + t);
 }
 
 // group of 32 sorted own particles that warp `warp` of W takes in its round r (see the hand-out below)
@@ -1143,8 +1170,7 @@ __device__ __forceinline__ void direct_entry(const DevP& p, const unsigned ibase
   const float4 xj = lds4(ibase + (j << 4));  // padding entries hit the far-away sentinel
   const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
   const float r2 = dx * dx + dy * dy + dz * dz;
-  const float rr = r2 + 1e-30f;  // r = 0 (coincident particles, R10) must not produce 0 * inf
-  const float w = __saturatef(fmaf(-(rr * rsqrt_fast(rr)), p.inv_rd, 1.0f));
+  const float w = __saturatef(fmaf(-sqrt_fast(r2), p.inv_rd, 1.0f));  // 1 at r = 0 (coincident particles, R10)
   rho = fmaf(w, w, rho);
   bool in = f2u(r2 - 1e-12f) < f2u(p.rc2 - 1e-12f);  // 1e-12 < r2 < rc2, exact (see density_entry)
   if (HAS_WALL && ALL) in = in && !(walli & f2u(xj.w) & 1u);  // frozen-frozen pairs do not interact (R8)
@@ -1456,8 +1482,7 @@ __device__ __forceinline__ void density_entry(const DevP& p, const unsigned pbas
   const float r2 = dx * dx + dy * dy + dz * dz;
   // The logic pipe (min/max, compares, shifts, selects) issues at half the rate of the FP32 pipe and bounds this loop:
   // the clamps are saturate modifiers of the FMAs, the two-sided range test is one add and one unsigned compare.
-  const float rr = r2 + 1e-30f;  // r = 0 (coincident particles, R10) must not produce 0 * inf
-  const float w = __saturatef(fmaf(-(rr * rsqrt_fast(rr)), p.inv_rd, 1.0f));  // 0 beyond rd; never above 1
+  const float w = __saturatef(fmaf(-sqrt_fast(r2), p.inv_rd, 1.0f));  // 0 beyond rd; 1 at r = 0 (coincident particles, R10)
   rho = fmaf(w, w, rho);
   // 1e-12 < r2 < rc2 (R10): r2 - 1e-12 is negative below the lower bound (huge as an unsigned), and equals r2 wherever
   // the upper bound could matter (1e-12 is far below half an ulp of rc2)
@@ -1488,6 +1513,9 @@ __global__ void __launch_bounds__(TPB, DENS_MINB) k_density(const DevP p) {
   const unsigned cur = p.ctl->cur;
   const TileInfo T = p.tiles[blockIdx.x];
   const uint4 hdr = p.runs[(size_t)blockIdx.x * p.run_stride];
+  const unsigned ahead = p.sms * DENS_MINB;
+  const uint4 R0 = first_record(p, ahead);
+  const uint4 hdrn = p.runs[(size_t)min(blockIdx.x + ahead, gridDim.x - 1u) * p.run_stride];
   const unsigned os = hdr.w, nown = hdr.z >> 16;
   const unsigned warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
   const unsigned ngroups = (nown + 31u) >> 5;
@@ -1501,8 +1529,9 @@ __global__ void __launch_bounds__(TPB, DENS_MINB) k_density(const DevP p) {
   }
 #pragma unroll
   for (int r = 0; r < PRE; ++r) head[r] = info[r].y ? p.nbr[os + (info[r].x & 0xFFFFu)] : make_uint4(0, 0, 0, 0);
-  if (!((p.tma_staging & 1u) ? stage_bulk<false>(p, T, hdr, p.pos[cur], nullptr, sm) : stage_fast<false>(p, T, hdr, p.pos[cur], nullptr, sm)))
+  if (!((p.tma_staging & 1u) ? stage_bulk<false>(p, T, hdr, R0, p.pos[cur], nullptr, sm) : stage_fast<false>(p, T, hdr, R0, p.pos[cur], nullptr, sm)))
     return;  // flagged by k_tile_recipe
+  prefetch_handout(p, ahead, hdrn, p.dinfo, p.nbr);
   float4* __restrict__ vel = p.vel[cur];
   const unsigned sent = p.tile_cap;
   const unsigned pbase = smem_addr(sm.spos);
@@ -1680,6 +1709,9 @@ __global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
   const unsigned cur = p.ctl->cur;
   const TileInfo T = p.tiles[blockIdx.x];
   const uint4 hdr = p.runs[(size_t)blockIdx.x * p.run_stride];
+  const unsigned ahead = p.sms * MINB;
+  const uint4 R0 = first_record(p, ahead);
+  const uint4 hdrn = p.runs[(size_t)min(blockIdx.x + ahead, gridDim.x - 1u) * p.run_stride];
   const unsigned os = hdr.w, nown = hdr.z >> 16;
   const unsigned warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
   const unsigned ngroups = (nown + 31u) >> 5;
@@ -1696,8 +1728,9 @@ __global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
 #pragma unroll
   for (int r = 0; r < PRE; ++r)
     head[r] = (info[r].y & 0x7FFFFFFFu) ? p.act[os + (info[r].x & 0xFFFFu)] : make_uint4(sentw, sentw, sentw, sentw);
-  if (!((p.tma_staging & 2u) ? stage_bulk<true>(p, T, hdr, p.pos[cur], p.vel[cur], sm) : stage_fast<true>(p, T, hdr, p.pos[cur], p.vel[cur], sm)))
+  if (!((p.tma_staging & 2u) ? stage_bulk<true>(p, T, hdr, R0, p.pos[cur], p.vel[cur], sm) : stage_fast<true>(p, T, hdr, R0, p.pos[cur], p.vel[cur], sm)))
     return;
+  prefetch_handout(p, ahead, hdrn, p.finfo, p.act);
   HashKeys K = make_keys(p.ctl->step, p.seed);
 #pragma unroll
   for (int q = 0; q < 6; ++q) K.k[q] = pin(K.k[q]);
@@ -2478,6 +2511,11 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
     CU_TRY(h, cudaMemcpyAsync(svel, vel, n * 12, cudaMemcpyDefault, h->stream));
     if (type) CU_TRY(h, cudaMemcpyAsync(stype, type, n, cudaMemcpyDefault, h->stream));
     LAUNCH(h, PS_OTHER, (k_pack<<<nblk(n, TPB), TPB, 0, h->stream>>>(h->d, spos, svel, type ? stype : nullptr, 0u)));
+  }
+  {
+    int v = 0;
+    CU_TRY(h, cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, h->device));
+    h->d.sms = (unsigned)v;
   }
   h->direct = (h->prm.flags & MDPD_FLAG_DIRECT) != 0;
   // chosen by measurement (profiles/r2_staging.md): bulk copies win in the density pass, per-particle cp.async in the force pass
