@@ -2525,7 +2525,10 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
   // shared memory (checked on the device after the sort).
   static const int kCand[][3] = {{4, 4, 4}, {4, 4, 2}, {4, 2, 2}, {2, 2, 2}, {2, 2, 1}, {2, 1, 1}, {1, 1, 1}};
   const int ncand = (int)(sizeof kCand / sizeof kCand[0]);
-  int first = 0;
+#ifndef MDPD_FIRST_TILE
+#define MDPD_FIRST_TILE 0  // measurement builds: start the search at a smaller tile shape (profiles/r2_experiments.md)
+#endif
+  int first = MDPD_FIRST_TILE;
   {
     auto ntiles_of = [&](const int* t) {
       return (size_t)((L.ncx + t[0] - 1) / t[0]) * ((L.ncy + t[1] - 1) / t[1]) * ((L.ncz + t[2] - 1) / t[2]);
