@@ -381,6 +381,7 @@ def main_ours(args, rank, world, local):
                 if k in per_kernel:
                     per_kernel[k]["dram_bytes_per_launch_ncu"] = v.get("dram_bytes_per_launch")
                     per_kernel[k]["smem_pipe_frac_ncu"] = v.get("smem_pipe_frac")
+                    per_kernel[k]["l1_data_pipe_frac_ncu"] = v.get("l1_data_pipe_frac")  # all LSU wavefronts: shared + global + local
             if dom in kc and not args.direct:
                 roof["traffic"] = kc[dom].get("dram_bytes_per_launch")
             roof["traffic_source"] = f"profiles/ncu_r2_{args.workload}.json (ncu --set full, commit {cap.get('commit')})"

@@ -35,6 +35,14 @@ METRICS = {
     "smem_wavefronts": "l1tex__data_pipe_lsu_wavefronts_mem_shared.sum",
     "smem_conflict_wavefronts": "l1tex__data_bank_conflicts_pipe_lsu_mem_shared.sum",
     "smem_pipe_pct": "l1tex__data_pipe_lsu_wavefronts_mem_shared.sum.pct_of_peak_sustained_elapsed",
+    "l1_pipe_pct": "l1tex__data_pipe_lsu_wavefronts.sum.pct_of_peak_sustained_elapsed",
+    "stall_long_scoreboard": "smsp__average_warps_issue_stalled_long_scoreboard_per_issue_active.ratio",
+    "stall_short_scoreboard": "smsp__average_warps_issue_stalled_short_scoreboard_per_issue_active.ratio",
+    "stall_barrier": "smsp__average_warps_issue_stalled_barrier_per_issue_active.ratio",
+    "stall_wait": "smsp__average_warps_issue_stalled_wait_per_issue_active.ratio",
+    "stall_not_selected": "smsp__average_warps_issue_stalled_not_selected_per_issue_active.ratio",
+    "stall_math_pipe": "smsp__average_warps_issue_stalled_math_pipe_throttle_per_issue_active.ratio",
+    "stall_mio": "smsp__average_warps_issue_stalled_mio_throttle_per_issue_active.ratio",
     "pipe_alu_pct": "sm__inst_executed_pipe_alu.avg.pct_of_peak_sustained_active",
     "pipe_fma_pct": "sm__inst_executed_pipe_fma.avg.pct_of_peak_sustained_active",
     "pipe_xu_pct": "sm__inst_executed_pipe_xu.avg.pct_of_peak_sustained_active",
@@ -84,7 +92,10 @@ def summarise(path: str):
         ent = {"launches_averaged": len(real), "launches_captured": len(launches), "gpu_time_ms": round(avg.get("ms", 0.0), 5),
                "dram_bytes_per_launch": round(avg.get("dram_read", 0.0) + avg.get("dram_write", 0.0)),
                "dram_read_bytes": round(avg.get("dram_read", 0.0)), "dram_write_bytes": round(avg.get("dram_write", 0.0)),
-               "smem_pipe_frac": round(avg.get("smem_pipe_pct", 0.0) / 100.0, 4)}
+               "smem_pipe_frac": round(avg.get("smem_pipe_pct", 0.0) / 100.0, 4),
+               "l1_data_pipe_frac": round(avg.get("l1_pipe_pct", 0.0) / 100.0, 4),
+               # warps of a scheduler waiting for each reason, per cycle in which the scheduler issued
+               "stalls_per_issue": {k[6:]: round(avg[k], 3) for k in METRICS if k.startswith("stall_") and k in avg}}
         for k in ("warp_inst", "issue_active_pct", "warps_per_sm", "threads_per_inst", "smem_wavefronts",
                   "smem_conflict_wavefronts", "pipe_alu_pct", "pipe_fma_pct", "pipe_xu_pct", "pipe_lsu_pct", "registers",
                   "block", "grid", "l2_hit_pct"):
@@ -111,19 +122,21 @@ def main():
     dst = os.path.join(ROOT, "profiles", f"ncu_r2_{a.workload}.json")
     json.dump(doc, open(dst, "w"), indent=1)
     n = a.particles
-    print(f"| kernel | launches | ms | DRAM MB (r + w) | {'B/particle | ' if n else ''}warp inst{'/particle' if n else ''} | issue % | smem pipe % | "
-          "conflict / all wavefronts | alu / fma / xu / lsu pipe % | warps/SM | regs x block |")
-    print("|---|---:|---:|---:|" + ("---:|" if n else "") + "---:|---:|---:|---:|---:|---:|---:|")
+    print(f"| kernel | launches | ms | DRAM MB (r + w) | {'B/particle | ' if n else ''}warp inst{'/particle' if n else ''} | issue % | L1 data pipe % (shared part) | "
+          "conflict / all wavefronts | alu / fma / xu / lsu pipe % | warps/SM | regs x block | stalled warps per issue: long sb / short sb / barrier / wait |")
+    print("|---|---:|---:|---:|" + ("---:|" if n else "") + "---:|---:|---:|---:|---:|---:|---:|---:|")
     for k, e in sorted(kernels.items(), key=lambda kv: -kv[1]["gpu_time_ms"]):
         wi = e.get("warp_inst", 0.0)
         cells = [k, f"{e['launches_averaged']} of {e['launches_captured']}", f"{e['gpu_time_ms']:.4f}",
                  f"{e['dram_read_bytes'] / 1e6:.1f} + {e['dram_write_bytes'] / 1e6:.1f}"]
         if n:
             cells.append(f"{e['dram_bytes_per_launch'] / n:.1f}")
-        cells += [f"{wi / n:.1f}" if n else f"{wi:.3g}", f"{e.get('issue_active_pct', 0):.1f}", f"{100 * e['smem_pipe_frac']:.1f}",
+        cells += [f"{wi / n:.1f}" if n else f"{wi:.3g}", f"{e.get('issue_active_pct', 0):.1f}",
+                  f"{100 * e['l1_data_pipe_frac']:.1f} ({100 * e['smem_pipe_frac']:.1f})",
                   f"{e.get('smem_conflict_wavefronts', 0):.3g} / {e.get('smem_wavefronts', 0):.3g}",
                   f"{e.get('pipe_alu_pct', 0):.0f} / {e.get('pipe_fma_pct', 0):.0f} / {e.get('pipe_xu_pct', 0):.0f} / {e.get('pipe_lsu_pct', 0):.0f}",
-                  f"{e.get('warps_per_sm', 0):.1f}", f"{e.get('registers', 0):.0f} x {e.get('block', 0):.0f}"]
+                  f"{e.get('warps_per_sm', 0):.1f}", f"{e.get('registers', 0):.0f} x {e.get('block', 0):.0f}",
+                  " / ".join(f"{e['stalls_per_issue'].get(q, 0):.2f}" for q in ("long_scoreboard", "short_scoreboard", "barrier", "wait"))]
         print("| " + " | ".join(cells) + " |")
     print(f"\nwritten: {dst}")
 
