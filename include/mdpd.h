@@ -54,7 +54,7 @@ typedef struct {
   float skin;             /* Verlet-list skin (default 0.25); list radius = rc + skin; rebuild when the largest
                              displacement since the last build exceeds skin/2                   DESIGN.md R3, R4      */
   float headroom;         /* capacity of a tile of cells (shared memory) = headroom x the fullest tile of the loaded
-                             state; 0 = default 1.15.  Raise it when the density will grow locally during the run (a
+                             state; 0 = default: 1.15, lowered to no less than 1.08 where that keeps two CTAs of the force pass per SM.  Raise it when the density will grow locally during the run (a
                              contracting slab, a filling pore): outgrowing the capacity is MDPD_EOVERFLOW              */
   uint32_t seed;          /* seed of the pair hash      */
   uint32_t max_neigh;     /* list capacity per particle, <= 128; 0 = automatic                                       */

@@ -2148,11 +2148,14 @@ void build_tile_ranks(const Layout& L, const int tdim[3], std::vector<unsigned>&
   for (unsigned long long code = 0; code < ncodes; ++code) {
     const unsigned tx = compact(code), ty = compact(code >> 1), tz = compact(code >> 2);
     if (tx >= ntx || ty >= nty || tz >= ntz) continue;
+    // tile t of nt along a dimension of nc cells starts at floor(t nc / nt): extents differ by at most one cell, no thin
+    // remainder tile at the upper faces (137 cells: 32 tiles of 4 and 3 of 3 instead of 34 of 4 and one of 1)
+    auto start = [](unsigned t, unsigned nt, unsigned nc) { return (int)((unsigned long long)t * nc / nt); };
     TileInfo T;
-    T.c0x = (int)(tx * tdim[0]); T.c0y = (int)(ty * tdim[1]); T.c0z = (int)(tz * tdim[2]);
-    T.ex = std::min<int>(tdim[0], (int)L.ncx - T.c0x);
-    T.ey = std::min<int>(tdim[1], (int)L.ncy - T.c0y);
-    T.ez = std::min<int>(tdim[2], (int)L.ncz - T.c0z);
+    T.c0x = start(tx, ntx, L.ncx); T.c0y = start(ty, nty, L.ncy); T.c0z = start(tz, ntz, L.ncz);
+    T.ex = start(tx + 1, ntx, L.ncx) - T.c0x;
+    T.ey = start(ty + 1, nty, L.ncy) - T.c0y;
+    T.ez = start(tz + 1, ntz, L.ncz) - T.c0z;
     T.rank0 = next;
     T.ncell_own = (unsigned)(T.ex * T.ey * T.ez);
     for (int lz = 0; lz < T.ez; ++lz)
@@ -2586,12 +2589,28 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
     {
       // at least `headroom` (default 15 %) over the fullest tile of the initial state; beyond that, all the shared memory that does not
       // cost a resident CTA of the force pass (the tightest: it stages positions and velocities)
-      const unsigned want = std::min<unsigned>(cap_limit, ((unsigned)(max_halo * headroom) + 64 + 63) / 64 * 64);
+      unsigned want = std::min<unsigned>(cap_limit, ((unsigned)(max_halo * headroom) + 64 + 63) / 64 * 64);
       const size_t sm_total = h->smem_limit + 1024;  // per-SM shared memory; 1 KB is reserved per resident CTA
+      if (!(h->prm.headroom > 0.0f)) {
+        // default head-room: 15 %, but no less than 8 % where the difference decides whether two CTAs of the force pass fit per SM
+        // (3.4 against 2.5 ms per launch on config 4a just above the limit; profiles/r2_experiments.md section 5)
+        const size_t half = sm_total / 2;
+        const unsigned two = half > 1024 + fixed ? (unsigned)((half - 1024 - fixed) / TILE_SLOT_BYTES / 64 * 64) : 0u;
+        if (want > two && (double)max_halo * 1.08 + 64.0 <= (double)two) want = two;
+      }
       const size_t per_cta = tile_smem_bytes(want, true, 0) + 1024;
       const size_t ctas = std::max<size_t>(1, sm_total / per_cta);
       const size_t room = sm_total / ctas - 1024 - fixed;
-      h->d.tile_cap = std::max<unsigned>(want, std::min<unsigned>(cap_limit, (unsigned)(room / TILE_SLOT_BYTES / 64 * 64)));
+      // ... nor one of the density pass (positions only, DENS_MINB CTAs per SM) or of the list build (two): when the force pass is
+      // down to one CTA per SM the capacity must not grow into the other passes' occupancy
+      const auto slots_for = [&](size_t n_ctas, size_t slot_bytes, size_t extra) {
+        const size_t per = sm_total / n_ctas;
+        const size_t fix = 1024 + tile_smem_bytes(0, false, 0) + extra;
+        return per > fix ? (per - fix) / slot_bytes : 0;
+      };
+      const size_t grow = std::min(std::min<size_t>(room / TILE_SLOT_BYTES, slots_for(DENS_MINB, 16, 0)),
+                                   slots_for(2, 16, HTAB * 2 + (size_t)CELLS_MAXW0 * CELLS_ROW0_BYTES));
+      h->d.tile_cap = std::max<unsigned>(want, std::min<unsigned>(cap_limit, (unsigned)(grow / 64 * 64)));
     }
     break;
   }
