@@ -59,6 +59,9 @@ typedef struct mdpd_ref_ctx {
   double *x, *v, *f, *fpair, *rho; /* [n][3], [n] ; index == tag == load order */
   uint8_t *type;    /* 1: frozen (never integrated), 0: mobile */
   uint8_t *species; /* material type of the particle: row / column of the pair-parameter matrices below */
+  uint32_t *tag;    /* NULL: tag == index (load order, R5).  mdpd_ref_set_tags: the particles are a SUBSET of a larger
+                     * system and keep the tags they have there, so that the hashed random force of a pair is the one the
+                     * whole system evaluates (the hash is a function of the two tags, the step and the seed). */
   /* Per-type-pair conservative parameters ("A_SL, B_SL"; Tables 1-2): ntypes == 0 means
    * one material, A and B of mdpd_ref_params for every pair, type byte != 0 <=> frozen.  Otherwise the type byte of a
    * particle is its species s in [0, ntypes), the pair (i, j) uses Am[s_i][s_j], Bm[s_i][s_j] (symmetric), and species s
@@ -124,9 +127,9 @@ int mdpd_ref_create(mdpd_ref_ctx **out) {
 }
 
 static void free_particles(mdpd_ref_ctx *h) {
-  free(h->x); free(h->v); free(h->f); free(h->fpair); free(h->rho); free(h->type); free(h->species); free(h->next);
+  free(h->x); free(h->v); free(h->f); free(h->fpair); free(h->rho); free(h->type); free(h->species); free(h->next); free(h->tag);
   h->x = h->v = h->f = h->fpair = h->rho = NULL;
-  h->type = NULL; h->species = NULL; h->next = NULL; h->n = 0;
+  h->type = NULL; h->species = NULL; h->next = NULL; h->tag = NULL; h->n = 0;
 }
 
 int mdpd_ref_destroy(mdpd_ref_ctx *h) {
@@ -289,7 +292,12 @@ static void force_pair(mdpd_ref_ctx *h, uint64_t i, uint64_t j, const double d[3
   double wR = (p->s == 1.0) ? w : pow(w, p->s);
   double ev = 0.0;
   for (int k = 0; k < 3; ++k) ev += e[k] * (h->v[3 * i + k] - h->v[3 * j + k]);
-  uint32_t hh = mdpd_ref_hash((uint32_t)i, (uint32_t)j, (uint32_t)h->step, p->seed); /* i < j here */
+  uint32_t ta = (uint32_t)i, tb = (uint32_t)j; /* i < j here */
+  if (h->tag) { /* caller-supplied tags: a = min tag, b = max tag */
+    ta = h->tag[i] < h->tag[j] ? h->tag[i] : h->tag[j];
+    tb = h->tag[i] < h->tag[j] ? h->tag[j] : h->tag[i];
+  }
+  uint32_t hh = mdpd_ref_hash(ta, tb, (uint32_t)h->step, p->seed);
   double xi = mdpd_ref_xi(hh);
   double Aij = p->A, Bij = p->B;
   if (h->ntypes) { /* per-type-pair parameters */
@@ -398,6 +406,21 @@ int mdpd_ref_load_wall_mask(mdpd_ref_ctx *h, const uint8_t *mask, const uint32_t
   for (uint64_t i = 0; i < h->n; ++i)
     if (!h->type[i] && in_solid(h, &h->x[3 * i])) bad++;
   return bad ? REF_EINSOLID : REF_OK;
+}
+
+/* Tags of a subset of a larger system (see mdpd_ref_ctx.tag): [n] distinct uint32, or NULL to return to tag == index.
+ * Forces are re-evaluated.  Pair lists (mdpd_ref_get_pairs) keep reporting indices. */
+int mdpd_ref_set_tags(mdpd_ref_ctx *h, const uint32_t *tags) {
+  if (!h || !h->x) return REF_ESTATE;
+  free(h->tag);
+  h->tag = NULL;
+  if (tags) {
+    uint64_t m = h->n ? h->n : 1;
+    h->tag = (uint32_t *)malloc(m * sizeof(uint32_t));
+    if (!h->tag) return REF_ENOMEM;
+    memcpy(h->tag, tags, h->n * sizeof(uint32_t));
+  }
+  return mdpd_ref_compute_forces(h);
 }
 
 int mdpd_ref_set_step(mdpd_ref_ctx *h, uint64_t step) {

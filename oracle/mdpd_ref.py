@@ -56,6 +56,7 @@ def lib():
         L.mdpd_ref_load_particles.argtypes = [vp, u64, vp, vp, vp]
         L.mdpd_ref_load_wall_mask.argtypes = [vp, vp, vp, C.c_double]
         L.mdpd_ref_set_step.argtypes = [vp, u64]
+        L.mdpd_ref_set_tags.argtypes = [vp, vp]
         L.mdpd_ref_set_velocities.argtypes = [vp, vp]
         L.mdpd_ref_step.argtypes = [vp, u32]
         L.mdpd_ref_get_state.argtypes = [vp, vp, vp, vp, vp, vp]
@@ -150,6 +151,16 @@ class RefSim:
 
     def set_step(self, k):
         _check(self._L.mdpd_ref_set_step(self._h, int(k)), "set_step")
+
+    def set_tags(self, tags):
+        """The loaded particles are a subset of a larger system: they keep the tags they have there (hash input, DESIGN.md
+        section 4).  None returns to tag == load index.  Forces are re-evaluated."""
+        if tags is None:
+            _check(self._L.mdpd_ref_set_tags(self._h, None), "set_tags")
+            return
+        t = np.ascontiguousarray(tags, np.uint32)
+        assert t.shape == (self.n,)
+        _check(self._L.mdpd_ref_set_tags(self._h, t.ctypes.data), "set_tags")
 
     def set_velocities(self, vel):
         vel = np.ascontiguousarray(vel, np.float64).reshape(-1, 3)

@@ -59,10 +59,10 @@ def test_config4b_one_million_particles_every_particle(gpu):
 def test_config4a_32_million_particles_sampled(gpu):
     """Config 4a (175^3 box, 32 156 250 particles), the workload bench.py times: 4 timesteps, then a SAMPLE the oracle
     can afford: all particles of a 16^3 sub-cube are handed to the oracle in a 24^3 box (no periodic images interact),
-    and the ~13 000 particles at least rc + rd = 1.75 inside the sub-cube (their neighbours, and the neighbours that
-    set their neighbours' rho, are all present) are compared.  The oracle numbers particles in load order, so the
-    hashed random force cannot be matched on a subset: both sides evaluate with sigma = 0 (conservative + many-body +
-    dissipative terms); the random term is covered bit-exactly by the RNG-stream test and by configs 0-4b.
+    WITH THE TAGS THEY HAVE IN THE WHOLE SYSTEM (mdpd_ref_set_tags; pinned in tests/test_oracle_pins.py), so that the
+    hashed random force at 32 M-particle tags is part of the comparison, and the ~13 000 particles at least rc + rd = 1.75
+    inside the sub-cube (their neighbours, and the neighbours that set their neighbours' rho, are all present) are
+    compared: rho and the full force (conservative + many-body + dissipative + random) within 1e-4 of the RMS.
     Sub-cubes: one in the bulk, one across three periodic faces of the big box."""
     from oracle.mdpd_ref import RefSim
     c = wl.make_config("4a")
@@ -73,11 +73,10 @@ def test_config4a_32_million_particles_sampled(gpu):
     s.step(4)
     ctr = s.counters()
     assert ctr["faults"] == 0 and ctr["steps"] == 4
-    s.set_params(sigma=0.0, kT=0.0)
     s.compute_forces()
     g = s.get_state()
     assert np.isfinite(g["force"]).all() and np.isfinite(g["rho"]).all()
-    p = dict(c["params"], sigma=0.0, kT=0.0, box=(24.0, 24.0, 24.0))
+    p = dict(c["params"], box=(24.0, 24.0, 24.0))
     L = 175.0
     for origin in ((80.0, 40.0, 120.0), (167.0, 167.0, 167.0)):
         o = np.asarray(origin, np.float64)
@@ -88,6 +87,8 @@ def test_config4a_32_million_particles_sampled(gpu):
         sub = rel + 4.0                                  # centred in the 24^3 box: > rc from every image
         r = RefSim(p)
         r.load_particles(sub, g["vel"][idx].astype(np.float64), None)
+        r.set_step(g["step"])
+        r.set_tags(idx.astype(np.uint32))                # re-evaluates the forces with the whole system's tags
         rs = r.get_state()
         core = ((rel >= 1.75) & (rel < 16.0 - 1.75)).all(1)
         assert core.sum() > 8000

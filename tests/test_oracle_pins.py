@@ -429,3 +429,44 @@ def test_bounce_back_mask_axis_order():
     assert nb == 0
     x, v, nb = run(my, [0.0, 0.0, 2.0], 150)
     assert nb == 0
+
+
+def test_subset_with_tags_evaluates_the_whole_systems_random_force():
+    """DESIGN.md section 4 / R5: the hashed random force of a pair is a function of the two TAGS, the step and the seed.
+    mdpd_ref_set_tags lets a SUBSET of a larger system keep the tags it has there (used by the 32 M-particle parity
+    test, where the oracle can only afford a sub-cube).  Pins: (a) one pair with tags (70001, 12) against the
+    independent Python restatement of the hash, both orders; (b) a sub-cube of a periodic liquid, loaded alone with its
+    original tags, reproduces the whole system's forces on every particle whose neighbours (and their neighbours inside
+    rd) are all present -- and does NOT without the tags."""
+    p = dict(P0, A=0.0, B=0.0, gamma=0.0, seed=77)
+    for tags in ((70001, 12), (12, 70001)):
+        s, d = two_particles(0.5, p)
+        s.set_step(5)
+        s.set_tags(np.array(tags, np.uint32))
+        f0 = s.get_state()["force"][0]
+        xi = xi_py(hash_py(12, 70001, 5, 77))
+        assert np.allclose(f0, 15.0 * xi * (-d), atol=1e-12)
+        s.set_tags(None)                                   # back to tag == index
+        assert np.allclose(s.get_state()["force"][0], 15.0 * xi_py(hash_py(0, 1, 5, 77)) * (-d), atol=1e-12)
+    c = wl.make_liquid(9.0, seed=4242)
+    whole = RefSim(c["params"])
+    whole.load_particles(c["pos"].astype(np.float64), c["vel"].astype(np.float64), c["type"])
+    whole.set_step(3)
+    whole.compute_forces()
+    W = whole.get_state()
+    pos = c["pos"].astype(np.float64)
+    inside = ((pos >= 1.0) & (pos < 8.0)).all(1)           # a 7^3 sub-cube, away from the periodic faces
+    idx = np.nonzero(inside)[0]
+    core = ((pos[idx] >= 1.0 + 1.75) & (pos[idx] < 8.0 - 1.75)).all(1)   # rc + rd inside: neighbours and their rho complete
+    assert core.sum() > 100
+    sub = RefSim(dict(c["params"], box=(12.0, 12.0, 12.0)))   # no periodic image of the sub-cube is within reach
+    sub.load_particles(pos[idx] + 1.0, c["vel"][idx].astype(np.float64), None)
+    sub.set_step(3)
+    sub.compute_forces()
+    S0 = sub.get_state()                                    # tags = load index of the subset: another random force
+    sub.set_tags(idx.astype(np.uint32))
+    S1 = sub.get_state()
+    frms = np.sqrt((W["force"] ** 2).sum(1).mean())
+    assert np.abs(S1["rho"][core] - W["rho"][idx][core]).max() < 1e-12
+    assert np.abs(S1["force"][core] - W["force"][idx][core]).max() < 1e-10 * frms
+    assert np.abs(S0["force"][core] - W["force"][idx][core]).max() > 0.05 * frms
