@@ -88,7 +88,7 @@ struct DevP {  // passed by value to every kernel
   uint4* act;                // [cap / 8][N] this step's in-range (r < rc) subset of the list, written by the density pass
   unsigned short* nact;      // [N] its length
   const TileInfo* tiles;     // [ntiles]
-  uint4* runs;               // [ntiles][run_stride] staging recipe of every tile, written by k_build_list (see stage_fast)
+  uint4* runs;               // [ntiles][run_stride] staging recipe of every tile, written by k_tile_recipe (see stage_fast)
   uint2* dinfo;              // [N] hand-out records of the density pass: own particles of every tile in order of decreasing
                              //     list length; x = index in the tile | own staged slot << 16, y = list length
   uint2* finfo;              // [N] ... of the force pass: in order of decreasing in-range count of this step (y = count,
@@ -672,7 +672,7 @@ __device__ __forceinline__ unsigned stage_tile(const DevP& p, const TileInfo& T,
 
 // ----------------------------------------------------------------------------------------------------------------
 // Staging recipe.  The per-step passes (density, force) do not rediscover the tile's geometry: at every list build
-// k_build_list writes, per tile, a header and one record per RUN of halo cells that is contiguous both in the staged
+// k_tile_recipe writes, per tile, a header and one record per RUN of halo cells that is contiguous both in the staged
 // image and in the sorted particle arrays (per (y, z) halo row: the cell at x = -1, the tile-aligned cells, the cell
 // at x = ex).  Header: x = staged particles (0xFFFFFFFF: tile does not fit), y = runs, z = items | own particles << 16,
 // w = first own particle.  Record: x = first global index, y = first staged slot | particles << 16, z = shift code
