@@ -132,3 +132,34 @@ def test_slit_pore_wetting_follows_A_SL(gpu):
         res[A_SL] = (near, spread)
     assert res[-35.0][0] > 1.15 * res[-20.0][0], res          # more liquid at the walls when they attract it more
     assert res[-35.0][1] > res[-20.0][1], res                 # and it spreads further along them
+
+
+def test_slit_pore_profiles_reproduce_figure_6(gpu):
+    """Section 4.2 of the paper, its protocol and its printed reading of Figure 6: 4 000 steps to
+    equilibrate, then 10 000 steps over which the number of liquid particles is averaged in EIGHT bins across the pore
+    width; "by dismissing the two near-wall points in those profiles, the curvatures of the profiles can be used to
+    quantify the contact angles": A_SL = -35 gives a partially wetting liquid (contact angle < 90 degrees: liquid
+    creeps along the walls, the profile curves upward), A_SL = -20 a partially non-wetting one (> 90 degrees: curves
+    downward), and "in the case of A_SL = -30, the profile is almost a straight line".  Curvature = quadratic
+    coefficient of a fit through the six inner bins (particles per bin per rc^2)."""
+    curv = {}
+    for A_SL in (-35.0, -30.0, -20.0):
+        c = wl.make_slit_wetting(A_SL)
+        s = gpu.Simulation(c["params"])
+        s.set_pair_params(c["pair_A"], c["pair_B"], c["frozen_mask"])
+        s.load_particles(c["pos"], c["vel"], c["type"], mask_dims=c["mask"].shape[::-1])
+        s.load_wall_mask(c["mask"], c["voxel"])
+        s.step(4000)
+        prof = np.zeros(8)
+        for _ in range(500):
+            s.step(20)
+            y = s.get_state(vel=False, force=False, rho=False)["pos"][c["type"] == 0][:, 1]
+            prof += np.histogram(y, bins=8, range=(1.0, 9.0))[0]
+        prof /= 500.0
+        assert s.counters()["faults"] == 0 and abs(prof.sum() - 4000.0) < 1e-6   # every liquid particle stays in the pore
+        yc = np.arange(8) + 0.5 - 4.0
+        curv[A_SL] = float(np.polyfit(yc[1:7], prof[1:7], 2)[0])
+        s.close()
+    assert curv[-35.0] > 1.5 and curv[-20.0] < -2.5, curv                      # wetting -> non-wetting (measured: +3.2, -5.2)
+    assert abs(curv[-30.0]) < 0.25 * min(curv[-35.0], -curv[-20.0]), curv      # "almost a straight line" (measured: +0.13)
+    assert curv[-35.0] > curv[-30.0] > curv[-20.0], curv
