@@ -135,3 +135,44 @@ def test_poiseuille_flow_rate_and_profile(gpu):
     assert np.abs(pg - pr).max() < 4 * sig_b, (pg, pr)
     assert pg[0] < pg[nb // 2] and pg[-1] < pg[nb // 2]            # slower at the walls
     assert ctr["bounces"] > 0
+
+
+def _gpu_pressure(pk, dens, **pover):
+    """The paper's protocol for Figure 3: 10 x 10 x 10 periodic box, pressure averaged over 1000 steps
+    after equilibration.  p = N kT / V + (sum over pairs of r . F^C) / (3 V): kinetic part from the velocities, the
+    configurational part from mdpd_compute_virial (conservative force; the dissipative and random parts average out)."""
+    c = wl.make_liquid(10.0, density=dens, seed=31, **pover)
+    s = pk.Simulation(c["params"])
+    s.load_particles(c["pos"], c["vel"], c["type"])
+    n, V = len(c["pos"]), 1000.0
+    s.step(1000)
+    ps, kts = [], []
+    for _ in range(100):
+        s.step(10)
+        W = s.compute_virial()
+        kt = kinetic_temperature(s.get_state(pos=False, force=False, rho=False)["vel"])
+        kts.append(kt)
+        ps.append(n * kt / V + (W[0] + W[1] + W[2]) / (3.0 * V))
+    assert s.counters()["faults"] == 0
+    s.close()
+    return float(np.mean(ps)), float(np.mean(kts))
+
+
+def test_equation_of_state_of_figure_3(gpu):
+    """Figure 3 of the paper on the GPU, both panels, against the closed forms it prints:
+    (b) mDPD, A = -40, B = 25, rd = 0.75:  p = rho kT + alpha A rho^2 + 2 alpha B rd^4 (rho^3 - c rho^2 + d), alpha = 0.101,
+        c = 4.16, d = 18 (R13)  ->  22.5, 60.2, 109.2, 170.9 at rho = 6.5, 7, 7.5, 8; measured 24.0, 61.2, 108.4,
+        167.1 -- the same tolerance as the oracle's pin (tests/test_oracle_statistics.py): max(5 %, 2.0);
+    (a) the original DPD model, a_ij = 25 (here A = +25, B = 0):  p = rho kT + 0.1 a rho^2  ->  44, 67.5, 96 at rho = 4, 5, 6;
+        measured 42.3, 66.3, 95.5 (the quadratic form is the high-density limit: 5 %)."""
+    for dens, ref in ((6.5, 22.5), (7.0, 60.2), (7.5, 109.2), (8.0, 170.9)):
+        closed = dens + 0.101 * -40.0 * dens ** 2 + 2 * 0.101 * 25.0 * 0.75 ** 4 * (dens ** 3 - 4.16 * dens ** 2 + 18.0)
+        assert abs(closed - ref) < 0.06                           # the paper's formula, evaluated by hand
+        p, kt = _gpu_pressure(gpu, dens)
+        assert abs(kt - 1.0) < 0.02, (dens, kt)
+        assert abs(p - closed) < max(0.05 * closed, 2.0), (dens, p, closed)
+    for dens in (4.0, 5.0, 6.0):
+        closed = dens + 0.1 * 25.0 * dens ** 2
+        p, kt = _gpu_pressure(gpu, dens, A=25.0, B=0.0)
+        assert abs(kt - 1.0) < 0.02, (dens, kt)
+        assert abs(p - closed) < 0.05 * closed, (dens, p, closed)

@@ -42,6 +42,24 @@ def test_thermostat_and_equation_of_state(dens):
     assert abs(np.mean(ps) - p_ref) < max(0.05 * p_ref, 2.0), (np.mean(ps), p_ref)
 
 
+def test_original_dpd_equation_of_state():
+    """Figure 3(a) of the paper: the original DPD model, a_ij = 25 (A = +25, B = 0 in Eq. (1)), kT = 1, gamma = 4.5:
+    p = rho kT + 0.1 a rho^2 = 67.5 at rho = 5 (the quadratic form is the high-density limit of the measured EOS: 5 %)."""
+    L, dens = 6.0, 5.0
+    c = wl.make_liquid(L, density=dens, seed=6, A=25.0, B=0.0)
+    s = RefSim(c["params"])
+    s.load_particles(c["pos"], c["vel"])
+    s.step(400)
+    n, V = len(c["pos"]), L ** 3
+    ps = []
+    for _ in range(120):
+        s.step(5)
+        ps.append(n * kinetic_temperature(s.get_state()["vel"]) / V + s.counters()["virial_c"] / (3 * V))
+    p_ref = dens + 0.1 * 25.0 * dens ** 2
+    assert p_ref == 67.5
+    assert abs(np.mean(ps) - p_ref) < 0.05 * p_ref, np.mean(ps)
+
+
 def shear_wave_viscosity():
     """Kinematic viscosity of the periodic mDPD liquid, no walls, no body force: a transverse velocity wave
     v_x = A sin(k z) decays as exp(-nu k^2 t) (linearised Navier-Stokes).  8 x 8 x 12 box, k = 2 pi / 12, A = 1; the
