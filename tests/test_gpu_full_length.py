@@ -170,3 +170,27 @@ def test_config4b_1000_steps_temperature_density_momentum(gpu):
     p = st["vel"].astype(np.float64).sum(0) / n
     assert np.abs(p).max() < 1e-5, p
     assert 250 < ctrs["rebuilds"] < 600
+
+
+def test_config4a_1000_steps_temperature_density_momentum(gpu):
+    """Config 4a (32 156 250 particles, the workload bench.py times, at the bench's skin 0.27) for the 1 000 steps
+    BASELINE.json states: no fault, kT = 1 within 2 % over the second half, <rho> stationary, total momentum conserved,
+    one list rebuild per ~3 steps.  Four read-backs of the state (the velocities and rho of 3.2e7 particles each)."""
+    c = wl.make_config("4a")
+    c["params"] = dict(c["params"], skin=0.27)
+    sim = load(gpu, c)
+    n = len(c["pos"])
+    kts, rhos = [], []
+    for k in range(4):
+        sim.step(250)
+        st = sim.get_state(pos=False, force=False)
+        kts.append(kinetic_temperature(st["vel"]))
+        rhos.append(st["rho"].astype(np.float64).mean())
+    ctrs = sim.counters()
+    sim.close()
+    assert ctrs["faults"] == 0 and ctrs["steps"] == 1000
+    assert abs(np.mean(kts[2:]) - 1.0) < 0.02, kts
+    assert abs(rhos[2] / rhos[3] - 1.0) < 0.005, rhos
+    p = st["vel"].astype(np.float64).sum(0) / n
+    assert np.abs(p).max() < 1e-5, p
+    assert 300 < ctrs["rebuilds"] < 420, ctrs["rebuilds"]
