@@ -280,12 +280,23 @@ def main_ours(args, rank, world, local):
     ts = c1["tile_shape"]
     tile_shape = [ts & 255, (ts >> 8) & 255, (ts >> 16) & 255]
 
+    # ---- spread: three more windows of K steps, same protocol (several windows, mean and spread) --------
+    repeats = []
+    for _ in range(0 if args.no_repeats else 3):
+        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        r0.record()
+        sim.step(K)
+        r1.record()
+        torch.cuda.synchronize()
+        repeats.append(round(r0.elapsed_time(r1) / K, 4))
+    cp = sim.counters()
+
     # ---- per-kernel CUDA-event times over another K steps (same stream) --------------------------------------
     sim.profile_begin()
     sim.step(K)
     prof = sim.profile_end()
     c2 = sim.counters()
-    reb_prof = c2["rebuilds"] - c1["rebuilds"]
+    reb_prof = c2["rebuilds"] - cp["rebuilds"]
     tot = sum(v[0] for v in prof.values())
     hot = [k for k in prof if k != "other"]
     dom = max(hot, key=lambda k: prof[k][0])
@@ -428,7 +439,8 @@ def main_ours(args, rank, world, local):
                        "tile_cells": tile_shape, "tiles": c1["ntiles"]},
             "e2e": {"value": e2e_v, "unit": UNIT, "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
                     "note": f"one job = load_particles(host, equilibrated state) + {K} steps + get_state(host); bytes are per job / {K}"},
-            "gpu_launches": launches, "clocks": clocks, "roofline": roof, "kernels": kernels}
+            "gpu_launches": launches, "clocks": clocks, "roofline": roof, "kernels": kernels,
+            "repeat_windows_ms_per_step": repeats}   # this rank's next three windows of K steps (untimed for `value`)
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         edge = oracle_sample_edge(20.0 * 4.0e5 / 20)          # ~20 s: 20 steps of a ~4e5-particle box
@@ -451,6 +463,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="4a", choices=["4a", "4b", "0", "1", "2", "3"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-repeats", action="store_true", help="skip the three extra windows that report the spread")
     ap.add_argument("--equilibrate", type=int, default=EQUILIBRATE, help="untimed steps after loading")
     ap.add_argument("--direct", action="store_true", help="list-free path (MDPD_FLAG_DIRECT): no Verlet list")
     ap.add_argument("--tma", action="store_true", help="both tile passes stage with cp.async.bulk (MDPD_FLAG_TMA_STAGING)")
