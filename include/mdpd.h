@@ -171,7 +171,8 @@ int mdpd_rng_fill(mdpd_ctx* h, uint64_t npairs, const uint32_t* pairs, uint32_t 
  * tile (tile + halo) at the last build, [6] device fault events (list / tile overflows + non-finite coordinates; also
  * latched as an error code), [7] kernels launched by this handle so far, [8] sum over all density passes so far of
  * the in-range (r < rc) neighbour counts = pair evaluations of the force passes, [9] number of density passes so far,
- * [10] tile shape tx | ty << 8 | tz << 16 (cells), [11] number of tiles; [12..15] see below (0 in a normal build).
+ * [10] tile shape tx | ty << 8 | tz << 16 (cells: the largest extent; tiles along a dimension differ by at most one cell),
+ * [11] number of tiles; [12..15] reserved (0).
  * Synchronises the stream. */
 int mdpd_get_counters(mdpd_ctx* h, uint64_t out[MDPD_NCOUNTERS]);
 
@@ -195,8 +196,6 @@ const char* mdpd_profile_name(int slot);
  * reports as maximum.  No handle needed.  Returns MDPD_OK or MDPD_ECUDA. */
 int mdpd_probe_issue_rates(int device, void* cuda_stream, double out[4]);
 
-/* [12..15] of mdpd_get_counters: clock cycles of k_force's staging and pair loop summed over CTAs, and the CTA count,
- * when the library was built with -DMDPD_PHASES (a tuning aid); 0 otherwise. */
 
 #ifdef __cplusplus
 }
