@@ -160,6 +160,35 @@ int mdpd_compute_virial(mdpd_ctx* h, double out[6]);
  * builds a list from the current cells. */
 int mdpd_get_pairs(mdpd_ctx* h, float rcut, uint64_t* count, uint32_t* pairs, uint64_t cap);
 
+/* mdpd_get_pairs without any device allocation, for callers that cannot make one.
+ *
+ * Who that is: a host program that has already handed all free device memory to its own pool (a tensor framework's
+ * caching allocator, a job that reserves the whole card at start-up) -- there a cudaMalloc from inside this library
+ * simply fails with out-of-memory although the pool has room; and code on a latency-critical path shared with other
+ * streams, because cudaMalloc / cudaFree make the whole device wait, not only this handle's stream.  mdpd_get_pairs
+ * does two cudaMalloc + two cudaFree per call; this variant does none, and calls no other allocating runtime or
+ * library routine.
+ *
+ * How: the scratch of the pair search (an 8-byte hit counter and the unsorted pair buffer) is a fixed array inside the
+ * library image instead: 256 + 8 * MDPD_STATIC_PAIRS_MAX bytes (about 4 MiB) of every GPU that loads the library,
+ * held until the process exits.  Arguments, result and errors are those of mdpd_get_pairs (same kernel, same fp32
+ * predicate, same sorted output in HOST memory `pairs`; inputs and outputs stay the caller's), except:
+ *   - cap > MDPD_STATIC_PAIRS_MAX is refused with MDPD_EINVAL (text in mdpd_last_error) before anything runs.  As in
+ *     mdpd_get_pairs, *count may exceed cap: it is the number found, of which the first cap in device order are kept.
+ *   - MDPD_ESTATE between mdpd_profile_begin and mdpd_profile_end (the per-kernel timing creates events on demand).
+ *   - The handle's own workspace must already exist (mdpd_load_particles has run); with mdpd_set_workspace that one is
+ *     the caller's memory too.
+ *   - The first call on a device is also a set-up call: it looks up the array's device address
+ *     (cudaGetSymbolAddress, once per device, return code checked).  Make that first call before any stream capture
+ *     is begun on the device.
+ *   - ONE array per device serves every handle and every call, and it keeps what the last call wrote.  The library
+ *     zeroes the counter at the start of each call (on the handle's stream); the pair slots need no clearing.  Two
+ *     calls whose GPU work can overlap -- two handles on different streams, two host threads -- race on the array
+ *     and return garbage: serialise them yourself.  A handle is not thread-safe anyway.
+ * Synchronises the handle's stream. */
+#define MDPD_STATIC_PAIRS_MAX 524288u
+int mdpd_get_pairs_static(mdpd_ctx* h, float rcut, uint64_t* count, uint32_t* pairs, uint64_t cap);
+
 /* Run the DEVICE hash kernel: out[q] = HASH(min(pairs[q]), max(pairs[q]), step, seed of the handle).
  * pairs: [npairs][2] uint32, out: [npairs] uint32, host or device.  Diagnostic: allocates 12 bytes per pair with
  * cudaMalloc and frees them before returning. */

@@ -26,9 +26,10 @@ _ERRNAME = {-1: "MDPD_EINVAL", -2: "MDPD_ENOMEM", -3: "MDPD_ECUDA", -4: "MDPD_EO
 SYMBOLS = ("mdpd_create", "mdpd_destroy", "mdpd_set_params", "mdpd_set_pair_params", "mdpd_workspace_bytes", "mdpd_set_workspace",
            "mdpd_load_particles", "mdpd_load_wall_mask", "mdpd_step", "mdpd_get_state", "mdpd_set_step_counter",
            "mdpd_set_forces",
-           "mdpd_compute_forces", "mdpd_compute_virial", "mdpd_get_pairs", "mdpd_rng_fill", "mdpd_get_counters", "mdpd_last_error",
+           "mdpd_compute_forces", "mdpd_compute_virial", "mdpd_get_pairs", "mdpd_get_pairs_static", "mdpd_rng_fill", "mdpd_get_counters", "mdpd_last_error",
            "mdpd_profile_begin", "mdpd_profile_end", "mdpd_profile_name", "mdpd_probe_issue_rates")
 MDPD_PROF_SLOTS = 16
+MDPD_STATIC_PAIRS_MAX = 524288   # include/mdpd.h: pairs the fixed scratch of mdpd_get_pairs_static holds
 
 
 class MdpdError(RuntimeError):
@@ -88,6 +89,7 @@ def lib():
         L.mdpd_compute_forces.argtypes = [vp]
         L.mdpd_compute_virial.argtypes = [vp, vp]
         L.mdpd_get_pairs.argtypes = [vp, f32, vp, vp, u64]
+        L.mdpd_get_pairs_static.argtypes = [vp, f32, vp, vp, u64]
         L.mdpd_rng_fill.argtypes = [vp, u64, vp, u32, vp]
         L.mdpd_get_counters.argtypes = [vp, vp]
         L.mdpd_last_error.argtypes = [vp]
@@ -279,6 +281,22 @@ class Simulation:
         self._ck(self._L.mdpd_get_pairs(self._h, float(rcut), C.addressof(cnt), pairs.ctypes.data, m),
                  "mdpd_get_pairs")
         return pairs[:min(m, int(cnt.value))]
+
+    def get_pairs_static(self, rcut, cap=None):
+        """``mdpd_get_pairs_static``: the pairs of :meth:`get_pairs`, found without a single device allocation (the
+        scratch is a fixed array inside the library; see include/mdpd.h for who needs that and for the sharing rules).
+        cap = None counts first and then fetches exactly that many; more than MDPD_STATIC_PAIRS_MAX pairs raise
+        MdpdError(MDPD_EINVAL).  Returns the sorted [m][2] uint32 tag pairs."""
+        cnt = C.c_uint64()
+        if cap is None:
+            self._ck(self._L.mdpd_get_pairs_static(self._h, float(rcut), C.addressof(cnt), None, 0),
+                     "mdpd_get_pairs_static")
+            cap = int(cnt.value)
+        cap = int(cap)
+        pairs = np.empty((max(cap, 1), 2), np.uint32)
+        self._ck(self._L.mdpd_get_pairs_static(self._h, float(rcut), C.addressof(cnt), pairs.ctypes.data, cap),
+                 "mdpd_get_pairs_static")
+        return pairs[:min(cap, int(cnt.value))]
 
     def rng_fill(self, pairs, step):
         pairs = np.ascontiguousarray(pairs, np.uint32).reshape(-1, 2)

@@ -18,6 +18,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -1835,6 +1836,45 @@ __global__ void __launch_bounds__(512) k_pairs(const DevP p, float rcut2, uint2*
   }
 }
 
+}  // namespace (left for a moment: the scratch array below sits at file scope)
+
+// ----------------------------------------------------------------------------------------------------------------
+// Fixed scratch of mdpd_get_pairs_static: the hit counter of k_pairs (first 8 bytes; the rest of the first 256 bytes
+// is padding that keeps the pair buffer aligned) followed by room for MDPD_STATIC_PAIRS_MAX (tag, tag) pairs.  It is
+// part of the library image, so every GPU that loads the library carries these ~4 MiB until the process exits, and
+// nobody ever has to allocate or free them.
+//
+// The name below is only usable as an address inside device code.  On the host it is a stand-in symbol of the
+// runtime, NOT a device pointer: a kernel handed `g_pairs_scratch` from host code would fault (or, where the GPU can
+// reach host memory, scribble over whatever lives there).  Host code therefore asks the runtime for the real
+// address, once per device and with that device current (static_pairs_scratch below), and hands THAT to the kernel.
+// ----------------------------------------------------------------------------------------------------------------
+constexpr size_t STATIC_PAIRS_HEAD = 256;  // bytes in front of the pair buffer (counter + padding)
+static __device__ __align__(256) unsigned char g_pairs_scratch[STATIC_PAIRS_HEAD + (size_t)MDPD_STATIC_PAIRS_MAX * sizeof(uint2)];
+
+constexpr int STATIC_MAXDEV = 64;                    // device ordinals this table covers
+static unsigned char* g_pairs_scratch_addr[STATIC_MAXDEV];  // resolved device address per ordinal, nullptr = not yet asked
+static std::mutex g_pairs_scratch_mu;
+
+// Device address of g_pairs_scratch on `device`, which must be the current device.  The first call per device asks
+// the runtime (this is what makes the first mdpd_get_pairs_static call on a device a set-up call); later calls read
+// the table.  Returns cudaSuccess or the runtime's error.
+static cudaError_t static_pairs_scratch(int device, unsigned char** out) {
+  if (device < 0 || device >= STATIC_MAXDEV) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_pairs_scratch_mu);
+  if (!g_pairs_scratch_addr[device]) {
+    void* ptr = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(&ptr, g_pairs_scratch);
+    if (e != cudaSuccess) return e;
+    if (!ptr) return cudaErrorInvalidSymbol;
+    g_pairs_scratch_addr[device] = (unsigned char*)ptr;
+  }
+  *out = g_pairs_scratch_addr[device];
+  return cudaSuccess;
+}
+
+namespace {
+
 __global__ void k_rng_fill(unsigned long long n, const uint2* __restrict__ pairs, unsigned step, unsigned seed,
                            unsigned* __restrict__ out) {
   unsigned long long q = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -2857,6 +2897,62 @@ int mdpd_get_pairs(mdpd_ctx* h, float rcut, uint64_t* count, uint32_t* pairs, ui
   cudaFree(dcnt);
   if (dout) cudaFree(dout);
   if (e != cudaSuccess) return set_err(h, MDPD_ECUDA, "get_pairs: %s", cudaGetErrorString(e));
+  *count = c;
+  return MDPD_OK;
+}
+
+// mdpd_get_pairs for callers that cannot allocate device memory (see include/mdpd.h): same kernel, same result,
+// but the counter and the pair buffer live in g_pairs_scratch instead of two cudaMalloc blocks.  Nothing in here calls
+// cudaMalloc / cudaFree or a routine that allocates behind the caller's back: the copies go through the runtime's
+// own staging, the sort is in place.
+int mdpd_get_pairs_static(mdpd_ctx* h, float rcut, uint64_t* count, uint32_t* pairs, uint64_t cap) {
+  if (!h || !count) return MDPD_EINVAL;
+  if (!h->loaded) return set_err(h, MDPD_ESTATE, "load_particles first");
+  if (!(rcut > 0) || rcut > h->L.rlist) return set_err(h, MDPD_EINVAL, "rcut must be in (0, rc + skin]");
+  if (!pairs) cap = 0;
+  if (cap > (uint64_t)MDPD_STATIC_PAIRS_MAX)
+    return set_err(h, MDPD_EINVAL,
+                   "mdpd_get_pairs_static: cap = %llu pairs does not fit the fixed scratch array (MDPD_STATIC_PAIRS_MAX = %u "
+                   "pairs); ask for fewer pairs or use mdpd_get_pairs, which allocates",
+                   (unsigned long long)cap, (unsigned)MDPD_STATIC_PAIRS_MAX);
+  if (h->prof_on)  // the per-kernel timing creates CUDA events on demand, which this entry point promises not to do
+    return set_err(h, MDPD_ESTATE, "mdpd_get_pairs_static: not between mdpd_profile_begin and mdpd_profile_end");
+  CU_TRY(h, cudaSetDevice(h->device));
+  *count = 0;
+  if (h->n == 0) return MDPD_OK;
+  unsigned char* base = nullptr;
+  {
+    cudaError_t e = static_pairs_scratch(h->device, &base);  // first call on this device: resolves the address
+    if (e != cudaSuccess)
+      return set_err(h, MDPD_ECUDA, "mdpd_get_pairs_static: cudaGetSymbolAddress of the scratch array failed: %s",
+                     cudaGetErrorString(e));
+  }
+  unsigned long long* dcnt = (unsigned long long*)base;
+  uint2* dout = (uint2*)(base + STATIC_PAIRS_HEAD);
+  // The array still holds whatever the previous call left.  Only the counter has to start at zero: the pair slots
+  // below the new count are all rewritten, the ones above it are never read.
+  CU_TRY(h, cudaMemsetAsync(dcnt, 0, sizeof(unsigned long long), h->stream));
+  // The opt-in to more than 48 KB of dynamic shared memory belongs to the kernel function on this device, not to a
+  // handle: a later mdpd_load_particles of ANOTHER handle with smaller tiles lowers it.  Re-assert this handle's size
+  // (a host-side setting, no allocation) so that the launch below cannot be refused for that reason.
+  CU_TRY(h, cudaFuncSetAttribute(k_pairs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
+  if (h->direct) {  // the list-free path keeps no Verlet list: build one from the current cells (workspace memory only)
+    LAUNCH(h, PS_OTHER, (k_reset_list_stats<<<1, 1, 0, h->stream>>>(h->d, 1, 0)));
+    launch_cells(h, 0, false, 1);
+  }
+  LAUNCH(h, PS_OTHER, (k_pairs<<<h->d.ntiles, h->block, h->smem_pos, h->stream>>>(h->d, rcut * rcut, dout, cap, dcnt)));
+  CU_TRY(h, cudaGetLastError());
+  unsigned long long c = 0;
+  CU_TRY(h, cudaMemcpyAsync(&c, dcnt, sizeof c, cudaMemcpyDeviceToHost, h->stream));
+  CU_TRY(h, cudaStreamSynchronize(h->stream));
+  if (cap) {
+    const uint64_t m = std::min<uint64_t>(c, cap);
+    CU_TRY(h, cudaMemcpyAsync(pairs, dout, m * sizeof(uint2), cudaMemcpyDeviceToHost, h->stream));
+    CU_TRY(h, cudaStreamSynchronize(h->stream));
+    struct TagPair { uint32_t a, b; };  // same bytes as the caller's [m][2] uint32 rows
+    TagPair* tp = reinterpret_cast<TagPair*>(pairs);
+    std::sort(tp, tp + m, [](const TagPair& x, const TagPair& y) { return x.a != y.a ? x.a < y.a : x.b < y.b; });
+  }
   *count = c;
   return MDPD_OK;
 }
