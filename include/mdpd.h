@@ -218,6 +218,11 @@ int mdpd_profile_end(mdpd_ctx* h, double ms[MDPD_PROF_SLOTS], uint64_t launches[
 /* Name of a kernel slot ("k_force", "k_density", ...; "" past the last one).  Static storage. */
 const char* mdpd_profile_name(int slot);
 
+/* The extra -D options this library was compiled with, sorted and comma-joined ("" for the plain build;
+ * "-DMDPD_CHECKS" for the build with the kernels' own bounds checks, "-DMDPD_FIRST_TILE=..." for a measurement build).
+ * bench.py prints it in its JSON line so that a timing can never be taken on a checks build unnoticed.  Static storage. */
+const char* mdpd_build_flags(void);
+
 /* Issue-rate probe for the ALU roofline: runs three short register-only kernels on `device`
  * (every SM, 64 resident warps, 8 independent dependency chains per thread), timed with CUDA events on `cuda_stream`, and
  * returns warp-instructions per second of the whole GPU: out[0] FP32 FMA (FFMA), out[1] logic pipe (LOP3 + VIMNMX),

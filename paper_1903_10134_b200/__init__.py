@@ -4,6 +4,6 @@
 ``binding.py`` is the thin ctypes layer; ``build.py`` compiles the library in-tree with nvcc.
 Importing the package never builds and never falls back to a CPU path.
 """
-from .binding import (LIB_PATH, SYMBOLS, MdpdError, Simulation, lib, make_params, mdpd_params,  # noqa: F401
+from .binding import (LIB_PATH, SYMBOLS, MdpdError, Simulation, build_flags, lib, make_params, mdpd_params,  # noqa: F401
                       probe_issue_rates)
 from .build import build  # noqa: F401

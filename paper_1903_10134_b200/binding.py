@@ -27,7 +27,7 @@ SYMBOLS = ("mdpd_create", "mdpd_destroy", "mdpd_set_params", "mdpd_set_pair_para
            "mdpd_load_particles", "mdpd_load_wall_mask", "mdpd_step", "mdpd_get_state", "mdpd_set_step_counter",
            "mdpd_set_forces",
            "mdpd_compute_forces", "mdpd_compute_virial", "mdpd_get_pairs", "mdpd_get_pairs_static", "mdpd_rng_fill", "mdpd_get_counters", "mdpd_last_error",
-           "mdpd_profile_begin", "mdpd_profile_end", "mdpd_profile_name", "mdpd_probe_issue_rates")
+           "mdpd_profile_begin", "mdpd_profile_end", "mdpd_profile_name", "mdpd_build_flags", "mdpd_probe_issue_rates")
 MDPD_PROF_SLOTS = 16
 MDPD_STATIC_PAIRS_MAX = 524288   # include/mdpd.h: pairs the fixed scratch of mdpd_get_pairs_static holds
 
@@ -99,6 +99,8 @@ def lib():
         L.mdpd_profile_name.argtypes = [i32]
         L.mdpd_profile_name.restype = C.c_char_p
         L.mdpd_probe_issue_rates.argtypes = [i32, vp, vp]
+        L.mdpd_build_flags.argtypes = []
+        L.mdpd_build_flags.restype = C.c_char_p
         for s in SYMBOLS:
             getattr(L, s).restype = getattr(L, s).restype  # touch: AttributeError if a symbol is missing
         _lib = L
@@ -116,6 +118,11 @@ def _ptr(a):
 
 COUNTER_NAMES = ("steps", "rebuilds", "bounces", "max_nbr", "sum_nbr", "max_staged", "faults", "launches",
                  "sum_act", "density_passes", "tile_shape", "ntiles")
+
+
+def build_flags() -> str:
+    """``mdpd_build_flags``: the extra -D options of the loaded library ("" = the plain build)."""
+    return lib().mdpd_build_flags().decode()
 
 
 def probe_issue_rates(device: int = 0, stream=None):

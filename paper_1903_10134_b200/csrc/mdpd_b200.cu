@@ -976,7 +976,6 @@ constexpr int CELLS_MAXW0 = CELLS_W0;  // most warps per CTA of the list build (
 constexpr int CELLS_MAXW = 8;          // ... of the list-free pass
 constexpr int CHMAX = 12;             // candidate chunks (of 32) held in registers at a time: one window
 constexpr unsigned ROW_SLACK = 40;    // row capacity beyond the list capacity: the saturated count (cap + 1) plus one chunk's worth of hits
-constexpr unsigned CELLS_ITEMS = 64;  // work items per tile: at most one per own cell
 
 __host__ __device__ inline unsigned cells_row_bytes(unsigned rowcap) {
   unsigned b = 2u * (rowcap + ROW_SLACK) + 16u;  // + one chunk of sentinel padding
@@ -1096,6 +1095,7 @@ __device__ __forceinline__ void cell_tests(const DevP& p, const CandRegs& C, con
       na = min(na + 2u * __popc(b), lim);
     }
     if (lane == 0) rowcnt[row] = (unsigned short)((na - ra) >> 1);
+    __syncwarp();  // orders this store before the re-read of rowcnt[row] by all lanes in the next window's call
   }
 }
 
@@ -1139,6 +1139,11 @@ __device__ __forceinline__ void cell_tests_flush(const DevP& p, const CandRegs& 
       MDPD_CHECK(p, na + 2u * __popc(b) <= ra + CELLS_ROW0_BYTES);
       if (hit) sts_u16(na + 2u * __popc(b & ltmask), C.s[t]);
       na += 2u * __popc(b);
+      // A single window (FIRST && LAST) cannot outgrow the row: 32 NCH - 1 hits at most.  When the fill is carried
+      // from window to window it can (a collapsed cluster, many coincident particles: R10 allows them), so there the
+      // write address saturates one chunk short of the row's end: 360 entries, far above any capacity (<= 128), so a
+      // saturated row still reads as an overflow below, and no store leaves the row.
+      if (!(FIRST && LAST)) na = min(na, ra + CELLS_ROW0_BYTES - 64u);
     }
     __syncwarp();
     unsigned n = (na - ra) >> 1;
@@ -2223,6 +2228,61 @@ bool choose_blocks(mdpd_ctx* h, unsigned max_own) {
 }
 
 // k_cells: mode 0 = Verlet list build, mode 1 = the list-free per-step pass (rho, compact list, hand-out of the force pass)
+// Every kernel that stages a tile in dynamic shared memory.  The opt-in to more than 48 KB belongs to the FUNCTION on the
+// device, not to a handle: were it set to each handle's own size, the load of a second handle with smaller tiles would
+// lower it under the first handle's launches ("invalid argument").  So every function is opened to the device's limit
+// minus its own static shared memory (the mbarrier of stage_bulk, the (A, B) table of k_force), whoever loads.
+#define MDPD_UNPAREN(...) __VA_ARGS__
+#define MDPD_TILE_KERNELS(X)                                                                                            \
+  X((k_cells<0, false, false>)) \
+  X((k_cells<1, false, false>)) \
+  X((k_cells<1, true, false>)) \
+  X((k_cells<1, true, true>)) \
+  X((k_density<true, true, DENS_TPB>)) \
+  X((k_density<true, false, DENS_TPB>)) \
+  X((k_density<false, false, DENS_TPB>)) \
+  X((k_density<true, true, DENS_TPB2>)) \
+  X((k_density<true, false, DENS_TPB2>)) \
+  X((k_density<false, false, DENS_TPB2>)) \
+  X((k_pairs)) \
+  X((k_force<true, false>)) \
+  X((k_force<false, false>)) \
+  X((k_force<true, true>)) \
+  X((k_force<true, false, false, true>)) \
+  X((k_force<false, false, false, true>)) \
+  X((k_force<true, true, true>)) \
+  X((k_force<true, false, true>)) \
+  X((k_force<false, true>))
+
+// Largest static shared memory of any tile kernel: what the capacity search has to leave free beside the dynamic part.
+cudaError_t tile_static_smem(size_t* out) {
+  size_t m = 0;
+  cudaFuncAttributes a;
+  cudaError_t e;
+#define X(fn)                                                      \
+  e = cudaFuncGetAttributes(&a, (const void*)(MDPD_UNPAREN fn));  \
+  if (e != cudaSuccess) return e;                                  \
+  m = std::max(m, a.sharedSizeBytes);
+  MDPD_TILE_KERNELS(X)
+#undef X
+  *out = m;
+  return cudaSuccess;
+}
+
+cudaError_t allow_tile_smem(mdpd_ctx* h) {
+  cudaFuncAttributes a;
+  cudaError_t e;
+#define X(fn)                                                                                                          \
+  e = cudaFuncGetAttributes(&a, (const void*)(MDPD_UNPAREN fn));                                                      \
+  if (e != cudaSuccess) return e;                                                                                      \
+  e = cudaFuncSetAttribute((const void*)(MDPD_UNPAREN fn), cudaFuncAttributeMaxDynamicSharedMemorySize,               \
+                           (int)(h->smem_limit - a.sharedSizeBytes));                                                  \
+  if (e != cudaSuccess) return e;
+  MDPD_TILE_KERNELS(X)
+#undef X
+  return cudaSuccess;
+}
+
 int launch_cells(mdpd_ctx* h, int mode, bool all, int always) {
   const DevP& d = h->d;
   const unsigned tpb = h->cells_warps[mode] * 32u;
@@ -2601,7 +2661,10 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
       }
       h->d.dot_margin = (float)(6e-6 * x2);
     }
-    const size_t fixed = tile_smem_bytes(0, true, 0);
+    // fixed part of a tile kernel's shared memory: tables of the staged image + the largest static allocation of any of them
+    size_t stat = 0;
+    CU_TRY(h, tile_static_smem(&stat));
+    const size_t fixed = tile_smem_bytes(0, true, 0) + stat;
     // capacity of a tile + halo in staged slots: what the force pass can hold in shared memory, what a 16-bit list entry can
     // address, and what the item list of stage_fast (2 * HTAB items: 3 * 36 runs + one item per 32 slots) can describe
     const unsigned cap_limit = (unsigned)std::min<size_t>(std::min<size_t>((h->smem_limit - fixed) / TILE_SLOT_BYTES, 65535),
@@ -2638,14 +2701,14 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
         const unsigned two = half > 1024 + fixed ? (unsigned)((half - 1024 - fixed) / TILE_SLOT_BYTES / 64 * 64) : 0u;
         if (want > two && (double)max_halo * 1.08 + 64.0 <= (double)two) want = two;
       }
-      const size_t per_cta = tile_smem_bytes(want, true, 0) + 1024;
+      const size_t per_cta = tile_smem_bytes(want, true, 0) + stat + 1024;
       const size_t ctas = std::max<size_t>(1, sm_total / per_cta);
       const size_t room = sm_total / ctas - 1024 - fixed;
       // ... nor one of the density pass (positions only, DENS_MINB CTAs per SM) or of the list build (two): when the force pass is
       // down to one CTA per SM the capacity must not grow into the other passes' occupancy
       const auto slots_for = [&](size_t n_ctas, size_t slot_bytes, size_t extra) {
         const size_t per = sm_total / n_ctas;
-        const size_t fix = 1024 + tile_smem_bytes(0, false, 0) + extra;
+        const size_t fix = 1024 + tile_smem_bytes(0, false, 0) + stat + extra;
         return per > fix ? (per - fix) / slot_bytes : 0;
       };
       const size_t grow = std::min(std::min<size_t>(room / TILE_SLOT_BYTES, slots_for(DENS_MINB, 16, 0)),
@@ -2670,25 +2733,7 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
     h->cells_warps[mode] = (unsigned)std::min<size_t>(nw, mode ? CELLS_MAXW : CELLS_MAXW0);
     h->smem_cells[mode] = base + h->cells_warps[mode] * rowb;
   }
-  CU_TRY(h, (cudaFuncSetAttribute(k_cells<0, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_cells[0])));
-  CU_TRY(h, (cudaFuncSetAttribute(k_cells<1, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_cells[1])));
-  CU_TRY(h, (cudaFuncSetAttribute(k_cells<1, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_cells[1])));
-  CU_TRY(h, (cudaFuncSetAttribute(k_cells<1, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_cells[1])));
-  CU_TRY(h, (cudaFuncSetAttribute(k_density<true, true, DENS_TPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos)));
-  CU_TRY(h, (cudaFuncSetAttribute(k_density<true, false, DENS_TPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos)));
-  CU_TRY(h, (cudaFuncSetAttribute(k_density<false, false, DENS_TPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos)));
-  CU_TRY(h, (cudaFuncSetAttribute(k_density<true, true, DENS_TPB2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos)));
-  CU_TRY(h, (cudaFuncSetAttribute(k_density<true, false, DENS_TPB2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos)));
-  CU_TRY(h, (cudaFuncSetAttribute(k_density<false, false, DENS_TPB2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos)));
-  CU_TRY(h, cudaFuncSetAttribute(k_pairs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
-  CU_TRY(h, cudaFuncSetAttribute(k_force<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
-  CU_TRY(h, cudaFuncSetAttribute(k_force<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
-  CU_TRY(h, cudaFuncSetAttribute(k_force<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
-  CU_TRY(h, (cudaFuncSetAttribute(k_force<true, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel)));
-  CU_TRY(h, (cudaFuncSetAttribute(k_force<false, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel)));
-  CU_TRY(h, (cudaFuncSetAttribute(k_force<true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel)));
-  CU_TRY(h, (cudaFuncSetAttribute(k_force<true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel)));
-  CU_TRY(h, cudaFuncSetAttribute(k_force<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_posvel));
+  CU_TRY(h, allow_tile_smem(h));
   if (n) {
     // the recipe again, now against the final capacity (a tile that does not fit is flagged), then the list and the forces
     LAUNCH(h, PS_RECIPE, (k_tile_recipe<<<h->d.ntiles, 128, 0, h->stream>>>(h->d, 1)));
@@ -2932,10 +2977,6 @@ int mdpd_get_pairs_static(mdpd_ctx* h, float rcut, uint64_t* count, uint32_t* pa
   // The array still holds whatever the previous call left.  Only the counter has to start at zero: the pair slots
   // below the new count are all rewritten, the ones above it are never read.
   CU_TRY(h, cudaMemsetAsync(dcnt, 0, sizeof(unsigned long long), h->stream));
-  // The opt-in to more than 48 KB of dynamic shared memory belongs to the kernel function on this device, not to a
-  // handle: a later mdpd_load_particles of ANOTHER handle with smaller tiles lowers it.  Re-assert this handle's size
-  // (a host-side setting, no allocation) so that the launch below cannot be refused for that reason.
-  CU_TRY(h, cudaFuncSetAttribute(k_pairs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_pos));
   if (h->direct) {  // the list-free path keeps no Verlet list: build one from the current cells (workspace memory only)
     LAUNCH(h, PS_OTHER, (k_reset_list_stats<<<1, 1, 0, h->stream>>>(h->d, 1, 0)));
     launch_cells(h, 0, false, 1);
@@ -3014,6 +3055,11 @@ int mdpd_profile_end(mdpd_ctx* h, double ms[MDPD_PROF_SLOTS], uint64_t launches[
   h->prof_recs.clear();
   return MDPD_OK;
 }
+
+#ifndef MDPD_BUILD_FLAGS
+#define MDPD_BUILD_FLAGS ""
+#endif
+const char* mdpd_build_flags(void) { return MDPD_BUILD_FLAGS; }
 
 const char* mdpd_profile_name(int slot) { return (slot >= 0 && slot < PS_COUNT) ? kProfNames[slot] : ""; }
 

@@ -307,6 +307,63 @@ def test_dense_system_takes_the_multi_window_list_build(gpu):
         s.close()
 
 
+@pytest.mark.parametrize("flags", [0, 2])
+def test_collapsed_cluster_overflows_cleanly(gpu, flags):
+    """600 particles inside a sphere of radius 0.3 (R10 allows coincident and near-coincident particles): every one of
+    them has ~600 candidates inside rc + skin, more than the 392 entries of a warp's row in the list build, and the row
+    fill is carried across the windows of the stencil.  The write address has to saturate inside the row: the answer
+    is MDPD_EOVERFLOW, not an illegal address that poisons the CUDA context -- the second simulation proves the
+    context is still alive."""
+    c = wl.make_liquid(6.0, seed=31)
+    rng = np.random.default_rng(32)
+    u = rng.normal(size=(600, 3))
+    u *= (0.3 * rng.random((600, 1)) ** (1 / 3)) / np.linalg.norm(u, axis=1, keepdims=True)
+    c["pos"][:600] = (np.array([3.1, 2.9, 3.3]) + u).astype(np.float32)
+    prm = dict(c["params"])
+    prm["flags"] = flags
+    s = gpu.Simulation(prm)
+    with pytest.raises(gpu.MdpdError) as e:
+        s.load_particles(c["pos"], c["vel"], c["type"])
+        s.step(1)
+        s.get_state()
+    assert e.value.code == -4, e.value                  # MDPD_EOVERFLOW
+    s.close()
+    ok = wl.make_liquid(5.0, seed=33)
+    s = gpu.Simulation(ok["params"])
+    s.load_particles(ok["pos"], ok["vel"], ok["type"])
+    s.step(2)
+    assert np.isfinite(s.get_state()["pos"]).all() and s.counters()["faults"] == 0
+    s.close()
+
+
+def test_two_handles_with_different_tile_sizes(gpu):
+    """The opt-in to large dynamic shared memory is a property of the kernel FUNCTION on the device.  A handle with big
+    tiles (dense liquid) must keep working after a second handle with small tiles (dilute gas) has been loaded: pair
+    search, force evaluation and stepping, interleaved."""
+    big = wl.make_liquid((7.5, 6.3, 5.1), density=9.5, seed=21)
+    small = wl.make_liquid(5.0, density=3.0, seed=22)
+    a = gpu.Simulation(big["params"])
+    a.load_particles(big["pos"], big["vel"], big["type"])
+    pa, sa = a.get_pairs(1.0), a.get_state()
+    assert len(pa) > 10000
+    b = gpu.Simulation(small["params"])
+    b.load_particles(small["pos"], small["vel"], small["type"])
+    pb = b.get_pairs(1.0)
+    assert 0 < len(pb) < len(pa)
+    assert np.array_equal(a.get_pairs(1.0), pa)              # a's kernels still launch after b's load
+    a.compute_forces()
+    s2 = a.get_state()
+    assert np.array_equal(s2["rho"], sa["rho"]) and np.array_equal(s2["force"], sa["force"])
+    for _ in range(3):
+        a.step(2)
+        b.step(2)
+    assert a.counters()["faults"] == 0 and b.counters()["faults"] == 0
+    assert np.array_equal(b.get_pairs(0.75), b.get_pairs_static(0.75))
+    assert np.array_equal(a.get_pairs(0.75), a.get_pairs_static(0.75))
+    a.close()
+    b.close()
+
+
 def test_tile_that_outgrows_its_capacity_is_reported(gpu):
     """headroom = 1.0: the shared-memory capacity of a tile is the fullest tile of the LOADED state.  A dilute gas that
     condenses (A = -40 at number density 3) outgrows it; the run must end in MDPD_EOVERFLOW, not in silent missing
