@@ -131,12 +131,12 @@ def host_cpu():
     return {"cpu_model": model, "nproc": os.cpu_count(), "threads_used": 1}
 
 
-def run_oracle_sample(workload, nsteps, edge, warm=0):
+def run_oracle_sample(workload, nsteps, edge, warm=0, seed_offset=0):
     """Times `nsteps` timesteps of the fp64 oracle on a bounded sample of the workload.  Returns (rate, n, seconds)."""
     import mdpd_workloads as wl
     from oracle.mdpd_ref import RefSim
     if workload in ("4a", "4b"):
-        c = wl.make_liquid(float(edge), seed=wl.BASE_SEED + 4)
+        c = wl.make_liquid(float(edge), seed=wl.BASE_SEED + 4 + 1000 * seed_offset)
         sample = f"periodic mDPD liquid {edge}^3 at density 6 ({len(c['pos'])} particles), same parameters"
     else:
         c = wl.make_config(int(workload))
@@ -153,6 +153,38 @@ def run_oracle_sample(workload, nsteps, edge, warm=0):
     n = len(c["pos"])
     s.close()
     return n * nsteps / dt, n, dt, sample
+
+
+def run_oracle_all_cores(workload, nsteps, edge):
+    """SURVEY.md S8d / BASELINE.md S3 ("1 thread; and all physical cores"; the paper compares 36 cores with one GPU,
+    PAPER.md L219): the oracle has no threads and is not given any -- instead one independent oracle process per host
+    core, each on its own seeded sample of the same recipe (disjoint seeds), all started together; the figure is the SUM
+    of their rates.  That is the throughput the box's cores deliver on this method with the oracle as it stands (an upper
+    bound for any decomposed run of it: no halo exchange is paid)."""
+    import subprocess
+    from oracle.mdpd_ref import build as build_oracle
+    build_oracle()                       # once, before the workers load it
+    nproc = os.cpu_count() or 1
+    code = ("import sys, json; sys.path.insert(0, %r); import bench; "
+            "r = bench.run_oracle_sample(%r, %d, %d, seed_offset=1 + int(sys.argv[1])); print(json.dumps(r[:3]))"
+            % (ROOT, workload, nsteps, edge))
+    env = dict(os.environ, OMP_NUM_THREADS="1", CUDA_VISIBLE_DEVICES="")
+    t0 = time.perf_counter()
+    procs = [subprocess.Popen([sys.executable, "-c", code, str(k)], stdout=subprocess.PIPE, text=True, env=env)
+             for k in range(nproc)]
+    res = []
+    for pr in procs:
+        out, _ = pr.communicate(timeout=1800)
+        if pr.returncode != 0:
+            raise RuntimeError("an oracle worker of the all-cores leg failed")
+        res.append(json.loads(out.strip().splitlines()[-1]))
+    wall = time.perf_counter() - t0
+    return {"value": float(sum(r[0] for r in res)), "unit": UNIT, "processes": nproc, "cores": nproc,
+            "threads_used": nproc, "per_process_min": float(min(r[0] for r in res)),
+            "per_process_max": float(max(r[0] for r in res)),
+            "sample": f"{nproc} independent oracle processes, one per core, each {nsteps} timesteps of its own seeded "
+                      f"{edge}^3 liquid ({res[0][1]} particles); slowest {max(r[2] for r in res):.1f} s, wall {wall:.1f} s "
+                      "with start-up; value = sum of the processes' rates"}
 
 
 def main_reference(args, rank, world):
@@ -281,14 +313,15 @@ def main_ours(args, rank, world, local):
     tile_shape = [ts & 255, (ts >> 8) & 255, (ts >> 16) & 255]
 
     # ---- spread: three more windows of K steps, same protocol (several windows, mean and spread) --------
-    repeats = []
+    repeats_ms = []
     for _ in range(0 if args.no_repeats else 3):
         r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
         r0.record()
         sim.step(K)
         r1.record()
         torch.cuda.synchronize()
-        repeats.append(round(r0.elapsed_time(r1) / K, 4))
+        repeats_ms.append(r0.elapsed_time(r1))
     cp = sim.counters()
 
     # ---- per-kernel CUDA-event times over another K steps (same stream) --------------------------------------
@@ -375,16 +408,18 @@ def main_ours(args, rank, world, local):
     roof["method_minimum_frac"] = None if roof.get("frac") is None else round(0.5 * roof["frac"], 4)
     roof["step"]["alu_frac_method_minimum"] = round(0.5 * roof["step"]["alu_frac"], 4)
     # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) and the shared-memory data-pipe utilisation come
-    # from the committed ncu --set full capture of this workload, profiles/ncu_r2_<workload>.json, which records the
+    # from the committed ncu --set full capture of this workload, profiles/ncu_r3_<workload>.json (else ncu_r2_), which records the
     # SHA-256 of the kernel source it was taken from: a capture of another build is reported as stale, not as a number.
     roof["traffic"], roof["traffic_source"] = None, None
     try:
         import hashlib
-        cap = json.load(open(os.path.join(ROOT, "profiles", f"ncu_r2_{args.workload}.json")))
+        cap_name = next((f for f in (f"ncu_r3_{args.workload}.json", f"ncu_r2_{args.workload}.json")
+                         if os.path.exists(os.path.join(ROOT, "profiles", f))), f"ncu_r3_{args.workload}.json")
+        cap = json.load(open(os.path.join(ROOT, "profiles", cap_name)))
         src = os.path.join(ROOT, "paper_1903_10134_b200", "csrc", "mdpd_b200.cu")
         sha = hashlib.sha256(open(src, "rb").read()).hexdigest()
         if sha != cap.get("kernel_source_sha256"):
-            roof["traffic_source"] = (f"stale: profiles/ncu_r2_{args.workload}.json was captured at commit {cap.get('commit')} "
+            roof["traffic_source"] = (f"stale: profiles/{cap_name} was captured at commit {cap.get('commit')} "
                                       "from another version of csrc/mdpd_b200.cu")
         else:
             kc = cap.get("kernels", {})
@@ -395,7 +430,7 @@ def main_ours(args, rank, world, local):
                     per_kernel[k]["l1_data_pipe_frac_ncu"] = v.get("l1_data_pipe_frac")  # all LSU wavefronts: shared + global + local
             if dom in kc and not args.direct:
                 roof["traffic"] = kc[dom].get("dram_bytes_per_launch")
-            roof["traffic_source"] = f"profiles/ncu_r2_{args.workload}.json (ncu --set full, commit {cap.get('commit')})"
+            roof["traffic_source"] = f"profiles/{cap_name} (ncu --set full, commit {cap.get('commit')})"
     except FileNotFoundError:
         roof["traffic_source"] = f"no capture committed for workload {args.workload}"
     roof["hbm_peak_gbs"] = peak_gbs
@@ -421,13 +456,44 @@ def main_ours(args, rank, world, local):
     h2d = n * (12 + 12 + 1) + (int(np.prod(md)) if md is not None else 0)
     d2h = n * 24
 
+    # ---- the same measurement at the other skin (one window), so that the line shows what a caller with the recipe's
+    # default skin gets and what the tuned skin buys; only where the two differ (config 4a) --------------------
+    alt_ms, alt_skin = None, None
+    if skin is not None and args.skin is None and not args.no_repeats:
+        alt_skin = 0.25
+        sim.close()
+        prm2 = dict(c["params"], skin=alt_skin)
+        sim = pk.Simulation(prm2, device=local)
+        sim.load_particles(e_pos, e_vel, h_typ, mask_dims=md)      # the equilibrated state
+        if c.get("mask") is not None:
+            sim.load_wall_mask(c["mask"], c["voxel"])
+        sim.step(W + 20)
+        sim.counters()
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        a0.record()
+        sim.step(K)
+        a1.record()
+        torch.cuda.synchronize()
+        barrier()
+        alt_ms = a0.elapsed_time(a1)
+        sim.counters()
+
     # ---- max over ranks ---------------------------------------------------------------------------------------
-    ms, e2e_s = max_over_ranks([ms, e2e_s], world, "cuda")
-    value = whole_job_rate(n, K, world, ms * 1e-3)
+    # `value` is taken over ALL timed windows (the first plus the repeats: SURVEY.md S8d "4 windows ..., report mean and
+    # spread"): a window of K steps holds a whole number of list rebuilds, so single windows differ by one rebuild
+    # (+- 3 % at K = 20).  Every window is the max over ranks; value = particle-steps of all windows / their summed time.
+    red = max_over_ranks([ms, e2e_s] + repeats_ms + ([alt_ms] if alt_ms is not None else []), world, "cuda")
+    ms, e2e_s = red[0], red[1]
+    windows_ms = [ms] + red[2:2 + len(repeats_ms)]
+    if alt_ms is not None:
+        alt_ms = red[-1]
+    ms_mean = float(np.mean(windows_ms))
+    value = whole_job_rate(n, K, world, ms_mean * 1e-3)
     e2e_v = whole_job_rate(n, K, world, e2e_s)
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms_mean / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": workload_name(args.workload, n), "particles_per_gpu": n,
                        "parallelism": "replicas only" if world > 1 else "1 gpu",
@@ -440,13 +506,23 @@ def main_ours(args, rank, world, local):
             "e2e": {"value": e2e_v, "unit": UNIT, "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
                     "note": f"one job = load_particles(host, equilibrated state) + {K} steps + get_state(host); bytes are per job / {K}"},
             "gpu_launches": launches, "clocks": clocks, "roofline": roof, "kernels": kernels,
-            "repeat_windows_ms_per_step": repeats}   # this rank's next three windows of K steps (untimed for `value`)
+            "build_flags": pk.build_flags(),   # "" = the plain build (a -DMDPD_CHECKS library must never be timed)
+            "windows_ms_per_step": [round(w / K, 4) for w in windows_ms],   # every timed window of K steps; value = their mean
+            "windows_spread": round((max(windows_ms) - min(windows_ms)) / ms_mean, 4)}
+    if alt_ms is not None:
+        line["other_skin"] = {"skin": alt_skin, "ms_per_step": alt_ms / K, "value": whole_job_rate(n, K, world, alt_ms * 1e-3),
+                              "unit": UNIT, "windows": 1,
+                              "note": "the same workload and protocol at the other Verlet skin (0.25 is the input recipe's "
+                                      "default, 0.27 the value this bench times config 4a at; the skin is the caller's "
+                                      "parameter, mdpd_params.skin, and the library has no hidden default of its own)"}
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         edge = oracle_sample_edge(20.0 * 4.0e5 / 20)          # ~20 s: 20 steps of a ~4e5-particle box
         rate, ns, dt, sample = run_oracle_sample(args.workload, 20, edge)
         line["cpu_baseline"] = dict({"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
                                      "sample": f"{sample}; 20 timesteps in {dt:.1f} s (serial C, fp64, one thread)"}, **host_cpu())
+        if not args.no_all_cores:
+            line["cpu_baseline"]["all_cores"] = run_oracle_all_cores(args.workload, 20, edge)
     sim.close()
     if rank == 0:
         print(json.dumps(line), flush=True)
@@ -463,7 +539,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="4a", choices=["4a", "4b", "0", "1", "2", "3"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-repeats", action="store_true", help="skip the three extra windows that report the spread")
+    ap.add_argument("--no-repeats", action="store_true", help="skip the three extra windows (value = the first window only) and the other-skin leg")
+    ap.add_argument("--no-all-cores", action="store_true", help="skip the one-oracle-process-per-core leg of cpu_baseline")
     ap.add_argument("--equilibrate", type=int, default=EQUILIBRATE, help="untimed steps after loading")
     ap.add_argument("--direct", action="store_true", help="list-free path (MDPD_FLAG_DIRECT): no Verlet list")
     ap.add_argument("--tma", action="store_true", help="both tile passes stage with cp.async.bulk (MDPD_FLAG_TMA_STAGING)")

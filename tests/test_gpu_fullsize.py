@@ -56,8 +56,11 @@ def test_config4b_one_million_particles_every_particle(gpu):
     s.close()
 
 
-def test_config4a_32_million_particles_sampled(gpu):
-    """Config 4a (175^3 box, 32 156 250 particles), the workload bench.py times: 4 timesteps, then a SAMPLE the oracle
+@pytest.mark.parametrize("skin", [0.25, 0.27])
+def test_config4a_32_million_particles_sampled(gpu, skin):
+    """skin = 0.27 is the exact launch configuration bench.py times (137 cells per dimension: tiles of 3 and 4 cells
+    mixed, the 416-thread density CTAs); 0.25 is the input recipe's default (140 cells, all tiles 4 x 4 x 4).
+    Config 4a (175^3 box, 32 156 250 particles), the workload bench.py times: 4 timesteps, then a SAMPLE the oracle
     can afford: all particles of a 16^3 sub-cube are handed to the oracle in a 24^3 box (no periodic images interact),
     WITH THE TAGS THEY HAVE IN THE WHOLE SYSTEM (mdpd_ref_set_tags; pinned in tests/test_oracle_pins.py), so that the
     hashed random force at 32 M-particle tags is part of the comparison, and the ~13 000 particles at least rc + rd = 1.75
@@ -68,7 +71,9 @@ def test_config4a_32_million_particles_sampled(gpu):
     c = wl.make_config("4a")
     n = len(c["pos"])
     assert n == 32_156_250
-    s = gpu.Simulation(c["params"])
+    import bench
+    assert bench.TUNED_SKIN["4a"] == 0.27            # the skin bench.py times config 4a at: this test must follow it
+    s = gpu.Simulation(dict(c["params"], skin=skin))
     s.load_particles(c["pos"], c["vel"], c["type"])
     s.step(4)
     ctr = s.counters()
