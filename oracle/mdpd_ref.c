@@ -69,6 +69,12 @@ typedef struct mdpd_ref_ctx {
   int ntypes;
   double Am[MDPD_REF_MAXTYPES * MDPD_REF_MAXTYPES], Bm[MDPD_REF_MAXTYPES * MDPD_REF_MAXTYPES];
   uint32_t frozen_mask;
+  /* Per-type-pair dissipative / random amplitudes (every pair carries F^D = -gamma wD (e.v) e and
+   * F^R = sigma wR xi / sqrt(dt) e with sigma^2 = 2 gamma kT; the paper runs water at gamma = 12.4, and its
+   * other fluids at 4.5, so a two-fluid system needs gamma_ij, sigma_ij).  have_gs == 0: gamma and sigma
+   * of mdpd_ref_params for every pair. */
+  int have_gs;
+  double Gm[MDPD_REF_MAXTYPES * MDPD_REF_MAXTYPES], Sm[MDPD_REF_MAXTYPES * MDPD_REF_MAXTYPES];
   uint8_t *mask; /* [nz][ny][nx], 1 = solid */
   uint32_t mdim[3];
   double voxel;
@@ -165,6 +171,28 @@ int mdpd_ref_set_pair_params(mdpd_ref_ctx *h, int ntypes, const double *A, const
     }
   h->ntypes = ntypes;
   h->frozen_mask = frozen_mask;
+  h->have_gs = 0; /* the amplitude matrices belong to a species set: a new set starts without them */
+  return REF_OK;
+}
+
+/* gamma_ij, sigma_ij ([ntypes][ntypes], symmetric, ntypes = that of the last mdpd_ref_set_pair_params).  G == NULL or
+ * S == NULL: back to gamma, sigma of mdpd_ref_params for every pair.  The values may change at any time (they enter the
+ * next force evaluation); nothing is checked against kT: sigma_ij^2 = 2 gamma_ij kT is the caller's business. */
+int mdpd_ref_set_pair_gamma_sigma(mdpd_ref_ctx *h, int ntypes, const double *G, const double *S) {
+  if (!h) return REF_EINVAL;
+  if (!G || !S) {
+    h->have_gs = 0;
+    return REF_OK;
+  }
+  if (ntypes <= 0 || ntypes != h->ntypes) return REF_EINVAL;
+  for (int a = 0; a < ntypes; ++a)
+    for (int b = 0; b < ntypes; ++b) {
+      if (G[a * ntypes + b] != G[b * ntypes + a] || S[a * ntypes + b] != S[b * ntypes + a]) return REF_EINVAL;
+      if (!(G[a * ntypes + b] >= 0.0) || !(S[a * ntypes + b] >= 0.0)) return REF_EINVAL;
+      h->Gm[a * ntypes + b] = G[a * ntypes + b];
+      h->Sm[a * ntypes + b] = S[a * ntypes + b];
+    }
+  h->have_gs = 1;
   return REF_OK;
 }
 
@@ -304,9 +332,14 @@ static void force_pair(mdpd_ref_ctx *h, uint64_t i, uint64_t j, const double d[3
     Aij = h->Am[h->species[i] * h->ntypes + h->species[j]];
     Bij = h->Bm[h->species[i] * h->ntypes + h->species[j]];
   }
+  double gij = p->gamma, sij = p->sigma;
+  if (h->ntypes && h->have_gs) { /* per-type-pair amplitudes, P:L75 with P:L89 / P:L141 */
+    gij = h->Gm[h->species[i] * h->ntypes + h->species[j]];
+    sij = h->Sm[h->species[i] * h->ntypes + h->species[j]];
+  }
   double FC = Aij * w + Bij * (h->rho[i] + h->rho[j]) * wd;            /* Eq. (1) */
-  double FD = -p->gamma * wR * wR * ev;                                /* P:L75, wD = wR^2 */
-  double FR = p->sigma * wR * xi / sqrt(p->dt);                        /* P:L75; R2 */
+  double FD = -gij * wR * wR * ev;                                     /* P:L75, wD = wR^2 */
+  double FR = sij * wR * xi / sqrt(p->dt);                             /* P:L75; R2 */
   double F = FC + FD + FR;
   for (int k = 0; k < 3; ++k) {
     h->fpair[3 * i + k] += F * e[k];

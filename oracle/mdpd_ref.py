@@ -52,6 +52,7 @@ def lib():
         L.mdpd_ref_set_params.argtypes = [vp, C.POINTER(_Params)]
         L.mdpd_ref_set_brute_force.argtypes = [vp, C.c_int]
         L.mdpd_ref_set_pair_params.argtypes = [vp, C.c_int, vp, vp, u32]
+        L.mdpd_ref_set_pair_gamma_sigma.argtypes = [vp, C.c_int, vp, vp]
         L.mdpd_ref_compute_forces.argtypes = [vp]
         L.mdpd_ref_load_particles.argtypes = [vp, u64, vp, vp, vp]
         L.mdpd_ref_load_wall_mask.argtypes = [vp, vp, vp, C.c_double]
@@ -129,6 +130,19 @@ class RefSim:
         assert A.shape == (nt, nt) and B.shape == (nt, nt)
         _check(self._L.mdpd_ref_set_pair_params(self._h, nt, A.ctypes.data, B.ctypes.data, int(frozen_mask)),
                "set_pair_params")
+
+    def set_pair_gamma_sigma(self, G, S):
+        """Per-type-pair gamma_ij, sigma_ij ([nt][nt], symmetric, the two parameter sets of P:L89 and P:L141) for
+        the species set of the last set_pair_params; G = None: back to the uniform gamma, sigma.  Takes effect at the
+        next force evaluation."""
+        if G is None or S is None:
+            _check(self._L.mdpd_ref_set_pair_gamma_sigma(self._h, 0, None, None), "set_pair_gamma_sigma")
+            return
+        G = np.ascontiguousarray(G, np.float64)
+        S = np.ascontiguousarray(S, np.float64)
+        nt = G.shape[0]
+        assert G.shape == (nt, nt) and S.shape == (nt, nt)
+        _check(self._L.mdpd_ref_set_pair_gamma_sigma(self._h, nt, G.ctypes.data, S.ctypes.data), "set_pair_gamma_sigma")
 
     def load_particles(self, pos, vel, type=None):
         pos = np.ascontiguousarray(pos, np.float64).reshape(-1, 3)

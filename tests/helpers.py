@@ -55,9 +55,10 @@ def brute_density(pos, box, rd):
     return w.sum(1)
 
 
-def brute_forces(pos, vel, typ, p, step, rho=None, species=None, Amat=None, Bmat=None):
+def brute_forces(pos, vel, typ, p, step, rho=None, species=None, Amat=None, Bmat=None, Gmat=None, Smat=None):
     """O(N^2) total force per particle (pairwise part + m g on fluid), fp64, python-loop hash.
-    typ: frozen flags.  species / Amat / Bmat: per-type-pair A_ij, B_ij (Tables 1-2); default one material."""
+    typ: frozen flags.  species / Amat / Bmat: per-type-pair A_ij, B_ij (Tables 1-2); default one material.
+    Gmat / Smat: per-type-pair gamma_ij, sigma_ij; default the uniform gamma, sigma of p."""
     pos = np.asarray(pos, np.float64)
     vel = np.asarray(vel, np.float64).copy()
     typ = np.asarray(typ).astype(bool)
@@ -82,9 +83,11 @@ def brute_forces(pos, vel, typ, p, step, rho=None, species=None, Amat=None, Bmat
         wR = w ** p["s"]
         xi = xi_py(hash_py(i, j, step, p["seed"]))
         A, B = (p["A"], p["B"]) if species is None else (Amat[species[i]][species[j]], Bmat[species[i]][species[j]])
+        gam = p["gamma"] if Gmat is None else Gmat[species[i]][species[j]]
+        sig = p["sigma"] if Smat is None else Smat[species[i]][species[j]]
         F = (A * w + B * (rho[i] + rho[j]) * wd
-             - p["gamma"] * wR * wR * float(e @ (vel[i] - vel[j]))
-             + p["sigma"] * wR * xi / math.sqrt(p["dt"]))
+             - gam * wR * wR * float(e @ (vel[i] - vel[j]))
+             + sig * wR * xi / math.sqrt(p["dt"]))
         f[i] += F * e
         f[j] -= F * e
     fpair = f.copy()
