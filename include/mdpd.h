@@ -87,10 +87,22 @@ int mdpd_set_params(mdpd_ctx* h, const mdpd_params* p);
  * symmetric (else MDPD_EINVAL), ntypes <= 8.  After this call the `type` byte of mdpd_load_particles is the SPECIES
  * index s in [0, ntypes) (a larger value: MDPD_EINVAL at load), the pair (i, j) uses A[s_i][s_j], B[s_i][s_j] in place
  * of mdpd_params.A / .B, and species s is frozen (never integrated, v = 0, R8) iff bit s of frozen_mask is
- * set.  gamma, sigma, rc, rd stay those of mdpd_params for every pair.  Call before mdpd_load_particles; afterwards
+ * set.  rc, rd stay those of mdpd_params for every pair; gamma, sigma too unless mdpd_set_pair_gamma_sigma is used.  Call before mdpd_load_particles; afterwards
  * only the VALUES may change (same ntypes and frozen_mask, else MDPD_ESTATE).  ntypes = 0 returns to one material
  * (type byte != 0 <=> frozen wall). */
 int mdpd_set_pair_params(mdpd_ctx* h, uint32_t ntypes, const float* A, const float* B, uint32_t frozen_mask);
+
+/* Per-type-pair dissipative and random amplitudes (every pair carries F^D = -gamma w_D (e.v) e and
+ * F^R = sigma w_R xi e with sigma^2 = 2 gamma kT; the paper runs water at gamma = 12.4, L141, and its other fluids at 4.5,
+ * L89 and L186, so a run with two fluids needs them per pair of species).  gamma, sigma: [ntypes][ntypes] float32
+ * row-major HOST arrays, symmetric, >= 0 (else MDPD_EINVAL); ntypes must be that of the preceding mdpd_set_pair_params
+ * (else MDPD_EINVAL).  The pair (i, j) then uses gamma[s_i][s_j], sigma[s_i][s_j] in place of mdpd_params.gamma / .sigma.
+ * Nothing is checked against kT: sigma_ij^2 = 2 gamma_ij kT is the caller's choice.  NULL for either matrix returns to the
+ * uniform amplitudes; so does a later mdpd_set_pair_params with another ntypes.  May be called before or after
+ * mdpd_load_particles (new values enter the next force evaluation).  The paper also names a per-pair r_d (L153); it is
+ * NOT offered: r_d = 0.75 r_c "for all particle interactions" (L81, L89) and a per-pair r_d would change the density
+ * weight itself (R22). */
+int mdpd_set_pair_gamma_sigma(mdpd_ctx* h, uint32_t ntypes, const float* gamma, const float* sigma);
 
 /* Device bytes needed for n particles (+ an optional mask of mask_dims = {nx, ny, nz} voxels).  Returns 0 on bad input. */
 size_t mdpd_workspace_bytes(const mdpd_params* p, uint64_t n, int has_mask, const uint32_t mask_dims[3]);

@@ -23,7 +23,7 @@ _ERRNAME = {-1: "MDPD_EINVAL", -2: "MDPD_ENOMEM", -3: "MDPD_ECUDA", -4: "MDPD_EO
             -6: "MDPD_ENAN", -7: "MDPD_EINSOLID"}
 
 # every symbol include/mdpd.h declares
-SYMBOLS = ("mdpd_create", "mdpd_destroy", "mdpd_set_params", "mdpd_set_pair_params", "mdpd_workspace_bytes", "mdpd_set_workspace",
+SYMBOLS = ("mdpd_create", "mdpd_destroy", "mdpd_set_params", "mdpd_set_pair_params", "mdpd_set_pair_gamma_sigma", "mdpd_workspace_bytes", "mdpd_set_workspace",
            "mdpd_load_particles", "mdpd_load_wall_mask", "mdpd_step", "mdpd_get_state", "mdpd_set_step_counter",
            "mdpd_set_forces",
            "mdpd_compute_forces", "mdpd_compute_virial", "mdpd_get_pairs", "mdpd_get_pairs_static", "mdpd_rng_fill", "mdpd_get_counters", "mdpd_last_error",
@@ -77,6 +77,7 @@ def lib():
         L.mdpd_destroy.argtypes = [vp]
         L.mdpd_set_params.argtypes = [vp, pp]
         L.mdpd_set_pair_params.argtypes = [vp, u32, vp, vp, u32]
+        L.mdpd_set_pair_gamma_sigma.argtypes = [vp, u32, vp, vp]
         L.mdpd_workspace_bytes.argtypes = [pp, u64, i32, vp]
         L.mdpd_workspace_bytes.restype = C.c_size_t
         L.mdpd_set_workspace.argtypes = [vp, vp, C.c_size_t]
@@ -188,6 +189,19 @@ class Simulation:
         self.params.update(changes)
         self._p = make_params(self.params)
         self._ck(self._L.mdpd_set_params(self._h, C.byref(self._p)), "mdpd_set_params")
+
+    def set_pair_gamma_sigma(self, gamma, sigma):
+        """mdpd_set_pair_gamma_sigma: per-type-pair gamma_ij, sigma_ij ([nt][nt], symmetric) for the species set of the last
+        set_pair_params; None returns to the uniform amplitudes."""
+        if gamma is None or sigma is None:
+            self._ck(self._L.mdpd_set_pair_gamma_sigma(self._h, 0, None, None), "mdpd_set_pair_gamma_sigma")
+            return
+        G = np.ascontiguousarray(gamma, np.float32)
+        S = np.ascontiguousarray(sigma, np.float32)
+        nt = G.shape[0]
+        if G.shape != (nt, nt) or S.shape != (nt, nt):
+            raise ValueError("gamma and sigma must be [ntypes][ntypes]")
+        self._ck(self._L.mdpd_set_pair_gamma_sigma(self._h, nt, G.ctypes.data, S.ctypes.data), "mdpd_set_pair_gamma_sigma")
 
     def set_pair_params(self, A, B, frozen_mask=0):
         """mdpd_set_pair_params: per-type-pair A_ij, B_ij ([nt][nt], symmetric) and the frozen species (bit s)."""

@@ -122,6 +122,7 @@ struct DevP {  // passed by value to every kernel
   unsigned ntypes;           // 0: one material (type byte != 0 <=> frozen); else the type byte is a species index
   unsigned frozen_mask;      // bit s: species s is frozen
   float2 AB[MAXTYPES * MAXTYPES];  // per-type-pair (A, B) of Eq. (1), row = species_i * MAXTYPES (Tables 1-2)
+  float2 GS[MAXTYPES * MAXTYPES];  // per-type-pair (gamma, sig_c) of F^D, F^R (water 12.4 L141, other fluids 4.5 L89)
   float thr2;                // (skin / 2)^2
   unsigned seed;
 };
@@ -1659,12 +1660,12 @@ struct ForceAcc {
   float x, y, z;
 };
 
-// MULTI: per-type-pair (A, B) from the table `ab` in shared memory (row = species of i), else the handle's A, B
+// MULTI: per-type-pair (A, B, gamma, sig_c) from the table `ab` in shared memory (row = species of i), else the handle's
 // VIRIAL: also accumulate r_a F^C_b of the pair (conservative part of the stress, section 4.1 of the paper) into vir[6]
 template <bool MULTI, bool VIRIAL, bool SPOW>
 __device__ __forceinline__ void force_entry(const DevP& p, const unsigned pbase, const unsigned vbase, const float4 xi,
                                             const float4 vi, const unsigned tagi, const unsigned j, const HashKeys& K,
-                                            const float2* ab, ForceAcc& acc, float* vir) {
+                                            const float4* ab, ForceAcc& acc, float* vir) {
   MDPD_CHECK(p, j <= p.tile_cap);
   const float4 xj = lds4(pbase + (j << 4));
   const float4 vj = lds4(vbase + (j << 4));
@@ -1673,11 +1674,13 @@ __device__ __forceinline__ void force_entry(const DevP& p, const unsigned pbase,
   const float rinv = rsqrt_fast(r2);
   const float r = r2 * rinv;
   const float w = __saturatef(fmaf(-r, p.inv_rc, 1.0f));  // > 0 for in-range entries, 0 for the sentinel
-  float Aij = p.A, Bij = p.B;
-  if (MULTI) {  // the species sits in bits 28..30 of the particle word (A_SL, B_SL)
-    const float2 t = ab[(f2u(xj.w) >> TAG_BITS) & (MAXTYPES - 1u)];
+  float Aij = p.A, Bij = p.B, gam = p.gamma, sigc = p.sig_c;
+  if (MULTI) {  // the species sits in bits 28..30 of the particle word (A_SL, B_SL; L75: gamma, sigma)
+    const float4 t = ab[(f2u(xj.w) >> TAG_BITS) & (MAXTYPES - 1u)];
     Aij = t.x;
     Bij = t.y;
+    gam = t.z;
+    sigc = t.w;
   }
   float F = Aij * w;
   const float wd = __saturatef(fmaf(-r, p.inv_rd, 1.0f));
@@ -1694,10 +1697,10 @@ __device__ __forceinline__ void force_entry(const DevP& p, const unsigned pbase,
   const float ev = (dx * (vi.x - vj.x) + dy * (vi.y - vj.y) + dz * (vi.z - vj.z)) * rinv;
   // wR = w^s (wD = wR^2); s = 1 unless SPOW.  w = 0 (sentinel) gives exp2(-inf) = 0.
   const float wR = SPOW ? __powf(w, p.s_exp) : w;
-  F -= p.gamma * wR * wR * ev;
+  F -= gam * wR * wR * ev;
   const unsigned h = pair_hash(tagi, f2u(xj.w) & TAG_MASK, K);
   const float xi_s = (float)((int)(h >> 8) - (1 << 23));  // exact
-  F += p.sig_c * wR * xi_s;
+  F += sigc * wR * xi_s;
   const float Fr = F * rinv;
   acc.x += Fr * dx;
   acc.y += Fr * dy;
@@ -1707,9 +1710,10 @@ __device__ __forceinline__ void force_entry(const DevP& p, const unsigned pbase,
 template <bool ALL, bool MULTI, bool VIRIAL = false, bool SPOW = false>  // SPOW: general exponent s of wR; ALL: also evaluate the (never used) forces on frozen particles, for parity checks
 __global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
   extern __shared__ __align__(16) unsigned char smraw[];
-  __shared__ float2 s_ab[MULTI ? MAXTYPES * MAXTYPES : 1];
+  __shared__ float4 s_ab[MULTI ? MAXTYPES * MAXTYPES : 1];
   if (MULTI) {
-    for (unsigned q = threadIdx.x; q < MAXTYPES * MAXTYPES; q += blockDim.x) s_ab[q] = p.AB[q];  // ordered by stage_fast's barriers
+    for (unsigned q = threadIdx.x; q < MAXTYPES * MAXTYPES; q += blockDim.x)  // ordered by stage_fast's barriers
+      s_ab[q] = make_float4(p.AB[q].x, p.AB[q].y, p.GS[q].x, p.GS[q].y);
   }
   const TileSmem sm = carve_smem(smraw, p.tile_cap, true);
   const unsigned cur = p.ctl->cur;
@@ -1765,7 +1769,7 @@ __global__ void __launch_bounds__(TILE_TPB, MINB) k_force(const DevP p) {
     const float4 xi = sm.spos[li];
     const unsigned wi = f2u(xi.w);
     const unsigned tagi = wi & TAG_MASK;
-    const float2* const ab = s_ab + (MULTI ? ((wi >> TAG_BITS) & (MAXTYPES - 1u)) * MAXTYPES : 0u);
+    const float4* const ab = s_ab + (MULTI ? ((wi >> TAG_BITS) & (MAXTYPES - 1u)) * MAXTYPES : 0u);
     const float4 vi = sm.svel[li];
     const unsigned na = rec.y;
     ForceAcc acc = {0.f, 0.f, 0.f};
@@ -2022,6 +2026,8 @@ struct mdpd_ctx {
   bool has_wall = false;  // some particle is frozen (type 1)
   unsigned ntypes = 0, frozen_mask = 0;        // mdpd_set_pair_params
   float pairA[MAXTYPES * MAXTYPES] = {}, pairB[MAXTYPES * MAXTYPES] = {};
+  bool have_gs = false;                        // mdpd_set_pair_gamma_sigma
+  float pairG[MAXTYPES * MAXTYPES] = {}, pairS[MAXTYPES * MAXTYPES] = {};
   uint64_t launches = 0;         // kernels launched directly (graph replays are added from graph_steps / ctl)
   uint64_t host_step = 0;
   cudaStream_t ls = nullptr;     // stream the LAUNCH macro targets (the handle's stream, or the capture stream)
@@ -2169,6 +2175,10 @@ void fill_physics(mdpd_ctx* h) {
     for (unsigned b = 0; b < MAXTYPES; ++b) {
       const bool in = a < h->ntypes && b < h->ntypes;
       d.AB[a * MAXTYPES + b] = make_float2(in ? h->pairA[a * h->ntypes + b] : p.A, in ? h->pairB[a * h->ntypes + b] : p.B);
+      const bool gs = in && h->have_gs;
+      const double sg = gs ? (double)h->pairS[a * h->ntypes + b] : (double)p.sigma;
+      d.GS[a * MAXTYPES + b] = make_float2(gs ? h->pairG[a * h->ntypes + b] : p.gamma,
+                                           (float)(sg * std::sqrt(3.0) * std::ldexp(1.0, -23) / std::sqrt((double)p.dt)));
     }
 }
 
@@ -2231,38 +2241,42 @@ bool choose_blocks(mdpd_ctx* h, unsigned max_own) {
 // Every kernel that stages a tile in dynamic shared memory.  The opt-in to more than 48 KB belongs to the FUNCTION on the
 // device, not to a handle: were it set to each handle's own size, the load of a second handle with smaller tiles would
 // lower it under the first handle's launches ("invalid argument").  So every function is opened to the device's limit
-// minus its own static shared memory (the mbarrier of stage_bulk, the (A, B) table of k_force), whoever loads.
+// minus its own static shared memory (the mbarrier of stage_bulk, the pair-parameter table of k_force), whoever loads.
 #define MDPD_UNPAREN(...) __VA_ARGS__
 #define MDPD_TILE_KERNELS(X)                                                                                            \
-  X((k_cells<0, false, false>)) \
-  X((k_cells<1, false, false>)) \
-  X((k_cells<1, true, false>)) \
-  X((k_cells<1, true, true>)) \
-  X((k_density<true, true, DENS_TPB>)) \
-  X((k_density<true, false, DENS_TPB>)) \
-  X((k_density<false, false, DENS_TPB>)) \
-  X((k_density<true, true, DENS_TPB2>)) \
-  X((k_density<true, false, DENS_TPB2>)) \
-  X((k_density<false, false, DENS_TPB2>)) \
-  X((k_pairs)) \
-  X((k_force<true, false>)) \
-  X((k_force<false, false>)) \
-  X((k_force<true, true>)) \
-  X((k_force<true, false, false, true>)) \
-  X((k_force<false, false, false, true>)) \
-  X((k_force<true, true, true>)) \
-  X((k_force<true, false, true>)) \
-  X((k_force<false, true>))
+  X((k_cells<0, false, false>), false) \
+  X((k_cells<1, false, false>), false) \
+  X((k_cells<1, true, false>), false) \
+  X((k_cells<1, true, true>), false) \
+  X((k_density<true, true, DENS_TPB>), false) \
+  X((k_density<true, false, DENS_TPB>), false) \
+  X((k_density<false, false, DENS_TPB>), false) \
+  X((k_density<true, true, DENS_TPB2>), false) \
+  X((k_density<true, false, DENS_TPB2>), false) \
+  X((k_density<false, false, DENS_TPB2>), false) \
+  X((k_pairs), false) \
+  X((k_force<true, false>), false) \
+  X((k_force<false, false>), false) \
+  X((k_force<true, true>), true) \
+  X((k_force<true, false, false, true>), false) \
+  X((k_force<false, false, false, true>), false) \
+  X((k_force<true, true, true>), true) \
+  X((k_force<true, false, true>), false) \
+  X((k_force<false, true>), true)
 
-// Largest static shared memory of any tile kernel: what the capacity search has to leave free beside the dynamic part.
-cudaError_t tile_static_smem(size_t* out) {
+// Largest static shared memory of any tile kernel this handle can launch (the per-type-pair instantiations of the force
+// pass, with their 1 KB parameter table, only when species are in use): what the capacity search has to leave free
+// beside the dynamic part.
+cudaError_t tile_static_smem(bool species, size_t* out) {
   size_t m = 0;
   cudaFuncAttributes a;
   cudaError_t e;
-#define X(fn)                                                      \
-  e = cudaFuncGetAttributes(&a, (const void*)(MDPD_UNPAREN fn));  \
-  if (e != cudaSuccess) return e;                                  \
-  m = std::max(m, a.sharedSizeBytes);
+#define X(fn, multi)                                                 \
+  if (species || !(multi)) {                                         \
+    e = cudaFuncGetAttributes(&a, (const void*)(MDPD_UNPAREN fn));  \
+    if (e != cudaSuccess) return e;                                  \
+    m = std::max(m, a.sharedSizeBytes);                              \
+  }
   MDPD_TILE_KERNELS(X)
 #undef X
   *out = m;
@@ -2272,7 +2286,7 @@ cudaError_t tile_static_smem(size_t* out) {
 cudaError_t allow_tile_smem(mdpd_ctx* h) {
   cudaFuncAttributes a;
   cudaError_t e;
-#define X(fn)                                                                                                          \
+#define X(fn, multi)                                                                                                   \
   e = cudaFuncGetAttributes(&a, (const void*)(MDPD_UNPAREN fn));                                                      \
   if (e != cudaSuccess) return e;                                                                                      \
   e = cudaFuncSetAttribute((const void*)(MDPD_UNPAREN fn), cudaFuncAttributeMaxDynamicSharedMemorySize,               \
@@ -2524,6 +2538,7 @@ int mdpd_set_pair_params(mdpd_ctx* h, uint32_t ntypes, const float* A, const flo
         return set_err(h, MDPD_EINVAL, "A and B must be symmetric");
   if (h->loaded && (ntypes != h->ntypes || frozen_mask != h->frozen_mask))
     return set_err(h, MDPD_ESTATE, "the number of species and the frozen set are fixed by load_particles");
+  if (ntypes != h->ntypes) h->have_gs = false;  // the amplitude matrices belong to a species set
   h->ntypes = ntypes;
   h->frozen_mask = frozen_mask;
   for (uint32_t q = 0; q < ntypes * ntypes; ++q) {
@@ -2544,6 +2559,35 @@ size_t mdpd_workspace_bytes(const mdpd_params* p, uint64_t n, int has_mask, cons
   Layout L;
   if (!make_layout(*p, n, has_mask, mask_dims, L, nullptr)) return 0;
   return L.total;
+}
+
+int mdpd_set_pair_gamma_sigma(mdpd_ctx* h, uint32_t ntypes, const float* gamma, const float* sigma) {
+  if (!h) return MDPD_EINVAL;
+  if (!gamma || !sigma) {
+    h->have_gs = false;
+  } else {
+    if (ntypes == 0 || ntypes != h->ntypes)
+      return set_err(h, MDPD_EINVAL, "gamma / sigma matrices need the species set of mdpd_set_pair_params (ntypes = %u there)", h->ntypes);
+    for (uint32_t a = 0; a < ntypes; ++a)
+      for (uint32_t b = 0; b <= a; ++b) {
+        if (gamma[a * ntypes + b] != gamma[b * ntypes + a] || sigma[a * ntypes + b] != sigma[b * ntypes + a])
+          return set_err(h, MDPD_EINVAL, "gamma and sigma must be symmetric");
+        if (!(gamma[a * ntypes + b] >= 0.0f) || !(sigma[a * ntypes + b] >= 0.0f))
+          return set_err(h, MDPD_EINVAL, "gamma and sigma must be >= 0");
+      }
+    for (uint32_t q = 0; q < ntypes * ntypes; ++q) {
+      h->pairG[q] = gamma[q];
+      h->pairS[q] = sigma[q];
+    }
+    h->have_gs = true;
+  }
+  if (h->loaded) {  // new values between steps: like mdpd_set_params
+    CU_TRY(h, cudaSetDevice(h->device));
+    if (h->pending_B) finalize_kick(h);
+    fill_physics(h);
+    h->graph_dirty = true;
+  }
+  return MDPD_OK;
 }
 
 int mdpd_set_workspace(mdpd_ctx* h, void* dev_ptr, size_t bytes) {
@@ -2663,7 +2707,7 @@ int mdpd_load_particles(mdpd_ctx* h, uint64_t n, const float* pos, const float* 
     }
     // fixed part of a tile kernel's shared memory: tables of the staged image + the largest static allocation of any of them
     size_t stat = 0;
-    CU_TRY(h, tile_static_smem(&stat));
+    CU_TRY(h, tile_static_smem(h->ntypes != 0, &stat));
     const size_t fixed = tile_smem_bytes(0, true, 0) + stat;
     // capacity of a tile + halo in staged slots: what the force pass can hold in shared memory, what a 16-bit list entry can
     // address, and what the item list of stage_fast (2 * HTAB items: 3 * 36 runs + one item per 32 slots) can describe
