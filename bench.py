@@ -255,7 +255,7 @@ def main_ours(args, rank, world, local):
     import paper_1903_10134_b200 as pk
     from paper_1903_10134_b200.build import build as build_cuda
     if rank == 0:
-        build_cuda()
+        build_cuda(defines=tuple(args.define))   # measurement builds: --define=-DMDPD_FIRST_TILE=1 (printed as build_flags)
     if world > 1:
         dist.barrier()
 
@@ -546,6 +546,7 @@ def main():
     ap.add_argument("--tma", action="store_true", help="both tile passes stage with cp.async.bulk (MDPD_FLAG_TMA_STAGING)")
     ap.add_argument("--cpasync", action="store_true", help="both tile passes stage with cp.async (MDPD_FLAG_CPASYNC_STAGING)")
     ap.add_argument("--no-graph", action="store_true", help="launch the kernels one by one (MDPD_FLAG_NO_GRAPH; for ncu)")
+    ap.add_argument("--define", action="append", default=[], help="extra -D option of a measurement build of the library, e.g. --define=-DMDPD_FIRST_TILE=1")
     ap.add_argument("--skin", type=float, default=None, help="override the Verlet-list skin (default: the config's 0.25)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
